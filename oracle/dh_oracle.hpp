@@ -1,0 +1,494 @@
+// ORACLE — test infrastructure only.
+//
+// Plain, slow, obviously-correct CPU implementation of the hot path of arxiv/paper_2512_13403
+// ("diffhydro"): one explicit step of the 3D compressible Euler finite-volume update on a uniform
+// periodic Cartesian grid, its CFL time step, the optional pointwise cooling source, and the
+// discrete adjoint (VJP) of the step.  Written from PAPER.md; it shares no code with the CUDA path
+// under paper_2512_13403_b200/ and neither imports the other.  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may build, load or call anything in oracle/.
+//
+// Everything is templated on the scalar type S so that the *same* literal transcription of the
+// scheme runs on double (forward), on dual numbers (exact JVP, and local Jacobians for the VJP)
+// and on float (the dt recipe, which must be reproduced bit-for-bit by the GPU).
+//
+// Citations are PAPER.md:<line> (section / equation).  Readings of silent or ambiguous points are
+// the A1..A16 rows of SURVEY.md §8(c); they are restated in DESIGN.md.
+//
+// Layout: U[f][k][j][i], f in {0:rho, 1:rho*vx, 2:rho*vy, 3:rho*vz, 4:E}  (Eq. 2;
+// PAPER.md:96-104), i (x) fastest, periodic in all three directions.
+#pragma once
+#include <cmath>
+#include <cstddef>
+#include <vector>
+
+namespace dho {
+
+// ------------------------------------------------------------------------------------------------
+// Parameters (plain C struct; mirrored field by field in oracle/oracle.py)
+// ------------------------------------------------------------------------------------------------
+struct Params {
+  double gamma;       // adiabatic index
+  double dx[3];       // cell sizes Delta x_a (Eq. A4)
+  double rho_floor;   // floors used only inside prim() (reading A6)
+  double p_floor;
+  int limiter;        // 0 minmod (A4), 1 van Leer, 2 MC, 3 piecewise-constant
+  int riemann;        // 0 HLLC, 1 HLL, 2 Rusanov/LF
+  int integrator;     // 0 predictor/corrector A6-A7, 1 Heun
+  int cooling;        // 0 off, 1 on: Eq. 23 with N_sub=1, reading A9
+  double lambda0;     // Lambda(T) = lambda0 * T^alpha (reading A10)
+  double alpha;
+  double t_floor;     // temperature floor, Eq. 24 with R=1
+};
+
+// ------------------------------------------------------------------------------------------------
+// Dual numbers with N derivative slots (forward-mode AD; exact to rounding)
+// ------------------------------------------------------------------------------------------------
+template <int N>
+struct Dual {
+  double v;
+  double d[N];
+  Dual() : v(0.0) { for (int i = 0; i < N; ++i) d[i] = 0.0; }
+  Dual(double x) : v(x) { for (int i = 0; i < N; ++i) d[i] = 0.0; }
+};
+
+template <int N> inline Dual<N> operator+(const Dual<N>& a, const Dual<N>& b) { Dual<N> r; r.v = a.v + b.v; for (int i = 0; i < N; ++i) r.d[i] = a.d[i] + b.d[i]; return r; }
+template <int N> inline Dual<N> operator-(const Dual<N>& a, const Dual<N>& b) { Dual<N> r; r.v = a.v - b.v; for (int i = 0; i < N; ++i) r.d[i] = a.d[i] - b.d[i]; return r; }
+template <int N> inline Dual<N> operator-(const Dual<N>& a) { Dual<N> r; r.v = -a.v; for (int i = 0; i < N; ++i) r.d[i] = -a.d[i]; return r; }
+template <int N> inline Dual<N> operator*(const Dual<N>& a, const Dual<N>& b) { Dual<N> r; r.v = a.v * b.v; for (int i = 0; i < N; ++i) r.d[i] = a.d[i] * b.v + a.v * b.d[i]; return r; }
+template <int N> inline Dual<N> operator/(const Dual<N>& a, const Dual<N>& b) { Dual<N> r; r.v = a.v / b.v; for (int i = 0; i < N; ++i) r.d[i] = (a.d[i] - r.v * b.d[i]) / b.v; return r; }
+template <int N> inline Dual<N> operator+(const Dual<N>& a, double b) { Dual<N> r = a; r.v += b; return r; }
+template <int N> inline Dual<N> operator+(double a, const Dual<N>& b) { return b + a; }
+template <int N> inline Dual<N> operator-(const Dual<N>& a, double b) { Dual<N> r = a; r.v -= b; return r; }
+template <int N> inline Dual<N> operator-(double a, const Dual<N>& b) { return (-b) + a; }
+template <int N> inline Dual<N> operator*(const Dual<N>& a, double b) { Dual<N> r; r.v = a.v * b; for (int i = 0; i < N; ++i) r.d[i] = a.d[i] * b; return r; }
+template <int N> inline Dual<N> operator*(double a, const Dual<N>& b) { return b * a; }
+template <int N> inline Dual<N> operator/(const Dual<N>& a, double b) { Dual<N> r; r.v = a.v / b; for (int i = 0; i < N; ++i) r.d[i] = a.d[i] / b; return r; }
+template <int N> inline Dual<N> operator/(double a, const Dual<N>& b) { return Dual<N>(a) / b; }
+
+// value of a scalar (the quantity every branch looks at: the a.e. derivative follows the branch
+// actually taken, reading A7)
+inline double val(double a) { return a; }
+inline double val(float a) { return (double)a; }
+template <int N> inline double val(const Dual<N>& a) { return a.v; }
+
+inline double ssqrt(double a) { return std::sqrt(a); }
+inline float ssqrt(float a) { return std::sqrt(a); }
+template <int N> inline Dual<N> ssqrt(const Dual<N>& a) { Dual<N> r; r.v = std::sqrt(a.v); for (int i = 0; i < N; ++i) r.d[i] = a.d[i] / (2.0 * r.v); return r; }
+
+inline double spow(double a, double p) { return std::pow(a, p); }
+template <int N> inline Dual<N> spow(const Dual<N>& a, double p) { Dual<N> r; r.v = std::pow(a.v, p); double g = (a.v > 0.0) ? p * std::pow(a.v, p - 1.0) : 0.0; for (int i = 0; i < N; ++i) r.d[i] = g * a.d[i]; return r; }
+
+// min/max: ties -> first argument (reading A7)
+template <class S> inline S smax(const S& a, const S& b) { return (val(a) >= val(b)) ? a : b; }
+template <class S> inline S smin(const S& a, const S& b) { return (val(a) <= val(b)) ? a : b; }
+template <class S> inline S sabs(const S& a) { return (val(a) >= 0.0) ? a : S(-a); }
+
+// ------------------------------------------------------------------------------------------------
+// Step 1 — primitive conversion  W = (rho, v, P),  P = (gamma-1)(E - rho|v|^2/2)   (
+// PAPER.md:811).  Floors act only here, conserved arrays are never modified (reading A6).
+// ------------------------------------------------------------------------------------------------
+template <class S>
+inline void prim(const S U[5], const Params& p, S W[5]) {
+  S rho = smax(U[0], S(p.rho_floor));
+  W[0] = rho;
+  W[1] = U[1] / rho;
+  W[2] = U[2] / rho;
+  W[3] = U[3] / rho;
+  S m2 = U[1] * U[1] + U[2] * U[2] + U[3] * U[3];
+  S P = (p.gamma - 1.0) * (U[4] - 0.5 * m2 / rho);
+  W[4] = smax(P, S(p.p_floor));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step 2 — slope limiters for Eq. A1; the menu is PAPER.md:820, formulas are the
+// textbook ones (reading A4).  a = W_{i+1}-W_i, b = W_i-W_{i-1}.
+// ------------------------------------------------------------------------------------------------
+template <class S>
+inline S limiter(const S& a, const S& b, int kind) {
+  if (kind == 3) return S(0.0);                      // piecewise constant
+  if (val(a) * val(b) <= 0.0) return S(0.0);         // extremum: zero slope (all limiters)
+  if (kind == 0) {                                   // minmod; |a|==|b| -> a (A7)
+    return (std::fabs(val(a)) <= std::fabs(val(b))) ? a : b;
+  } else if (kind == 1) {                            // van Leer: harmonic mean
+    return 2.0 * a * b / (a + b);
+  } else {                                           // MC: minmod(2a, 2b, (a+b)/2)
+    S c = 0.5 * (a + b);
+    S a2 = 2.0 * a, b2 = 2.0 * b;
+    S m = (std::fabs(val(a2)) <= std::fabs(val(b2))) ? a2 : b2;
+    return (std::fabs(val(m)) <= std::fabs(val(c))) ? m : c;
+  }
+}
+
+// Euler flux along axis ax of a primitive state, and its conserved vector.
+template <class S>
+inline void phys_flux(const S W[5], int ax, double gamma, S Ucons[5], S F[5]) {
+  S rho = W[0], P = W[4];
+  S un = W[1 + ax];
+  S E = P / (gamma - 1.0) + 0.5 * rho * (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+  Ucons[0] = rho;
+  Ucons[1] = rho * W[1];
+  Ucons[2] = rho * W[2];
+  Ucons[3] = rho * W[3];
+  Ucons[4] = E;
+  F[0] = rho * un;
+  F[1] = rho * un * W[1];
+  F[2] = rho * un * W[2];
+  F[3] = rho * un * W[3];
+  F[1 + ax] = F[1 + ax] + P;
+  F[4] = un * (E + P);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step 3 — Riemann flux at a face from left/right primitive states.
+// Wave speeds: Eq. A3, c_s^2 = gamma P / rho.  The rest of HLLC is
+// not printed in the paper (it defers to HL25); textbook HLLC with the pressure-based contact
+// speed and the F_K + S_K (U*_K - U_K) form is used (reading A3).  Select order and >=/<= as in
+// SURVEY.md §8(c) step 3 (reading A7).
+// ------------------------------------------------------------------------------------------------
+template <class S>
+inline void riemann(const S L[5], const S R[5], int ax, const Params& p, S F[5]) {
+  const double g = p.gamma;
+  S uL = L[1 + ax], uR = R[1 + ax];
+  S cL = ssqrt(g * L[4] / L[0]);
+  S cR = ssqrt(g * R[4] / R[0]);
+  S SL = smin(S(uL - cL), S(uR - cR));   // Eq. A3
+  S SR = smax(S(uL + cL), S(uR + cR));
+  S UL[5], UR[5], FL[5], FR[5];
+  phys_flux(L, ax, g, UL, FL);
+  phys_flux(R, ax, g, UR, FR);
+
+  if (p.riemann == 2) {  // Rusanov / local Lax-Friedrichs
+    S a = smax(sabs(SL), sabs(SR));
+    for (int f = 0; f < 5; ++f) F[f] = 0.5 * (FL[f] + FR[f]) - 0.5 * a * (UR[f] - UL[f]);
+    return;
+  }
+  if (val(SL) >= 0.0) { for (int f = 0; f < 5; ++f) F[f] = FL[f]; return; }
+  if (val(SR) <= 0.0) { for (int f = 0; f < 5; ++f) F[f] = FR[f]; return; }
+  if (p.riemann == 1) {  // two-wave HLL
+    for (int f = 0; f < 5; ++f) F[f] = (SR * FL[f] - SL * FR[f] + SL * SR * (UR[f] - UL[f])) / (SR - SL);
+    return;
+  }
+  // HLLC
+  S rhoL = L[0], rhoR = R[0], PL = L[4], PR = R[4];
+  S Sstar = (PR - PL + rhoL * uL * (SL - uL) - rhoR * uR * (SR - uR)) /
+            (rhoL * (SL - uL) - rhoR * (SR - uR));
+  const bool left = (val(Sstar) >= 0.0);
+  const S* W = left ? L : R;
+  const S* UK = left ? UL : UR;
+  const S* FK = left ? FL : FR;
+  S SK = left ? SL : SR;
+  S rhoK = W[0], uK = W[1 + ax], PK = W[4];
+  S fac = rhoK * (SK - uK) / (SK - Sstar);
+  S Ustar[5];
+  Ustar[0] = fac;
+  Ustar[1] = fac * W[1];
+  Ustar[2] = fac * W[2];
+  Ustar[3] = fac * W[3];
+  Ustar[1 + ax] = fac * Sstar;
+  Ustar[4] = fac * (UK[4] / rhoK + (Sstar - uK) * (Sstar + PK / (rhoK * (SK - uK))));
+  for (int f = 0; f < 5; ++f) F[f] = FK[f] + SK * (Ustar[f] - UK[f]);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Steps 2+3 for one face i+1/2 from the four cells i-1, i, i+1, i+2 along the axis:
+// Delta W_i = lim(W_{i+1}-W_i, W_i-W_{i-1})                        (Eq. A1)
+// W^L = W_i + Delta W_i / 2,  W^R = W_{i+1} - Delta W_{i+1} / 2    (Eq. A2)
+// ------------------------------------------------------------------------------------------------
+template <class S>
+inline void face_states(const S Wm1[5], const S W0[5], const S Wp1[5], const S Wp2[5],
+                        const Params& p, S WL[5], S WR[5]) {
+  for (int c = 0; c < 5; ++c) {
+    S d0 = limiter(S(Wp1[c] - W0[c]), S(W0[c] - Wm1[c]), p.limiter);
+    S d1 = limiter(S(Wp2[c] - Wp1[c]), S(Wp1[c] - W0[c]), p.limiter);
+    WL[c] = W0[c] + 0.5 * d0;
+    WR[c] = Wp1[c] - 0.5 * d1;
+  }
+}
+
+template <class S>
+inline void face_flux(const S Wm1[5], const S W0[5], const S Wp1[5], const S Wp2[5], int ax,
+                      const Params& p, S F[5]) {
+  S WL[5], WR[5];
+  face_states(Wm1, W0, Wp1, Wp2, p, WL, WR);
+  riemann(WL, WR, ax, p, F);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step 6 — pointwise cooling, Eq. 23 with N_sub = 1 and the floor of Eq. 24,
+// applied once after the hydro update and changing only E.  Code units n = rho,
+// T = P/rho, Gamma = 0, Lambda = lambda0 T^alpha (reading A10).
+// ------------------------------------------------------------------------------------------------
+template <class S>
+inline void cool(const S U[5], double dt, const Params& p, S out[5]) {
+  S rho = U[0];
+  S Ek = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
+  S Eth = U[4] - Ek;
+  S T = (p.gamma - 1.0) * Eth / rho;
+  S Tpos = smax(T, S(0.0));
+  S Edot = -1.0 * rho * rho * p.lambda0 * spow(Tpos, p.alpha);
+  S Efloor = rho * p.t_floor / (p.gamma - 1.0);
+  S Eth1 = smax(Efloor, S(Eth + Edot * dt));
+  out[0] = U[0]; out[1] = U[1]; out[2] = U[2]; out[3] = U[3];
+  out[4] = Ek + Eth1;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Grid helpers
+// ------------------------------------------------------------------------------------------------
+struct Grid {
+  int n[3];  // nx, ny, nz
+  size_t N() const { return (size_t)n[0] * n[1] * n[2]; }
+  size_t idx(int i, int j, int k) const { return ((size_t)k * n[1] + j) * n[0] + i; }
+};
+inline int wrap(int i, int n) { i %= n; return i < 0 ? i + n : i; }
+
+// neighbour of cell (i,j,k) shifted by s cells along axis ax (periodic)
+inline size_t shifted(const Grid& g, int i, int j, int k, int ax, int s) {
+  int c[3] = {i, j, k};
+  c[ax] = wrap(c[ax] + s, g.n[ax]);
+  return g.idx(c[0], c[1], c[2]);
+}
+
+template <class S>
+void compute_prims(const Grid& g, const Params& p, const S* U, S* W) {
+  const size_t N = g.N();
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    S u[5], w[5];
+    for (int f = 0; f < 5; ++f) u[f] = U[f * N + c];
+    prim(u, p, w);
+    for (int f = 0; f < 5; ++f) W[f * N + c] = w[f];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step 4 — D(U)_i = sum_a (F_{a,i+1/2} - F_{a,i-1/2}) / dx_a      (Eq. A4, PAPER.md:849;
+// roll direction: reading A5).  Natural loop nest with a face-flux array per axis.
+// ------------------------------------------------------------------------------------------------
+template <class S>
+void flux_divergence(const Grid& g, const Params& p, const S* U, S* D) {
+  const size_t N = g.N();
+  std::vector<S> W(5 * N), F(5 * N);
+  compute_prims(g, p, U, W.data());
+  for (size_t c = 0; c < 5 * N; ++c) D[c] = S(0.0);
+  for (int ax = 0; ax < 3; ++ax) {
+    // F[.][cell i] holds the flux through the face i+1/2 along ax
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          size_t cm1 = shifted(g, i, j, k, ax, -1), c0 = g.idx(i, j, k);
+          size_t cp1 = shifted(g, i, j, k, ax, +1), cp2 = shifted(g, i, j, k, ax, +2);
+          S a[5], b[5], c[5], d[5], f[5];
+          for (int q = 0; q < 5; ++q) { a[q] = W[q * N + cm1]; b[q] = W[q * N + c0]; c[q] = W[q * N + cp1]; d[q] = W[q * N + cp2]; }
+          face_flux(a, b, c, d, ax, p, f);
+          for (int q = 0; q < 5; ++q) F[q * N + c0] = f[q];
+        }
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          size_t c0 = g.idx(i, j, k), cm1 = shifted(g, i, j, k, ax, -1);
+          for (int q = 0; q < 5; ++q) D[q * N + c0] = D[q * N + c0] + (F[q * N + c0] - F[q * N + cm1]) / p.dx[ax];
+        }
+  }
+}
+
+template <class S>
+void apply_cooling(const Grid& g, const Params& p, double dt, S* U) {
+  const size_t N = g.N();
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    S u[5], o[5];
+    for (int f = 0; f < 5; ++f) u[f] = U[f * N + c];
+    cool(u, dt, p, o);
+    U[4 * N + c] = o[4];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Step 5 — one full time step.
+// integrator 0 (default, reading A1/A2): U* = U^n - dt/2 D(U^n);  U^{n+1} = U^n - dt D(U*)
+//                                        (Eqs. A6-A7 form, applied unsplit, Eq. A4)
+// integrator 1: Heun RK2: U1 = U^n - dt D(U^n);  U^{n+1} = (U^n + U1 - dt D(U1)) / 2
+// then cooling once (reading A8).
+// ------------------------------------------------------------------------------------------------
+template <class S>
+void step(const Grid& g, const Params& p, const S* U, double dt, S* Uout) {
+  const size_t M = 5 * g.N();
+  std::vector<S> D(M), Us(M);
+  flux_divergence(g, p, U, D.data());
+  if (p.integrator == 0) {
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - (0.5 * dt) * D[c];
+    flux_divergence(g, p, Us.data(), D.data());
+    for (size_t c = 0; c < M; ++c) Uout[c] = U[c] - dt * D[c];
+  } else {
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];
+    flux_divergence(g, p, Us.data(), D.data());
+    for (size_t c = 0; c < M; ++c) Uout[c] = 0.5 * (U[c] + (Us[c] - dt * D[c]));
+  }
+  if (p.cooling) apply_cooling(g, p, dt, Uout);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Reverse mode, scatter form (SURVEY.md §8(c) "VJP", dt held constant:
+// PAPER.md:876, reading A12).
+//
+// One stage V = B - tau D(U) with cotangent g on V.  This routine ADDS  -tau J_D(U)^T g  to Ubar.
+// Per axis and face i+1/2 the flux cotangent is lambda = (tau/dx_a)(g_{i+1} - g_i); the local
+// 5x20 Jacobian of face_flux w.r.t. (W_{i-1}, W_i, W_{i+1}, W_{i+2}) is obtained exactly (to
+// rounding) with 20-slot dual numbers through the same face_flux as the forward pass, and its
+// transpose times lambda is scattered into Wbar of those four cells.  Finally
+// Ubar_i += (dW/dU)_i^T Wbar_i with 5-slot duals through prim().
+// ------------------------------------------------------------------------------------------------
+inline void stage_vjp_accumulate(const Grid& g, const Params& p, const double* U, double tau,
+                                 const double* gV, double* Ubar) {
+  const size_t N = g.N();
+  std::vector<double> W(5 * N), Wbar(5 * N, 0.0);
+  compute_prims(g, p, U, W.data());
+  for (int ax = 0; ax < 3; ++ax) {
+    // rows along `ax` are independent of each other: parallelise over an outer index that is
+    // not the scatter direction
+    const int o1 = (ax == 2) ? 1 : 2;  // outer loop axis
+    const int o2 = (ax == 0) ? 1 : 0;  // middle loop axis (the remaining one)
+#pragma omp parallel for schedule(static)
+    for (int a = 0; a < g.n[o1]; ++a)
+      for (int b = 0; b < g.n[o2]; ++b)
+        for (int s = 0; s < g.n[ax]; ++s) {
+          int c[3];
+          c[o1] = a; c[o2] = b; c[ax] = s;
+          const int i = c[0], j = c[1], k = c[2];
+          size_t cell[4] = {shifted(g, i, j, k, ax, -1), g.idx(i, j, k), shifted(g, i, j, k, ax, +1),
+                            shifted(g, i, j, k, ax, +2)};
+          double lam[5];
+          for (int q = 0; q < 5; ++q) lam[q] = (tau / p.dx[ax]) * (gV[q * N + cell[2]] - gV[q * N + cell[1]]);
+          Dual<20> w[4][5], f[5];
+          for (int m = 0; m < 4; ++m)
+            for (int q = 0; q < 5; ++q) { w[m][q] = Dual<20>(W[q * N + cell[m]]); w[m][q].d[m * 5 + q] = 1.0; }
+          face_flux(w[0], w[1], w[2], w[3], ax, p, f);
+          for (int m = 0; m < 4; ++m)
+            for (int q = 0; q < 5; ++q) {
+              double acc = 0.0;
+              for (int r = 0; r < 5; ++r) acc += f[r].d[m * 5 + q] * lam[r];
+              Wbar[q * N + cell[m]] += acc;
+            }
+        }
+  }
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    Dual<5> u[5], w[5];
+    for (int q = 0; q < 5; ++q) { u[q] = Dual<5>(U[q * N + c]); u[q].d[q] = 1.0; }
+    prim(u, p, w);
+    for (int q = 0; q < 5; ++q) {
+      double acc = 0.0;
+      for (int r = 0; r < 5; ++r) acc += w[r].d[q] * Wbar[r * N + c];
+      Ubar[q * N + c] += acc;
+    }
+  }
+}
+
+// cotangent through the cooling update at U1 (the pre-cooling state): gbar = J_cool(U1)^T g
+inline void cooling_vjp(const Grid& g, const Params& p, double dt, const double* U1, const double* gout,
+                        double* gbar) {
+  const size_t N = g.N();
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    Dual<5> u[5], o[5];
+    for (int q = 0; q < 5; ++q) { u[q] = Dual<5>(U1[q * N + c]); u[q].d[q] = 1.0; }
+    cool(u, dt, p, o);
+    for (int q = 0; q < 5; ++q) {
+      double acc = 0.0;
+      for (int r = 0; r < 5; ++r) acc += o[r].d[q] * gout[r * N + c];
+      gbar[q * N + c] = acc;
+    }
+  }
+}
+
+// VJP of the full step: g_in = (dU^{n+1}/dU^n)^T g_out.
+inline void step_vjp(const Grid& g, const Params& p, const double* U, double dt, const double* gout,
+                     double* gin) {
+  const size_t M = 5 * g.N();
+  std::vector<double> D(M), Us(M), g1(M), gs(M, 0.0);
+  flux_divergence(g, p, U, D.data());
+  if (p.integrator == 0) {
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - (0.5 * dt) * D[c];
+    if (p.cooling) {
+      std::vector<double> U1(M);
+      flux_divergence(g, p, Us.data(), D.data());
+      for (size_t c = 0; c < M; ++c) U1[c] = U[c] - dt * D[c];
+      cooling_vjp(g, p, dt, U1.data(), gout, g1.data());
+    } else {
+      for (size_t c = 0; c < M; ++c) g1[c] = gout[c];
+    }
+    // U1 = U - dt D(U*):  Ubar += g1,  U*bar += -dt J_D(U*)^T g1
+    stage_vjp_accumulate(g, p, Us.data(), dt, g1.data(), gs.data());
+    // U* = U - dt/2 D(U):  Ubar += U*bar - dt/2 J_D(U)^T U*bar
+    for (size_t c = 0; c < M; ++c) gin[c] = g1[c] + gs[c];
+    stage_vjp_accumulate(g, p, U, 0.5 * dt, gs.data(), gin);
+  } else {
+    // Heun: Ua = U - dt D(U); U1 = (U + Ua - dt D(Ua)) / 2
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];
+    if (p.cooling) {
+      std::vector<double> U1(M);
+      flux_divergence(g, p, Us.data(), D.data());
+      for (size_t c = 0; c < M; ++c) U1[c] = 0.5 * (U[c] + (Us[c] - dt * D[c]));
+      cooling_vjp(g, p, dt, U1.data(), gout, g1.data());
+    } else {
+      for (size_t c = 0; c < M; ++c) g1[c] = gout[c];
+    }
+    std::vector<double> h(M);
+    for (size_t c = 0; c < M; ++c) { h[c] = 0.5 * g1[c]; gs[c] = h[c]; }   // Uabar = g1/2 + ...
+    stage_vjp_accumulate(g, p, Us.data(), dt, h.data(), gs.data());       // ... - dt J_D(Ua)^T g1/2
+    for (size_t c = 0; c < M; ++c) gin[c] = h[c] + gs[c];                  // Ubar = g1/2 + Uabar ...
+    stage_vjp_accumulate(g, p, U, dt, gs.data(), gin);                     // ... - dt J_D(U)^T Uabar
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// CFL time step, Eq. A8:  dt = C min_a dx_a / max_cells(|v_a| + c_s).
+// The "dt recipe" of SURVEY.md §8(c): every operation in T, in exactly this order, no FMA
+// contraction (this file is compiled with -ffp-contract=off), constants formed in double and
+// rounded to T once.  Returns 0, or -4 if any input or wave speed is not finite.
+// ------------------------------------------------------------------------------------------------
+template <class T>
+int cfl_dt(const Grid& g, const Params& p, double cfl, const T* U, double* dt_out, double smax_out[3]) {
+  const size_t N = g.N();
+  const T gam = (T)p.gamma, gm1 = (T)(p.gamma - 1.0);
+  const T rfl = (T)p.rho_floor, pfl = (T)p.p_floor, half = (T)0.5;
+  T Smax[3] = {(T)0, (T)0, (T)0};
+  T S0 = (T)0, S1 = (T)0, S2 = (T)0;
+  int nbad = 0;
+  // max is exact and order-independent, so the thread count cannot change a bit of the result
+#pragma omp parallel for schedule(static) reduction(max : S0, S1, S2) reduction(+ : nbad)
+  for (long long c = 0; c < (long long)N; ++c) {
+    T rho = U[c], mx = U[N + c], my = U[2 * N + c], mz = U[3 * N + c], E = U[4 * N + c];
+    T rt = (rho >= rfl) ? rho : rfl;
+    T vx = mx / rt, vy = my / rt, vz = mz / rt;
+    T q = ((mx * mx) + (my * my)) + (mz * mz);
+    T P = gm1 * (E - half * (q / rt));
+    P = (P >= pfl) ? P : pfl;
+    T cs = std::sqrt((gam * P) / rt);
+    T sx = std::fabs(vx) + cs, sy = std::fabs(vy) + cs, sz = std::fabs(vz) + cs;
+    // the floors (a compare-select) would silently swallow a NaN in rho or E: test the inputs too
+    if (!std::isfinite(rho) || !std::isfinite(mx) || !std::isfinite(my) || !std::isfinite(mz) || !std::isfinite(E) ||
+        !std::isfinite(sx) || !std::isfinite(sy) || !std::isfinite(sz)) nbad += 1;
+    if (sx > S0) S0 = sx;
+    if (sy > S1) S1 = sy;
+    if (sz > S2) S2 = sz;
+  }
+  Smax[0] = S0; Smax[1] = S1; Smax[2] = S2;
+  for (int a = 0; a < 3; ++a) smax_out[a] = (double)Smax[a];
+  if (nbad) return -4;
+  T best = (T)0;
+  bool first = true;
+  for (int a = 0; a < 3; ++a) {
+    T dxa = (T)p.dx[a];
+    T r = dxa / Smax[a];
+    if (first || r < best) { best = r; first = false; }
+  }
+  T dt = (T)cfl * best;
+  *dt_out = (double)dt;
+  return 0;
+}
+
+}  // namespace dho

@@ -1,0 +1,228 @@
+"""ORACLE — test infrastructure only.
+
+ctypes wrapper around ``oracle/dh_oracle.{hpp,cpp}``: the plain CPU implementation of the hot path
+of arxiv/paper_2512_13403 (one periodic 3D Euler finite-volume step, its CFL dt, cooling and VJP),
+written from PAPER.md (citations in the C++ header).  Only ``tests/``, ``__graft_entry__.smoke()``
+and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may import this module; the product
+path (``paper_2512_13403_b200``) never does, and this module never imports the product.
+
+All state arrays are numpy ``[5, nz, ny, nx]`` (rho, rho*vx, rho*vy, rho*vz, E); x is fastest.
+State arithmetic is fp64; the dt recipe runs in the dtype of the array handed in (fp32 or fp64).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = [os.path.join(_HERE, "dh_oracle.cpp"), os.path.join(_HERE, "dh_oracle.hpp")]
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lock = threading.Lock()
+_lib = None
+
+LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2, "constant": 3}
+RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}
+INTEGRATORS = {"vl2": 0, "heun": 1}
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [
+        ("gamma", ctypes.c_double),
+        ("dx", ctypes.c_double * 3),
+        ("rho_floor", ctypes.c_double),
+        ("p_floor", ctypes.c_double),
+        ("limiter", ctypes.c_int),
+        ("riemann", ctypes.c_int),
+        ("integrator", ctypes.c_int),
+        ("cooling", ctypes.c_int),
+        ("lambda0", ctypes.c_double),
+        ("alpha", ctypes.c_double),
+        ("t_floor", ctypes.c_double),
+    ]
+
+
+def build(force: bool = False) -> str:
+    """Compile liboracle.so with g++ (``-ffp-contract=off`` so the dt recipe has no FMA)."""
+    with _lock:
+        stale = force or not os.path.exists(_LIB) or any(
+            os.path.getmtime(s) > os.path.getmtime(_LIB) for s in _SRC
+        )
+        if stale:
+            tmp = _LIB + f".tmp{os.getpid()}"
+            cmd = ["g++", "-std=c++17", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC",
+                   _SRC[0], "-o", tmp]
+            subprocess.run(cmd, check=True, cwd=_HERE)
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB)
+        lib.dho_num_threads.restype = ctypes.c_int
+        lib.dho_limiter.restype = ctypes.c_double
+        lib.dho_limiter.argtypes = [ctypes.c_double, ctypes.c_double, ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().dho_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().dho_set_num_threads(ctypes.c_int(int(n)))
+
+
+def params(gamma=5.0 / 3.0, dx=None, shape=None, rho_floor=1e-10, p_floor=1e-10, limiter="minmod",
+           riemann="hllc", integrator="vl2", cooling=False, lambda0=1e-3, alpha=0.5, t_floor=0.01):
+    """Scheme parameters.  ``dx`` defaults to the unit box, dx_a = 1/n_a (reading A13)."""
+    p = _Params()
+    p.gamma = float(gamma)
+    if dx is None:
+        if shape is None:
+            raise ValueError("give dx=(dx,dy,dz) or shape=(nz,ny,nx)")
+        nz, ny, nx = shape[-3:]
+        dx = (1.0 / nx, 1.0 / ny, 1.0 / nz)
+    p.dx[0], p.dx[1], p.dx[2] = (float(d) for d in dx)
+    p.rho_floor, p.p_floor = float(rho_floor), float(p_floor)
+    p.limiter, p.riemann, p.integrator = LIMITERS[limiter], RIEMANN[riemann], INTEGRATORS[integrator]
+    p.cooling = int(bool(cooling))
+    p.lambda0, p.alpha, p.t_floor = float(lambda0), float(alpha), float(t_floor)
+    return p
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _ptr(a):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _dims(U):
+    assert U.ndim == 4 and U.shape[0] == 5, "state must be [5, nz, ny, nx]"
+    _, nz, ny, nx = U.shape
+    return ctypes.c_int(nx), ctypes.c_int(ny), ctypes.c_int(nz)
+
+
+def cfl_dt(U, p, cfl=0.4):
+    """Eq. A8 in the array's own dtype.  Returns (dt, smax[3]); raises on NaN/Inf."""
+    lib = _load()
+    U = np.ascontiguousarray(U)
+    assert U.dtype in (np.float32, np.float64)
+    dt = ctypes.c_double(0.0)
+    smax = (ctypes.c_double * 3)()
+    rc = lib.dho_cfl_dt(*_dims(U), ctypes.byref(p), ctypes.c_double(cfl),
+                        ctypes.c_int(0 if U.dtype == np.float32 else 1), _ptr(U), ctypes.byref(dt), smax)
+    if rc != 0:
+        raise FloatingPointError("non-finite wave speed")
+    return dt.value, np.array(list(smax))
+
+
+def prims(U, p):
+    lib = _load()
+    U = _f64(U)
+    W = np.empty_like(U)
+    lib.dho_prims(*_dims(U), ctypes.byref(p), _ptr(U), _ptr(W))
+    return W
+
+
+def flux_divergence(U, p):
+    """D(U) of Eq. A4."""
+    lib = _load()
+    U = _f64(U)
+    D = np.empty_like(U)
+    lib.dho_flux_divergence(*_dims(U), ctypes.byref(p), _ptr(U), _ptr(D))
+    return D
+
+
+def step(U, dt, p):
+    """U^n -> U^{n+1}: two stages (+ cooling if p.cooling)."""
+    lib = _load()
+    U = _f64(U)
+    out = np.empty_like(U)
+    lib.dho_step(*_dims(U), ctypes.byref(p), _ptr(U), ctypes.c_double(dt), _ptr(out))
+    return out
+
+
+def step_jvp(U, V, dt, p):
+    """(U^{n+1}, J V) by dual numbers through the same step code."""
+    lib = _load()
+    U, V = _f64(U), _f64(V)
+    out, dout = np.empty_like(U), np.empty_like(U)
+    lib.dho_step_jvp(*_dims(U), ctypes.byref(p), _ptr(U), _ptr(V), ctypes.c_double(dt), _ptr(out), _ptr(dout))
+    return out, dout
+
+
+def step_vjp(U, dt, g_out, p):
+    """g_in = (dU^{n+1}/dU^n)^T g_out, dt held constant."""
+    lib = _load()
+    U, g_out = _f64(U), _f64(g_out)
+    gin = np.empty_like(U)
+    lib.dho_step_vjp(*_dims(U), ctypes.byref(p), _ptr(U), ctypes.c_double(dt), _ptr(g_out), _ptr(gin))
+    return gin
+
+
+def stage_vjp(U, tau, gV, p):
+    """-tau J_D(U)^T gV for one stage V = B - tau D(U)."""
+    lib = _load()
+    U, gV = _f64(U), _f64(gV)
+    gU = np.empty_like(U)
+    lib.dho_stage_vjp(*_dims(U), ctypes.byref(p), _ptr(U), ctypes.c_double(tau), _ptr(gV), _ptr(gU))
+    return gU
+
+
+def cooling(U, dt, p):
+    lib = _load()
+    U = _f64(U)
+    flat = np.ascontiguousarray(U.reshape(5, -1))
+    out = np.empty_like(flat)
+    lib.dho_cooling(ctypes.c_longlong(flat.shape[1]), ctypes.byref(p), ctypes.c_double(dt), _ptr(flat), _ptr(out))
+    return out.reshape(U.shape)
+
+
+def riemann(WL, WR, axis, p):
+    """Batch of Riemann fluxes; WL, WR are [5, n] primitive (rho, vx, vy, vz, P)."""
+    lib = _load()
+    WL, WR = _f64(WL).reshape(5, -1), _f64(WR).reshape(5, -1)
+    F = np.empty_like(WL)
+    lib.dho_riemann(ctypes.c_longlong(WL.shape[1]), ctypes.byref(p), ctypes.c_int(axis), _ptr(WL), _ptr(WR), _ptr(F))
+    return F
+
+
+def reconstruct(W, p):
+    """Face states along one periodic line; W is [5, n].  Returns (WL, WR) at faces i+1/2."""
+    lib = _load()
+    W = _f64(W)
+    WL, WR = np.empty_like(W), np.empty_like(W)
+    lib.dho_reconstruct(ctypes.c_int(W.shape[1]), ctypes.byref(p), _ptr(W), _ptr(WL), _ptr(WR))
+    return WL, WR
+
+
+def limiter(a, b, kind="minmod"):
+    return float(_load().dho_limiter(float(a), float(b), LIMITERS[kind]))
+
+
+def window_step(U_full, dt, p, lo, size, halo=4):
+    """Windowed oracle: one step has a finite domain of dependence (+-4 cells per
+    axis), so stepping a periodic-wrapped window of `size`+2*halo cells is exact on its interior.
+    `lo`, `size` are (k, j, i) triples into the full periodic grid.  Returns [5, *size]."""
+    idx = [np.arange(lo[a] - halo, lo[a] + size[a] + halo) % U_full.shape[1 + a] for a in range(3)]
+    win = np.asarray(U_full)[:, idx[0][:, None, None], idx[1][None, :, None], idx[2][None, None, :]]
+    out = step(win, dt, p)
+    return out[:, halo:-halo, halo:-halo, halo:-halo]
+
+
+def window_step_vjp(U_full, dt, g_full, p, lo, size, halo=8):
+    """Windowed VJP: cotangent reach +-4, primal reach +-7 per axis for the two-stage step."""
+    idx = [np.arange(lo[a] - halo, lo[a] + size[a] + halo) % U_full.shape[1 + a] for a in range(3)]
+    sel = (slice(None), idx[0][:, None, None], idx[1][None, :, None], idx[2][None, None, :])
+    out = step_vjp(np.asarray(U_full)[sel], dt, np.asarray(g_full)[sel], p)
+    return out[:, halo:-halo, halo:-halo, halo:-halo]
