@@ -1,0 +1,137 @@
+/* dh.h — C ABI of the B200-native (sm_100a) hot path of arxiv/paper_2512_13403 ("diffhydro").
+ *
+ * One explicit time step of the 3D compressible Euler finite-volume update on a uniform periodic
+ * Cartesian grid, and its discrete adjoint.  The operation is the paper's pure step
+ *     U^{n+1} = H(U^n)                                   (Eq. 1)
+ * on global dense field arrays, with a separate time-step query (
+ * Eq. A8) and a vector-Jacobian product in which dt is data.
+ *
+ * Scheme (App. A; the readings of silent points are listed in DESIGN.md):
+ *   W = (rho, v, P), P = (gamma-1)(E - rho|v|^2/2)        (Eq. 2)
+ *   dW_i = minmod(W_{i+1}-W_i, W_i-W_{i-1}),  W^L_{i+1/2} = W_i + dW_i/2,
+ *   W^R_{i+1/2} = W_{i+1} - dW_{i+1}/2                    (Eqs. A1-A2)
+ *   F = HLLC(W^L, W^R) with S_L = min(v_L-c_L, v_R-c_R), S_R = max(v_L+c_L, v_R+c_R)
+ *                                                         (Eq. A3)
+ *   D(U)_i = sum_a (F_{a,i+1/2} - F_{a,i-1/2}) / dx_a     (Eq. A4)
+ *   U* = U^n - dt/2 D(U^n);  U^{n+1} = U^n - dt D(U*)     (Eqs. A6-A7, unsplit)
+ *   optional cooling of E after the update                (Eqs. 23-24)
+ *   dt = C_CFL min_a dx_a / max_cells(|v_a| + c_s)        (Eq. A8)
+ *
+ * ARRAYS.  A state is ONE contiguous array [5][nz][ny][nx] of T (float for DH_F32, double for
+ * DH_F64): field f in {0: rho, 1: rho*v_x, 2: rho*v_y, 3: rho*v_z, 4: E},
+ * x fastest, no ghost cells, periodic in x, y and z.  Unless a function says HOST, every array
+ * pointer is a DEVICE pointer (e.g. torch.Tensor.data_ptr()), at least 16-byte aligned.  The caller
+ * owns all arrays; the library neither frees nor retains them beyond the call (work is ordered on the
+ * context's stream).  The library owns its scratch (one state for U*, further states allocated
+ * lazily on the first VJP, reduction slots) and frees it in dh_destroy.
+ *
+ * GRID.  Unit box by default: dx_a = L_a / n_a with L = (1,1,1) (settable).  n_a >= 4.
+ *
+ * ERRORS.  Functions return DH_OK or a negative code; dh_last_error() gives a message for the last
+ * failure on the calling thread.  No function falls back to a CPU path: if no CUDA device / kernel
+ * image for sm_100 is available the call fails with DH_ERR_CUDA.
+ *
+ * THREADS.  One context per stream; a context is not re-entrant.
+ */
+#ifndef DH_H_
+#define DH_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dh_ctx dh_ctx;
+
+enum { DH_F32 = 0, DH_F64 = 1 };
+
+enum {
+  DH_OK = 0,
+  DH_ERR_ARG = -1,       /* bad argument (NULL, n_a < 4, dt <= 0 or non-finite, unknown option ...) */
+  DH_ERR_CUDA = -2,      /* a CUDA runtime call or kernel launch failed */
+  DH_ERR_ALLOC = -3,     /* device or pinned-host allocation failed */
+  DH_ERR_NONFINITE = -4  /* dh_cfl_dt: a NaN/Inf input or wave speed was found */
+};
+
+/* Keys of dh_set_option / dh_get_option.  Values are doubles; flags are 0 / 1. */
+enum {
+  DH_OPT_CFL = 0,        /* C_CFL of Eq. A8, default 0.4 */
+  DH_OPT_LX = 1,         /* box lengths, default 1; dx_a = L_a / n_a */
+  DH_OPT_LY = 2,
+  DH_OPT_LZ = 3,
+  DH_OPT_COOLING = 4,    /* 0 (default) / 1: E_th <- max(E_floor(rho), E_th - rho^2 Lambda0 T^alpha dt) after stage 2 */
+  DH_OPT_LAMBDA0 = 5,    /* default 1e-3 */
+  DH_OPT_ALPHA = 6,      /* default 0.5 */
+  DH_OPT_T_FLOOR = 7,    /* default 0.01; E_floor = rho T_floor / (gamma-1) (Eq. 24 with R = 1) */
+  DH_OPT_RHO_FLOOR = 8,  /* floors used only inside the primitive conversion, default 1e-10 */
+  DH_OPT_P_FLOOR = 9,
+  DH_OPT_KERNEL = 10,    /* 0 (default): fused z-sweep stage kernels; 1: one-thread-per-cell gather kernels
+                            (same arithmetic, kept for cross-checking and as the fallback for odd grid sizes) */
+  DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
+  DH_OPT_COUNT_
+};
+
+/* Create a context for an nx x ny x nz periodic grid, adiabatic index gamma, dtype DH_F32/DH_F64, on the
+ * current CUDA device.  Allocates the U* scratch state.  Returns NULL on failure (see dh_last_error). */
+dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype);
+
+/* Free the context and everything it owns.  NULL is allowed. */
+void dh_destroy(dh_ctx* ctx);
+
+/* Use `cuda_stream` (a cudaStream_t) for all subsequent work of this context.  Default: stream 0. */
+int dh_set_stream(dh_ctx* ctx, void* cuda_stream);
+
+int dh_set_option(dh_ctx* ctx, int key, double value);
+int dh_get_option(const dh_ctx* ctx, int key, double* value_out);
+
+/* CFL time step, Eq. A8: one block-reduced max-wavespeed kernel over the 5 fields, then
+ * dt = C * min_a(dx_a / S_a) formed on the device in T with IEEE-rounded, non-contracted operations, so
+ * that it is bit-identical to the same recipe evaluated on a CPU.  U: DEVICE, read only.
+ * dt_out: HOST; receives the T value widened exactly.  Synchronises the stream (the only host sync of
+ * the path).  Returns DH_ERR_NONFINITE (and leaves *dt_out untouched) if any input or speed is NaN/Inf. */
+int dh_cfl_dt(dh_ctx* ctx, const void* U, double* dt_out);
+
+/* One step in place, U^n -> U^{n+1} (stage 1 into the library's U* scratch, stage 2 back into U, cooling
+ * in the stage-2 epilogue if enabled).  U: DEVICE, read and overwritten.  dt > 0 finite.  Asynchronous on
+ * the context's stream. */
+int dh_step(dh_ctx* ctx, void* U, double dt);
+
+/* Same, with dt taken from the device-resident result of the last dh_cfl_dt_async / dh_cfl_dt on this
+ * context (no host round trip). */
+int dh_step_devdt(dh_ctx* ctx, void* U);
+
+/* Eq. A8 without the host read-back: leaves dt in the context's device slot for dh_step_devdt.
+ * Non-finite detection is deferred to dh_poll_status. */
+int dh_cfl_dt_async(dh_ctx* ctx, const void* U);
+
+/* Synchronise the stream and report (dt of the last CFL, non-finite flag -> DH_ERR_NONFINITE). */
+int dh_poll_status(dh_ctx* ctx, double* dt_out);
+
+/* Vector-Jacobian product of the full step (dt held constant):
+ *   gU_in = (dU^{n+1}/dU^n)^T gU_out   evaluated at U = U^n (the PRE-step state) and dt.
+ * Nothing is stored by dh_step: U* is recomputed, then the two stages are reversed by gather-form kernels
+ * (no atomics; deterministic).  U, gU_out: DEVICE, read only.  gU_in: DEVICE, overwritten; must not alias
+ * U or gU_out.  Asynchronous on the context's stream. */
+int dh_step_vjp(dh_ctx* ctx, const void* U, double dt, const void* gU_out, void* gU_in);
+
+/* HOST-buffer entry points (used for end-to-end measurements): U_host is a HOST array (pinned memory gives
+ * asynchronous copies) of the same layout.  The library copies it to a device state it owns, runs
+ * `nsteps` x (CFL dt + step) with the device-resident dt, copies the result back and synchronises.
+ * dt_last_out (HOST, may be NULL) receives the last dt. */
+int dh_run_host(dh_ctx* ctx, void* U_host, int nsteps, double* dt_last_out);
+
+/* HOST-buffer VJP: copies U and gU_out in, runs dh_step_vjp, copies gU_in out, synchronises. */
+int dh_step_vjp_host(dh_ctx* ctx, const void* U_host, double dt, const void* gU_out_host, void* gU_in_host);
+
+/* Number of kernel launches issued by this context since creation (bench.py's gpu_launches). */
+unsigned long long dh_launch_count(const dh_ctx* ctx);
+
+/* Message describing the last error on the calling thread ("" if none). */
+const char* dh_last_error(void);
+
+/* Library version string, e.g. "dh 0.1 sm_100a". */
+const char* dh_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DH_H_ */

@@ -1,0 +1,341 @@
+// dh_api.cu — the C ABI of include/dh.h: context management, option handling, and the launch sequences of
+// dh_cfl_dt / dh_step / dh_step_vjp.  No arithmetic of the scheme lives here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "../../include/dh.h"
+#include "dh_internal.cuh"
+
+using namespace dh;
+
+struct dh_ctx : public dh::Ctx {};
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, const char* detail = "") {
+  snprintf(g_err, sizeof(g_err), fmt, detail);
+  return code;
+}
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_err, sizeof(g_err), "%s: %s", where, cudaGetErrorString(e));
+  return DH_ERR_CUDA;
+}
+#define DH_CUDA(call, where)                                  \
+  do {                                                        \
+    cudaError_t e_ = (call);                                  \
+    if (e_ != cudaSuccess) return cuda_fail(e_, where);       \
+  } while (0)
+
+namespace dh {
+size_t elem_size(const Ctx* c) { return c->dtype == DH_F32 ? 4 : 8; }
+}  // namespace dh
+
+static size_t state_bytes(const dh_ctx* c) { return 5 * c->N * elem_size(c); }
+
+template <class T>
+static Consts<T> make_consts(const dh_ctx* c) {
+  Consts<T> k;
+  k.gamma = (T)c->gamma;
+  k.gm1 = (T)(c->gamma - 1.0);
+  k.inv_gm1 = (T)(1.0 / (c->gamma - 1.0));
+  k.rho_floor = (T)c->rho_floor;
+  k.p_floor = (T)c->p_floor;
+  k.lambda0 = (T)c->lambda0;
+  k.alpha = (T)c->alpha;
+  k.t_floor = (T)c->t_floor;
+  k.alpha_is_half = (c->alpha == 0.5);
+  return k;
+}
+
+static int lazy_alloc(dh_ctx* c, void** slot, size_t bytes, const char* what) {
+  if (*slot) return DH_OK;
+  cudaError_t e = cudaMalloc(slot, bytes);
+  if (e != cudaSuccess) {
+    *slot = nullptr;
+    cudaGetLastError();
+    return fail(DH_ERR_ALLOC, "cudaMalloc failed for %s", what);
+  }
+  return DH_OK;
+}
+
+extern "C" {
+
+const char* dh_last_error(void) { return g_err; }
+const char* dh_version(void) { return "dh 0.1 sm_100a"; }
+
+dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
+  g_err[0] = 0;
+  if (nx < 4 || ny < 4 || nz < 4) { fail(DH_ERR_ARG, "dh_create: every n_a must be >= 4%s"); return nullptr; }
+  if (!(gamma > 1.0) || !isfinite(gamma)) { fail(DH_ERR_ARG, "dh_create: gamma must be finite and > 1%s"); return nullptr; }
+  if (dtype != DH_F32 && dtype != DH_F64) { fail(DH_ERR_ARG, "dh_create: dtype must be DH_F32 or DH_F64%s"); return nullptr; }
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { cuda_fail(e, "dh_create: cudaGetDevice (no CUDA device? there is no CPU fallback)"); return nullptr; }
+  dh_ctx* c = new (std::nothrow) dh_ctx();
+  if (!c) { fail(DH_ERR_ALLOC, "dh_create: out of host memory%s"); return nullptr; }
+  memset(static_cast<dh::Ctx*>(c), 0, sizeof(dh::Ctx));
+  c->nx = nx; c->ny = ny; c->nz = nz; c->dtype = dtype;
+  c->N = (size_t)nx * ny * nz;
+  c->gamma = gamma;
+  c->cfl = 0.4;
+  c->L[0] = c->L[1] = c->L[2] = 1.0;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0;
+  c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
+  c->rho_floor = 1e-10; c->p_floor = 1e-10;
+  c->stream = 0;
+  cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  if (c->sm_count <= 0) c->sm_count = 148;
+  bool ok = cudaMalloc(&c->Us, state_bytes(c)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->acc, 4 * sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && cudaMalloc(&c->dt_dev, 8) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->result_dev, sizeof(CflResult)) == cudaSuccess;
+  ok = ok && cudaMallocHost((void**)&c->result_host, sizeof(CflResult)) == cudaSuccess;
+  ok = ok && cudaMemset(c->acc, 0, 4 * sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && cudaMemset(c->dt_dev, 0, 8) == cudaSuccess;
+  ok = ok && cudaMemset(c->result_dev, 0, sizeof(CflResult)) == cudaSuccess;
+  if (!ok) {
+    cudaError_t le = cudaGetLastError();
+    dh_destroy(c);
+    snprintf(g_err, sizeof(g_err), "dh_create: allocation failed (%s)", cudaGetErrorString(le));
+    return nullptr;
+  }
+  memset(c->result_host, 0, sizeof(CflResult));
+  return c;
+}
+
+void dh_destroy(dh_ctx* c) {
+  if (!c) return;
+  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->acc, c->dt_dev, c->result_dev};
+  for (void* p : dev)
+    if (p) cudaFree(p);
+  if (c->result_host) cudaFreeHost(c->result_host);
+  delete c;
+}
+
+int dh_set_stream(dh_ctx* c, void* cuda_stream) {
+  if (!c) return fail(DH_ERR_ARG, "dh_set_stream: NULL context%s");
+  c->stream = (cudaStream_t)cuda_stream;
+  return DH_OK;
+}
+
+int dh_set_option(dh_ctx* c, int key, double v) {
+  if (!c) return fail(DH_ERR_ARG, "dh_set_option: NULL context%s");
+  if (!isfinite(v)) return fail(DH_ERR_ARG, "dh_set_option: value must be finite%s");
+  switch (key) {
+    case DH_OPT_CFL: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: CFL must be > 0%s"); c->cfl = v; break;
+    case DH_OPT_LX: case DH_OPT_LY: case DH_OPT_LZ:
+      if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: box length must be > 0%s");
+      c->L[key - DH_OPT_LX] = v; break;
+    case DH_OPT_COOLING: c->cooling = (v != 0.0); break;
+    case DH_OPT_LAMBDA0: c->lambda0 = v; break;
+    case DH_OPT_ALPHA: c->alpha = v; break;
+    case DH_OPT_T_FLOOR: c->t_floor = v; break;
+    case DH_OPT_RHO_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->rho_floor = v; break;
+    case DH_OPT_P_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->p_floor = v; break;
+    case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0 or 1%s"); c->kernel = (int)v; break;
+    case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
+    default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
+  }
+  return DH_OK;
+}
+
+int dh_get_option(const dh_ctx* c, int key, double* out) {
+  if (!c || !out) return fail(DH_ERR_ARG, "dh_get_option: NULL argument%s");
+  switch (key) {
+    case DH_OPT_CFL: *out = c->cfl; break;
+    case DH_OPT_LX: case DH_OPT_LY: case DH_OPT_LZ: *out = c->L[key - DH_OPT_LX]; break;
+    case DH_OPT_COOLING: *out = c->cooling; break;
+    case DH_OPT_LAMBDA0: *out = c->lambda0; break;
+    case DH_OPT_ALPHA: *out = c->alpha; break;
+    case DH_OPT_T_FLOOR: *out = c->t_floor; break;
+    case DH_OPT_RHO_FLOOR: *out = c->rho_floor; break;
+    case DH_OPT_P_FLOOR: *out = c->p_floor; break;
+    case DH_OPT_KERNEL: *out = c->kernel; break;
+    case DH_OPT_LIMITER: *out = c->limiter; break;
+    default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
+  }
+  return DH_OK;
+}
+
+unsigned long long dh_launch_count(const dh_ctx* c) { return c ? c->launches : 0ull; }
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ CFL
+template <class T>
+static int cfl_launch(dh_ctx* c, const void* U) {
+  CflParams<T> p;
+  p.U = (const T*)U;
+  p.N = c->N;
+  p.gamma = (T)c->gamma;
+  p.gm1 = (T)(c->gamma - 1.0);
+  p.rho_floor = (T)c->rho_floor;
+  p.p_floor = (T)c->p_floor;
+  const int n[3] = {c->nx, c->ny, c->nz};
+  for (int a = 0; a < 3; ++a) p.dx[a] = (T)(c->L[a] / n[a]);
+  p.cfl = (T)c->cfl;
+  p.acc = c->acc;
+  p.dt_dev = (T*)c->dt_dev;
+  p.result = c->result_dev;
+  DH_CUDA(launch_cfl<T>(p, c->sm_count, c->stream), "dh_cfl_dt: kernel launch");
+  c->launches += 2;
+  return DH_OK;
+}
+
+// ------------------------------------------------------------------------------------------ forward
+template <class T>
+static int stage_launch(dh_ctx* c, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool) {
+  StageParams<T> p;
+  p.U = (const T*)U; p.B = (const T*)B; p.out = (T*)out;
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+  const int n[3] = {c->nx, c->ny, c->nz};
+  for (int a = 0; a < 3; ++a) p.inv_dx[a] = (T)(n[a] / c->L[a]);
+  p.dt = (T)dt;
+  p.dt_dev = devdt ? (const T*)c->dt_dev : nullptr;
+  p.frac = (T)frac;
+  p.cool = cool ? 1 : 0;
+  p.c = make_consts<T>(c);
+  bool done = false;
+  if (c->kernel == 0) {
+    bool supported = false;
+    cudaError_t e = launch_stage_fused<T>(p, c->limiter, c->sm_count, c->stream, &supported);
+    if (supported) {
+      if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
+      done = true;
+    }
+  }
+  if (!done) DH_CUDA(launch_stage_naive<T>(p, c->limiter, c->stream), "dh_step: stage kernel launch");
+  c->launches += 1;
+  return DH_OK;
+}
+
+template <class T>
+static int step_impl(dh_ctx* c, void* U, double dt, bool devdt) {
+  // predictor: U* = U^n - dt/2 D(U^n)   (Eq. A6);  corrector, in place: U^{n+1} = U^n - dt D(U*)   (Eq. A7)
+  int rc = stage_launch<T>(c, U, U, c->Us, dt, devdt, 0.5, false);
+  if (rc) return rc;
+  return stage_launch<T>(c, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0);
+}
+
+// ------------------------------------------------------------------------------------------ reverse
+template <class T>
+static int rev_launch(dh_ctx* c, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+  RevParams<T> p;
+  p.U = (const T*)U; p.g = (const T*)g; p.b1 = (const T*)b1; p.b2 = (const T*)b2; p.out = (T*)out;
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
+  const int n[3] = {c->nx, c->ny, c->nz};
+  for (int a = 0; a < 3; ++a) p.inv_dx[a] = (T)(n[a] / c->L[a]);
+  p.dt = (T)dt;
+  p.frac = (T)frac;
+  p.c = make_consts<T>(c);
+  DH_CUDA(launch_rev_naive<T>(p, c->limiter, c->stream), "dh_step_vjp: reverse stage kernel launch");
+  c->launches += 1;
+  return DH_OK;
+}
+
+template <class T>
+static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
+  int rc = lazy_alloc(c, &c->gs, state_bytes(c), "the U* cotangent state");
+  if (rc) return rc;
+  // recompute U* = U^n - dt/2 D(U^n)  (nothing was stored by dh_step)
+  rc = stage_launch<T>(c, U, U, c->Us, dt, false, 0.5, false);
+  if (rc) return rc;
+  const void* g1 = gout;
+  if (c->cooling) {
+    // pre-cooling state U1 = U^n - dt D(U*), then g1 = J_cool(U1)^T g_out
+    rc = lazy_alloc(c, &c->U1, state_bytes(c), "the pre-cooling state");
+    if (rc) return rc;
+    rc = lazy_alloc(c, &c->g1, state_bytes(c), "the pre-cooling cotangent");
+    if (rc) return rc;
+    rc = stage_launch<T>(c, c->Us, U, c->U1, dt, false, 1.0, false);
+    if (rc) return rc;
+    DH_CUDA(launch_cool_vjp<T>((const T*)c->U1, (const T*)gout, (T*)c->g1, c->N, (T)dt, make_consts<T>(c), c->stream),
+            "dh_step_vjp: cooling reverse kernel launch");
+    c->launches += 1;
+    g1 = c->g1;
+  }
+  // reverse corrector:  gs = -dt J_D(U*)^T g1
+  rc = rev_launch<T>(c, c->Us, g1, nullptr, nullptr, c->gs, dt, 1.0);
+  if (rc) return rc;
+  // reverse predictor:  g_in = g1 + gs - dt/2 J_D(U^n)^T gs
+  return rev_launch<T>(c, U, c->gs, g1, c->gs, gin, dt, 0.5);
+}
+
+extern "C" {
+
+int dh_cfl_dt_async(dh_ctx* c, const void* U) {
+  if (!c || !U) return fail(DH_ERR_ARG, "dh_cfl_dt: NULL argument%s");
+  return c->dtype == DH_F32 ? cfl_launch<float>(c, U) : cfl_launch<double>(c, U);
+}
+
+int dh_poll_status(dh_ctx* c, double* dt_out) {
+  if (!c) return fail(DH_ERR_ARG, "dh_poll_status: NULL context%s");
+  DH_CUDA(cudaMemcpyAsync(c->result_host, c->result_dev, sizeof(CflResult), cudaMemcpyDeviceToHost, c->stream), "dh_poll_status: copy");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_poll_status: synchronize");
+  if (c->result_host->nonfinite) return fail(DH_ERR_NONFINITE, "dh_cfl_dt: non-finite input or wave speed%s");
+  if (dt_out) *dt_out = c->result_host->dt;
+  return DH_OK;
+}
+
+int dh_cfl_dt(dh_ctx* c, const void* U, double* dt_out) {
+  if (!dt_out) return fail(DH_ERR_ARG, "dh_cfl_dt: NULL dt_out%s");
+  int rc = dh_cfl_dt_async(c, U);
+  if (rc) return rc;
+  return dh_poll_status(c, dt_out);
+}
+
+int dh_step(dh_ctx* c, void* U, double dt) {
+  if (!c || !U) return fail(DH_ERR_ARG, "dh_step: NULL argument%s");
+  if (!(dt > 0.0) || !isfinite(dt)) return fail(DH_ERR_ARG, "dh_step: dt must be finite and > 0%s");
+  if (U == c->Us) return fail(DH_ERR_ARG, "dh_step: U aliases library scratch%s");
+  return c->dtype == DH_F32 ? step_impl<float>(c, U, dt, false) : step_impl<double>(c, U, dt, false);
+}
+
+int dh_step_devdt(dh_ctx* c, void* U) {
+  if (!c || !U) return fail(DH_ERR_ARG, "dh_step_devdt: NULL argument%s");
+  return c->dtype == DH_F32 ? step_impl<float>(c, U, 0.0, true) : step_impl<double>(c, U, 0.0, true);
+}
+
+int dh_step_vjp(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
+  if (!c || !U || !gout || !gin) return fail(DH_ERR_ARG, "dh_step_vjp: NULL argument%s");
+  if (!(dt > 0.0) || !isfinite(dt)) return fail(DH_ERR_ARG, "dh_step_vjp: dt must be finite and > 0%s");
+  if (gin == U || gin == gout) return fail(DH_ERR_ARG, "dh_step_vjp: gU_in must not alias U or gU_out%s");
+  return c->dtype == DH_F32 ? vjp_impl<float>(c, U, dt, gout, gin) : vjp_impl<double>(c, U, dt, gout, gin);
+}
+
+int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {
+  if (!c || !U_host || nsteps < 0) return fail(DH_ERR_ARG, "dh_run_host: bad argument%s");
+  int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
+  if (rc) return rc;
+  DH_CUDA(cudaMemcpyAsync(c->Uhost_dev, U_host, state_bytes(c), cudaMemcpyHostToDevice, c->stream), "dh_run_host: H2D");
+  for (int s = 0; s < nsteps; ++s) {
+    rc = dh_cfl_dt_async(c, c->Uhost_dev);
+    if (rc) return rc;
+    rc = dh_step_devdt(c, c->Uhost_dev);
+    if (rc) return rc;
+  }
+  DH_CUDA(cudaMemcpyAsync(U_host, c->Uhost_dev, state_bytes(c), cudaMemcpyDeviceToHost, c->stream), "dh_run_host: D2H");
+  return dh_poll_status(c, dt_last_out);
+}
+
+int dh_step_vjp_host(dh_ctx* c, const void* U_host, double dt, const void* gout_host, void* gin_host) {
+  if (!c || !U_host || !gout_host || !gin_host) return fail(DH_ERR_ARG, "dh_step_vjp_host: NULL argument%s");
+  int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
+  if (rc) return rc;
+  rc = lazy_alloc(c, &c->gA, state_bytes(c), "the device cotangent (in)");
+  if (rc) return rc;
+  rc = lazy_alloc(c, &c->gB, state_bytes(c), "the device cotangent (out)");
+  if (rc) return rc;
+  DH_CUDA(cudaMemcpyAsync(c->Uhost_dev, U_host, state_bytes(c), cudaMemcpyHostToDevice, c->stream), "dh_step_vjp_host: H2D");
+  DH_CUDA(cudaMemcpyAsync(c->gA, gout_host, state_bytes(c), cudaMemcpyHostToDevice, c->stream), "dh_step_vjp_host: H2D");
+  rc = dh_step_vjp(c, c->Uhost_dev, dt, c->gA, c->gB);
+  if (rc) return rc;
+  DH_CUDA(cudaMemcpyAsync(gin_host, c->gB, state_bytes(c), cudaMemcpyDeviceToHost, c->stream), "dh_step_vjp_host: D2H");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_step_vjp_host: synchronize");
+  return DH_OK;
+}
+
+}  // extern "C"

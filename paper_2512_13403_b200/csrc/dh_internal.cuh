@@ -1,0 +1,91 @@
+// dh_internal.cuh — context, kernel parameter blocks and launcher declarations shared by the .cu files.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "dh_math.cuh"
+
+namespace dh {
+
+// Parameters of one stage  out = B - frac*dt * D(U)  (Eqs. A4, A6-A7).
+template <class T>
+struct StageParams {
+  const T* U;        // stencil input state [5][nz][ny][nx]
+  const T* B;        // base state (U^n); may alias `out` (stage 2 runs in place)
+  T* out;
+  int nx, ny, nz;
+  T inv_dx[3];       // 1 / dx_a
+  T dt;              // used when dt_dev == nullptr
+  const T* dt_dev;   // device-resident dt (result of the CFL kernel)
+  T frac;            // 1/2 for the predictor, 1 for the corrector
+  int cool;          // apply the cooling source to the result (corrector only)
+  Consts<T> c;
+};
+
+// Parameters of one reversed stage  out = b1 + b2 - frac*dt * J_D(U)^T g   (gather form).
+template <class T>
+struct RevParams {
+  const T* U;        // primal state the stage was evaluated at
+  const T* g;        // cotangent of the stage output
+  const T* b1;       // optional additive terms (nullptr = none)
+  const T* b2;
+  T* out;
+  int nx, ny, nz;
+  T inv_dx[3];
+  T dt;
+  T frac;
+  Consts<T> c;
+};
+
+// result block of the CFL reduction (device + pinned host mirror); all slots 8 bytes wide
+struct CflResult {
+  double smax[3];    // T values widened
+  double dt;         // T value widened
+  unsigned long long nonfinite;
+};
+
+template <class T>
+struct CflParams {
+  const T* U;
+  size_t N;
+  T gamma, gm1, rho_floor, p_floor;
+  T dx[3];
+  T cfl;
+  unsigned long long* acc;   // [0..2] running max (bit pattern of T, zero-extended), [3] non-finite flag
+  T* dt_dev;                 // dt in T for the stage kernels
+  CflResult* result;         // device copy of the result block
+};
+
+struct Ctx {
+  int nx, ny, nz, dtype;
+  size_t N;
+  double gamma, cfl, L[3];
+  int cooling, kernel, limiter;
+  double lambda0, alpha, t_floor, rho_floor, p_floor;
+  cudaStream_t stream;
+  int sm_count;
+  void* Us;                    // U* scratch (always)
+  void* gs;                    // cotangent of U* (first VJP)
+  void* U1;                    // pre-cooling state, cooling VJP only
+  void* g1;                    // cotangent of U1, cooling VJP only
+  void* Uhost_dev;             // device state for the HOST entry points
+  void* gA;                    // device cotangent buffers for dh_step_vjp_host
+  void* gB;
+  unsigned long long* acc;     // device accumulators of the CFL reduction
+  void* dt_dev;                // device dt (T)
+  CflResult* result_dev;
+  CflResult* result_host;      // pinned
+  unsigned long long launches;
+};
+
+size_t elem_size(const Ctx* c);
+
+// launchers (each returns the cudaError_t of the launch)
+template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, cudaStream_t s);
+template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
+template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s);
+template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
+template <class T> cudaError_t launch_cfl(const CflParams<T>& p, int sm_count, cudaStream_t s);   // 2 launches
+
+}  // namespace dh

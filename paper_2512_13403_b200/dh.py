@@ -1,0 +1,243 @@
+"""Thin ctypes binding over the C-ABI library (include/dh.h): argument marshalling only.
+
+Every step of the path (CFL reduction, both RK2 stages, cooling, the reverse-mode stages) runs in the CUDA
+kernels of ``libdh.so``; PyTorch is used for device memory and streams.  There is no CPU fallback: if the
+library cannot be built/loaded, or no CUDA device is present, calls raise.
+
+The module-level functions carry the C names (``dh_create`` ... ``dh_destroy``); ``Solver`` wraps a context.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+DH_F32, DH_F64 = 0, 1
+DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, -4
+OPTIONS = {
+    "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
+    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11,
+}
+LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
+KERNELS = {"fused": 0, "gather": 1}
+
+# every symbol include/dh.h declares (checked by tests/test_abi.py)
+SYMBOLS = [
+    "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
+    "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
+    "dh_launch_count", "dh_last_error", "dh_version",
+]
+
+_lib = None
+
+
+class DhError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"dh error {code}: {msg}")
+        self.code = code
+
+
+def load(rebuild: bool = False):
+    """Load libdh.so (building it in-tree with nvcc if it is missing or stale).  Raises on failure."""
+    global _lib
+    if _lib is not None and not rebuild:
+        return _lib
+    path = _build.build(force=rebuild)
+    lib = ctypes.CDLL(path)
+    vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+    pd = ctypes.POINTER(ctypes.c_double)
+    lib.dh_create.restype = vp
+    lib.dh_create.argtypes = [ci, ci, ci, cd, ci]
+    lib.dh_destroy.restype = None
+    lib.dh_destroy.argtypes = [vp]
+    lib.dh_set_stream.argtypes = [vp, vp]
+    lib.dh_set_option.argtypes = [vp, ci, cd]
+    lib.dh_get_option.argtypes = [vp, ci, pd]
+    lib.dh_cfl_dt.argtypes = [vp, vp, pd]
+    lib.dh_cfl_dt_async.argtypes = [vp, vp]
+    lib.dh_poll_status.argtypes = [vp, pd]
+    lib.dh_step.argtypes = [vp, vp, cd]
+    lib.dh_step_devdt.argtypes = [vp, vp]
+    lib.dh_step_vjp.argtypes = [vp, vp, cd, vp, vp]
+    lib.dh_run_host.argtypes = [vp, vp, ci, pd]
+    lib.dh_step_vjp_host.argtypes = [vp, vp, cd, vp, vp]
+    lib.dh_launch_count.restype = ctypes.c_ulonglong
+    lib.dh_launch_count.argtypes = [vp]
+    lib.dh_last_error.restype = ctypes.c_char_p
+    lib.dh_version.restype = ctypes.c_char_p
+    for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
+               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host"):
+        getattr(lib, fn).restype = ci
+    _lib = lib
+    return lib
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def _check(rc: int):
+    if rc != DH_OK:
+        raise DhError(rc, load().dh_last_error().decode())
+
+
+# ------------------------------------------------------------------------------------ C-named functions
+def dh_version() -> str:
+    return load().dh_version().decode()
+
+
+def dh_last_error() -> str:
+    return load().dh_last_error().decode()
+
+
+def dh_create(nx: int, ny: int, nz: int, gamma: float, dtype: int):
+    h = load().dh_create(int(nx), int(ny), int(nz), float(gamma), int(dtype))
+    if not h:
+        raise DhError(DH_ERR_ARG, dh_last_error())
+    return h
+
+
+def dh_destroy(ctx) -> None:
+    load().dh_destroy(ctx)
+
+
+def dh_set_stream(ctx, cuda_stream: int) -> None:
+    _check(load().dh_set_stream(ctx, ctypes.c_void_p(cuda_stream)))
+
+
+def dh_set_option(ctx, key: int, value: float) -> None:
+    _check(load().dh_set_option(ctx, int(key), float(value)))
+
+
+def dh_get_option(ctx, key: int) -> float:
+    out = ctypes.c_double()
+    _check(load().dh_get_option(ctx, int(key), ctypes.byref(out)))
+    return out.value
+
+
+def dh_cfl_dt(ctx, U_ptr: int) -> float:
+    out = ctypes.c_double()
+    _check(load().dh_cfl_dt(ctx, ctypes.c_void_p(U_ptr), ctypes.byref(out)))
+    return out.value
+
+
+def dh_cfl_dt_async(ctx, U_ptr: int) -> None:
+    _check(load().dh_cfl_dt_async(ctx, ctypes.c_void_p(U_ptr)))
+
+
+def dh_poll_status(ctx) -> float:
+    out = ctypes.c_double()
+    _check(load().dh_poll_status(ctx, ctypes.byref(out)))
+    return out.value
+
+
+def dh_step(ctx, U_ptr: int, dt: float) -> None:
+    _check(load().dh_step(ctx, ctypes.c_void_p(U_ptr), float(dt)))
+
+
+def dh_step_devdt(ctx, U_ptr: int) -> None:
+    _check(load().dh_step_devdt(ctx, ctypes.c_void_p(U_ptr)))
+
+
+def dh_step_vjp(ctx, U_ptr: int, dt: float, gout_ptr: int, gin_ptr: int) -> None:
+    _check(load().dh_step_vjp(ctx, ctypes.c_void_p(U_ptr), float(dt), ctypes.c_void_p(gout_ptr), ctypes.c_void_p(gin_ptr)))
+
+
+def dh_run_host(ctx, U_host_ptr: int, nsteps: int) -> float:
+    out = ctypes.c_double()
+    _check(load().dh_run_host(ctx, ctypes.c_void_p(U_host_ptr), int(nsteps), ctypes.byref(out)))
+    return out.value
+
+
+def dh_step_vjp_host(ctx, U_host_ptr: int, dt: float, gout_host_ptr: int, gin_host_ptr: int) -> None:
+    _check(load().dh_step_vjp_host(ctx, ctypes.c_void_p(U_host_ptr), float(dt), ctypes.c_void_p(gout_host_ptr),
+                                   ctypes.c_void_p(gin_host_ptr)))
+
+
+def dh_launch_count(ctx) -> int:
+    return int(load().dh_launch_count(ctx))
+
+
+# ------------------------------------------------------------------------------------------- convenience
+class Solver:
+    """A dh context bound to a grid; states are torch CUDA tensors [5, nz, ny, nx]."""
+
+    def __init__(self, nx: int, ny: int, nz: int, gamma: float = 5.0 / 3.0, dtype=torch.float32, stream=None, **options):
+        if dtype not in (torch.float32, torch.float64):
+            raise TypeError("dtype must be torch.float32 or torch.float64")
+        if not torch.cuda.is_available():
+            raise RuntimeError("dh needs a CUDA device; there is no CPU fallback")
+        self.shape = (5, int(nz), int(ny), int(nx))
+        self.dtype = dtype
+        self.ctx = dh_create(nx, ny, nz, gamma, DH_F32 if dtype == torch.float32 else DH_F64)
+        stream = stream if stream is not None else torch.cuda.current_stream()
+        dh_set_stream(self.ctx, stream.cuda_stream)
+        self.stream = stream
+        self.set_options(**options)
+
+    def set_options(self, **options):
+        for k, v in options.items():
+            if k == "limiter" and isinstance(v, str):
+                v = LIMITERS[v]
+            if k == "kernel" and isinstance(v, str):
+                v = KERNELS[v]
+            dh_set_option(self.ctx, OPTIONS[k], float(v))
+
+    def get_option(self, name: str) -> float:
+        return dh_get_option(self.ctx, OPTIONS[name])
+
+    def _dev(self, t: torch.Tensor, name: str) -> int:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {self.shape} and dtype {self.dtype}")
+        return t.data_ptr()
+
+    def _host(self, t: torch.Tensor, name: str) -> int:
+        if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape):
+            raise ValueError(f"{name} must be a contiguous host tensor of shape {self.shape} and dtype {self.dtype}")
+        return t.data_ptr()
+
+    def cfl_dt(self, U) -> float:
+        return dh_cfl_dt(self.ctx, self._dev(U, "U"))
+
+    def cfl_dt_async(self, U) -> None:
+        dh_cfl_dt_async(self.ctx, self._dev(U, "U"))
+
+    def poll(self) -> float:
+        return dh_poll_status(self.ctx)
+
+    def step(self, U, dt: float) -> None:
+        dh_step(self.ctx, self._dev(U, "U"), dt)
+
+    def step_devdt(self, U) -> None:
+        dh_step_devdt(self.ctx, self._dev(U, "U"))
+
+    def step_vjp(self, U, dt: float, g_out, g_in=None):
+        if g_in is None:
+            g_in = torch.empty_like(U)
+        dh_step_vjp(self.ctx, self._dev(U, "U"), dt, self._dev(g_out, "g_out"), self._dev(g_in, "g_in"))
+        return g_in
+
+    def run_host(self, U_host, nsteps: int) -> float:
+        return dh_run_host(self.ctx, self._host(U_host, "U_host"), nsteps)
+
+    def step_vjp_host(self, U_host, dt: float, g_out_host, g_in_host) -> None:
+        dh_step_vjp_host(self.ctx, self._host(U_host, "U_host"), dt, self._host(g_out_host, "g_out_host"),
+                         self._host(g_in_host, "g_in_host"))
+
+    @property
+    def launch_count(self) -> int:
+        return dh_launch_count(self.ctx)
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            dh_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -132,7 +132,8 @@ def test_vjp_stencil_reach_and_window():
     win = oracle.window_step_vjp(U, dt, g, p, lo=(17, 0, 9), size=(5, 4, 6))
     idx = [np.arange(lo, lo + s) % 20 for lo, s in zip((17, 0, 9), (5, 4, 6))]
     want = full[:, idx[0][:, None, None], idx[1][None, :, None], idx[2][None, None, :]]
-    assert np.array_equal(win, want)
+    # scatter-add order differs between the window and the full grid: equal to rounding, not bitwise
+    assert np.abs(win - want).max() <= 1e-14 * np.abs(want).max()
     fwin = oracle.window_step(U, dt, p, lo=(17, 0, 9), size=(5, 4, 6))
     fwant = oracle.step(U, dt, p)[:, idx[0][:, None, None], idx[1][None, :, None], idx[2][None, None, :]]
     assert np.array_equal(fwin, fwant)
