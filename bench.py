@@ -1,0 +1,397 @@
+"""bench.py — throughput of the hot path (CFL dt + one RK2 step of the 3D Euler finite-volume update, and the
+VJP of that step) on synthetic workloads shaped like the paper's, through the C ABI of include/dh.h.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 1024] [--impl dh|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+One JSON line on stdout (rank 0).  Contract and the meaning of every key: DESIGN.md §"Measurement".
+
+* workload (default): BASELINE.json configs[4] — 1024^3 fp32 periodic decaying turbulence, rms Mach 2, no
+  cooling (21.5 GB per state, far larger than the 126 MB L2, so no L2 flush is needed between iterations).
+* a "step" = dh_cfl_dt_async + dh_step_devdt (CFL reduction, predictor stage, corrector stage; dt never leaves
+  the device).  `value` = cells * K / time, inputs resident in HBM.  The VJP of the step (dh_step_vjp) is timed
+  in the same run and reported under "vjp".
+* "e2e" = the same step through dh_run_host: pinned HOST buffer -> device, CFL + step, device -> HOST, all
+  inside the timed region.
+* N > 1: the path does not shard in this build ("replicas only"): every rank runs the same-shaped
+  workload (its own seed) on its own GPU, no data-path collective; value = sum of the ranks' cells / max time.
+* --impl reference: the CPU oracle (oracle/), as it stands, on the host cores, on a bounded sample of the same
+  workload.  This and the `cpu_baseline` leg are the only places this file touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s per RK2 step (forward: CFL dt + predictor + corrector)"
+UNIT = "cell-updates/s"
+FWD_WORDS, VJP_WORDS = 25, 45          # algorithmic words per cell: SURVEY.md §8(d), DESIGN.md §"Kernels"
+STAGE_WORDS = {"stage1": 10, "stage2": 15, "rev2": 15, "rev1": 20, "cfl_reduce": 5}
+FALLBACK_HBM_GBS = 6650.0              # /opt/skills/guides/B200_PROFILING.md, used only without MEASURED_PEAKS.json
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="dh", choices=["dh", "reference"])
+    ap.add_argument("--n", type=int, default=1024, help="grid size per axis (default 1024: BASELINE configs[4])")
+    ap.add_argument("--cooling", type=int, default=0, help="1: configs[3]'s cooling source in the corrector epilogue")
+    ap.add_argument("--mach", type=float, default=2.0)
+    ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
+    ap.add_argument("--no-vjp", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-sample", type=int, default=192, help="edge of the periodic sub-block the oracle is timed on")
+    return ap.parse_args()
+
+
+def workload_name(a) -> str:
+    if a.cooling:
+        return f"cooling_turbulence_{a.n}^3_fp32_mach{a.mach:g} (BASELINE configs[3] recipe)"
+    return f"decaying_turbulence_{a.n}^3_fp32_mach{a.mach:g} (BASELINE configs[4] recipe)"
+
+
+def measured_peak():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
+
+
+def committed_traffic(n: int):
+    """DRAM bytes per stage-kernel launch from the committed ncu --set full capture (profiles/traffic.json:
+    {"<n>": bytes}), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(str(n))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                          "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        rows = [r for t, r in self.rows if t0 <= t <= t1 + 0.2 and len(r) >= 7] or [r for _, r in self.rows if len(r) >= 7]
+        if not rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for i, nm in enumerate(names) if any(r[3 + i].lower().startswith("active") for r in rows)]
+        num = lambda s: float(s) if s.replace(".", "", 1).isdigit() else float("nan")
+        return {"sm_mhz": statistics.median(num(r[0]) for r in rows), "sm_max_mhz": num(rows[0][1]),
+                "power_w_max": max(num(r[2]) for r in rows), "samples": len(rows), "reasons": reasons}
+
+
+# --------------------------------------------------------------------------------------------- oracle legs
+def oracle_sample(U_block, gamma: float, cooling: bool, with_vjp: bool = False, seed: int = 2005) -> dict:
+    """Time the CPU oracle, as it stands, for one CFL dt + one full step on `U_block` ([5, m, m, m] numpy,
+    treated as its own periodic box).  Returns cell-updates/s and what was timed."""
+    import numpy as np
+
+    import oracle
+
+    p = oracle.params(gamma=gamma, shape=tuple(U_block.shape), cooling=cooling)
+    cells = int(np.prod(U_block.shape[1:]))
+    t0 = time.perf_counter()
+    dt, _ = oracle.cfl_dt(U_block, p)
+    oracle.step(U_block, dt, p)
+    t_fwd = time.perf_counter() - t0
+    out = {"value": cells / t_fwd, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+           "sample": f"one CFL dt + RK2 step on a {U_block.shape[3]}x{U_block.shape[2]}x{U_block.shape[1]} periodic sub-block "
+                     f"of the workload's initial state ({cells} cells, {t_fwd:.2f} s, fp64 oracle, OpenMP)"}
+    if with_vjp:
+        m = min(96, U_block.shape[1])
+        sub = np.ascontiguousarray(U_block[:, :m, :m, :m])
+        g = np.random.default_rng(seed).normal(size=sub.shape)
+        ps = oracle.params(gamma=gamma, shape=tuple(sub.shape), cooling=cooling)
+        t0 = time.perf_counter()
+        oracle.step_vjp(sub, dt, g, ps)
+        t_v = time.perf_counter() - t0
+        out["vjp_value"] = m ** 3 / t_v
+        out["vjp_sample"] = f"one step VJP on a {m}^3 sub-block ({t_v:.2f} s)"
+    return out
+
+
+def cpu_block(a, m: int, seed: int):
+    """The bounded CPU sample: the workload's own recipe generated at edge m (same generator, same spectrum band
+    rule) — used when no device state is at hand (--impl reference)."""
+    import torch
+
+    from paper_2512_13403_b200 import workloads
+
+    wl = workloads.turbulence(m, seed=seed, mach=a.mach, cooling=bool(a.cooling), dtype=torch.float32)
+    return wl.U.numpy(), wl.gamma
+
+
+def run_reference(a):
+    """--impl reference: the oracle on the host cores; each step = one bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    m = min(a.cpu_sample, a.n, 128)
+    U, gamma = cpu_block(a, m, 1005 if not a.cooling else 1004)
+    import oracle
+
+    oracle.build()
+    for _ in range(min(a.warmup, 1)):
+        oracle_sample(U, gamma, bool(a.cooling))
+    times, last = [], None
+    for _ in range(a.steps):
+        t0 = time.perf_counter()
+        last = oracle_sample(U, gamma, bool(a.cooling))
+        times.append(time.perf_counter() - t0)
+    cells = m ** 3
+    total = sum(times)
+    value = cells * a.steps / total
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": 1e3 * total / a.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(a), "sample": f"{m}^3 periodic box of the same recipe per step",
+                       "l2": "CPU run"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["cores"], "kind": "oracle",
+                             "sample": f"{a.steps} x (CFL dt + RK2 step) on a {m}^3 box generated by the workload's recipe"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------- dh leg
+def run_dh(a):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2512_13403_b200 import dh, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the dh path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    n, K, W = a.n, a.steps, max(a.warmup, 0)
+    N = n ** 3
+    seed = (1004 if a.cooling else 1005) + 17 * rank       # replicas: same recipe, own seed per rank
+    wl = workloads.turbulence(n, seed=seed, mach=a.mach, cooling=bool(a.cooling), dtype=torch.float32, device=dev)
+    U = wl.U
+    torch.cuda.empty_cache()
+    # the oracle's bounded sample: a sub-block of the initial state, taken before anything is stepped
+    m = min(a.cpu_sample, n)
+    U_cpu_block = U[:, :m, :m, :m].contiguous().cpu().numpy() if (rank == 0 and world == 1 and not a.no_cpu) else None
+
+    s = dh.Solver(n, n, n, gamma=wl.gamma, dtype=torch.float32, kernel=a.kernel, cooling=int(a.cooling),
+                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def fwd_step():
+        s.cfl_dt_async(U)
+        s.step_devdt(U)
+
+    # a state that fits in the 126 MB L2 (n <= 128) is evicted between iterations by writing a 512 MB buffer;
+    # the flush is outside the per-iteration event pairs
+    fits_l2 = 5 * 4 * N <= 4 * 126e6
+    flush = torch.empty(128 * 1024 * 1024, device=dev, dtype=torch.float32) if fits_l2 else None
+
+    def timed(fn, iters):
+        """K calls bracketed by barrier + synchronize on both sides, CUDA events on the launching stream; the
+        max over ranks is taken by the caller."""
+        barrier()
+        l0 = s.launch_count
+        t0 = time.time()
+        if flush is None:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(iters):
+                fn()
+            e1.record()
+            barrier()
+            ms = e0.elapsed_time(e1)
+        else:
+            pairs = []
+            for _ in range(iters):
+                flush.zero_()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                fn()
+                e1.record()
+                pairs.append((e0, e1))
+            barrier()
+            ms = sum(x.elapsed_time(y) for x, y in pairs)
+        t1 = time.time()
+        return ms, s.launch_count - l0, t0, t1
+
+    def max_over_ranks(ms):
+        if world == 1:
+            return ms
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    # ---- forward: warm-up, then the timed region with per-kernel events and the clock sampler running
+    for _ in range(W):
+        fwd_step()
+    dt_w = s.poll()                                        # raises on a non-finite state
+    s.profile(True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    ms_fwd, launches, t0, t1 = timed(fwd_step, K)
+    clocks = sampler.stop(t0, t1) if sampler else None
+    prof = s.profile_read()
+    dt_last = s.poll()
+    ms_fwd = max_over_ranks(ms_fwd)
+    value = world * N * K / (ms_fwd * 1e-3)
+
+    peak, peak_src = measured_peak()
+    gbs = lambda words, ms, cnt: (words * 4.0 * N * cnt) / (ms * 1e-3) / 1e9 if ms > 0 else None
+    st_ms = prof["stage1"][0] + prof["stage2"][0]
+    st_cnt = prof["stage1"][1] + prof["stage2"][1]
+    st_bytes = 4.0 * N * (STAGE_WORDS["stage1"] * prof["stage1"][1] + STAGE_WORDS["stage2"] * prof["stage2"][1])
+    achieved = st_bytes / (st_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "stage kernel (predictor + corrector launches of the same kernel)",
+                "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": committed_traffic(n), "bytes_per_launch": st_bytes / max(st_cnt, 1),
+                "ms_per_launch": st_ms / max(st_cnt, 1),
+                "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
+                                   "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
+                               for k, v in prof.items() if v[1] > 0},
+                "step_GB/s": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9,
+                "step_frac": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9 / peak}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
+                       "cfl": 0.4, "limiter": "minmod", "riemann": "hllc", "integrator": "rk2 predictor/corrector",
+                       "cooling": bool(a.cooling), "kernel": a.kernel, "parallelism": f"replicas x{world}",
+                       "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
+                       if fits_l2 else f"inputs larger than L2 ({5 * 4 * N / 1e6:.0f} MB per state vs 126 MB), no flush",
+                       "dt_last": dt_last},
+            "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
+    s.profile(False)
+
+    # ---- VJP of the step, same state, seeded Gaussian cotangent on all five fields (configs[4])
+    if not a.no_vjp:
+        g = workloads.cotangent(U.shape, seed=2005 + rank, dtype=torch.float32, device=dev)
+        gin = torch.empty_like(U)
+        vjp = lambda: s.step_vjp(U, dt_last, g, gin)
+        for _ in range(min(W, 2)):
+            vjp()
+        s.profile(True)
+        Kv = max(1, min(K, 5))
+        ms_v, launches_v, _, _ = timed(vjp, Kv)
+        pv = s.profile_read()
+        s.profile(False)
+        ms_v = max_over_ranks(ms_v)
+        if not bool(torch.isfinite(gin[:, :2]).all()):
+            raise RuntimeError("non-finite VJP result")
+        line["vjp"] = {"value": world * N * Kv / (ms_v * 1e-3), "unit": "cell-VJPs/s", "steps": Kv, "ms_per_step": ms_v / Kv,
+                       "gpu_launches": launches_v,
+                       "roofline": {"bound": "hbm", "achieved": VJP_WORDS * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9, "peak": peak,
+                                    "unit": "GB/s", "frac": VJP_WORDS * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9 / peak,
+                                    "words_per_cell": VJP_WORDS,
+                                    "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
+                                                       "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
+                                                   for k, v in pv.items() if v[1] > 0}}}
+        line["gpu_launches"] += launches_v
+        del g, gin
+        torch.cuda.empty_cache()
+
+    # ---- end to end: pinned HOST state -> dh_run_host (H2D, CFL + step, D2H) -> HOST, all inside the timed region
+    if not a.no_e2e:
+        try:
+            import psutil
+            avail = psutil.virtual_memory().available
+        except Exception:
+            avail = 1 << 62
+        state_bytes = 5 * 4 * N
+        if avail < 2.5 * state_bytes:
+            line["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes,
+                           "note": f"skipped: host has {avail / 1e9:.0f} GB available, the pinned state needs {state_bytes / 1e9:.1f} GB"}
+        else:
+            h = torch.empty(U.shape, dtype=torch.float32, pin_memory=True)
+            h.copy_(U)
+            torch.cuda.synchronize()
+            Ke = max(1, min(K, 3))
+            s.run_host(h, 1)                                  # warm-up (allocates the library's device state)
+            barrier()
+            t0 = time.perf_counter()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(Ke):
+                s.run_host(h, 1)
+            e1.record()
+            barrier()
+            wall = time.perf_counter() - t0
+            ms_e = max_over_ranks(max(e0.elapsed_time(e1), wall * 1e3))
+            line["e2e"] = {"value": world * N * Ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": state_bytes,
+                           "d2h_bytes_per_step": state_bytes, "steps": Ke, "ms_per_step": ms_e / Ke,
+                           "host_link_GB/s": 2 * state_bytes * Ke / (ms_e * 1e-3) / 1e9,
+                           "call": "dh_run_host(ctx, U_host, 1, &dt): pinned H2D + CFL + RK2 step + D2H + sync"}
+            del h
+
+    # ---- the oracle beside it, on this box's host cores (rank 0, N = 1 only)
+    if U_cpu_block is not None:
+        import oracle
+
+        oracle.build()
+        line["cpu_baseline"] = oracle_sample(U_cpu_block, wl.gamma, bool(a.cooling), with_vjp=not a.no_vjp)
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_dh(a)
+
+
+if __name__ == "__main__":
+    main()

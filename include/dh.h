@@ -125,6 +125,23 @@ int dh_step_vjp_host(dh_ctx* ctx, const void* U_host, double dt, const void* gU_
 /* Number of kernel launches issued by this context since creation (bench.py's gpu_launches). */
 unsigned long long dh_launch_count(const dh_ctx* ctx);
 
+/* Per-kernel device timing (used by bench.py for the roofline of each kernel).  While enabled, every kernel
+ * launch of this context is bracketed by a pair of CUDA events on the context's stream.  dh_profile_read
+ * synchronises the stream and ADDS the elapsed milliseconds / launch counts recorded since the last read into
+ * ms_out[DH_K_COUNT_] / launches_out[DH_K_COUNT_] (HOST arrays the caller zeroes; either may be NULL). */
+enum {
+  DH_K_CFL_REDUCE = 0,   /* max-wavespeed reduction, Eq. A8 */
+  DH_K_CFL_FINISH = 1,   /* one-thread dt epilogue */
+  DH_K_STAGE1 = 2,       /* predictor stage  U* = U^n - dt/2 D(U^n) */
+  DH_K_STAGE2 = 3,       /* corrector stage  U^{n+1} = U^n - dt D(U*) (+ cooling) */
+  DH_K_REV2 = 4,         /* reverse corrector */
+  DH_K_REV1 = 5,         /* reverse predictor */
+  DH_K_COOL_VJP = 6,     /* pointwise cooling adjoint */
+  DH_K_COUNT_ = 7
+};
+int dh_profile_enable(dh_ctx* ctx, int on);
+int dh_profile_read(dh_ctx* ctx, double* ms_out, unsigned long long* launches_out);
+
 /* Message describing the last error on the calling thread ("" if none). */
 const char* dh_last_error(void);
 

@@ -2,6 +2,7 @@
 // dh_cfl_dt / dh_step / dh_step_vjp.  No arithmetic of the scheme lives here.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -61,6 +62,38 @@ static int lazy_alloc(dh_ctx* c, void** slot, size_t bytes, const char* what) {
   return DH_OK;
 }
 
+// Brackets one kernel launch with a pair of events while profiling is on (RAII: start in the constructor,
+// stop in the destructor, both on the context's stream).
+struct ProfScope {
+  dh_ctx* c;
+  ProfRec* r;
+  ProfScope(dh_ctx* ctx, int kind) : c(ctx), r(nullptr) {
+    if (!c->prof_on) return;
+    if (c->prof_n == c->prof_cap) {
+      int cap = c->prof_cap ? 2 * c->prof_cap : 256;
+      ProfRec* q = (ProfRec*)realloc(c->prof, (size_t)cap * sizeof(ProfRec));
+      if (!q) return;
+      c->prof = q;
+      c->prof_cap = cap;
+    }
+    ProfRec* rec = &c->prof[c->prof_n];
+    rec->kind = kind;
+    if (cudaEventCreate(&rec->a) != cudaSuccess) return;
+    if (cudaEventCreate(&rec->b) != cudaSuccess) { cudaEventDestroy(rec->a); return; }
+    cudaEventRecord(rec->a, c->stream);
+    c->prof_n += 1;
+    r = rec;
+  }
+  ~ProfScope() {
+    if (r) cudaEventRecord(r->b, c->stream);
+  }
+};
+
+static void prof_drop(dh_ctx* c) {
+  for (int i = 0; i < c->prof_n; ++i) { cudaEventDestroy(c->prof[i].a); cudaEventDestroy(c->prof[i].b); }
+  c->prof_n = 0;
+}
+
 extern "C" {
 
 const char* dh_last_error(void) { return g_err; }
@@ -112,6 +145,8 @@ void dh_destroy(dh_ctx* c) {
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
+  prof_drop(c);
+  free(c->prof);
   delete c;
 }
 
@@ -162,6 +197,31 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
 
 unsigned long long dh_launch_count(const dh_ctx* c) { return c ? c->launches : 0ull; }
 
+int dh_profile_enable(dh_ctx* c, int on) {
+  if (!c) return fail(DH_ERR_ARG, "dh_profile_enable: NULL context%s");
+  if (!on) {
+    DH_CUDA(cudaStreamSynchronize(c->stream), "dh_profile_enable: synchronize");
+    prof_drop(c);
+  }
+  c->prof_on = on ? 1 : 0;
+  return DH_OK;
+}
+
+int dh_profile_read(dh_ctx* c, double* ms_out, unsigned long long* launches_out) {
+  if (!c) return fail(DH_ERR_ARG, "dh_profile_read: NULL context%s");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_profile_read: synchronize");
+  for (int i = 0; i < c->prof_n; ++i) {
+    const ProfRec& r = c->prof[i];
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess && r.kind >= 0 && r.kind < DH_K_COUNT_) {
+      if (ms_out) ms_out[r.kind] += (double)ms;
+      if (launches_out) launches_out[r.kind] += 1ull;
+    }
+  }
+  prof_drop(c);
+  return DH_OK;
+}
+
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------ CFL
@@ -180,14 +240,21 @@ static int cfl_launch(dh_ctx* c, const void* U) {
   p.acc = c->acc;
   p.dt_dev = (T*)c->dt_dev;
   p.result = c->result_dev;
-  DH_CUDA(launch_cfl<T>(p, c->sm_count, c->stream), "dh_cfl_dt: kernel launch");
+  {
+    ProfScope ps(c, DH_K_CFL_REDUCE);
+    DH_CUDA(launch_cfl_reduce<T>(p, c->sm_count, c->stream), "dh_cfl_dt: reduction kernel launch");
+  }
+  {
+    ProfScope ps(c, DH_K_CFL_FINISH);
+    DH_CUDA(launch_cfl_finish<T>(p, c->stream), "dh_cfl_dt: epilogue kernel launch");
+  }
   c->launches += 2;
   return DH_OK;
 }
 
 // ------------------------------------------------------------------------------------------ forward
 template <class T>
-static int stage_launch(dh_ctx* c, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool) {
+static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool) {
   StageParams<T> p;
   p.U = (const T*)U; p.B = (const T*)B; p.out = (T*)out;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
@@ -198,6 +265,7 @@ static int stage_launch(dh_ctx* c, const void* U, const void* B, void* out, doub
   p.frac = (T)frac;
   p.cool = cool ? 1 : 0;
   p.c = make_consts<T>(c);
+  ProfScope ps(c, kind);
   bool done = false;
   if (c->kernel == 0) {
     bool supported = false;
@@ -215,14 +283,14 @@ static int stage_launch(dh_ctx* c, const void* U, const void* B, void* out, doub
 template <class T>
 static int step_impl(dh_ctx* c, void* U, double dt, bool devdt) {
   // predictor: U* = U^n - dt/2 D(U^n)   (Eq. A6);  corrector, in place: U^{n+1} = U^n - dt D(U*)   (Eq. A7)
-  int rc = stage_launch<T>(c, U, U, c->Us, dt, devdt, 0.5, false);
+  int rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 0.5, false);
   if (rc) return rc;
-  return stage_launch<T>(c, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0);
+  return stage_launch<T>(c, DH_K_STAGE2, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0);
 }
 
 // ------------------------------------------------------------------------------------------ reverse
 template <class T>
-static int rev_launch(dh_ctx* c, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
   RevParams<T> p;
   p.U = (const T*)U; p.g = (const T*)g; p.b1 = (const T*)b1; p.b2 = (const T*)b2; p.out = (T*)out;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
@@ -231,6 +299,7 @@ static int rev_launch(dh_ctx* c, const void* U, const void* g, const void* b1, c
   p.dt = (T)dt;
   p.frac = (T)frac;
   p.c = make_consts<T>(c);
+  ProfScope ps(c, kind);
   DH_CUDA(launch_rev_naive<T>(p, c->limiter, c->stream), "dh_step_vjp: reverse stage kernel launch");
   c->launches += 1;
   return DH_OK;
@@ -241,7 +310,7 @@ static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void*
   int rc = lazy_alloc(c, &c->gs, state_bytes(c), "the U* cotangent state");
   if (rc) return rc;
   // recompute U* = U^n - dt/2 D(U^n)  (nothing was stored by dh_step)
-  rc = stage_launch<T>(c, U, U, c->Us, dt, false, 0.5, false);
+  rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, false, 0.5, false);
   if (rc) return rc;
   const void* g1 = gout;
   if (c->cooling) {
@@ -250,18 +319,19 @@ static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void*
     if (rc) return rc;
     rc = lazy_alloc(c, &c->g1, state_bytes(c), "the pre-cooling cotangent");
     if (rc) return rc;
-    rc = stage_launch<T>(c, c->Us, U, c->U1, dt, false, 1.0, false);
+    rc = stage_launch<T>(c, DH_K_STAGE2, c->Us, U, c->U1, dt, false, 1.0, false);
     if (rc) return rc;
+    ProfScope ps(c, DH_K_COOL_VJP);
     DH_CUDA(launch_cool_vjp<T>((const T*)c->U1, (const T*)gout, (T*)c->g1, c->N, (T)dt, make_consts<T>(c), c->stream),
             "dh_step_vjp: cooling reverse kernel launch");
     c->launches += 1;
     g1 = c->g1;
   }
   // reverse corrector:  gs = -dt J_D(U*)^T g1
-  rc = rev_launch<T>(c, c->Us, g1, nullptr, nullptr, c->gs, dt, 1.0);
+  rc = rev_launch<T>(c, DH_K_REV2, c->Us, g1, nullptr, nullptr, c->gs, dt, 1.0);
   if (rc) return rc;
   // reverse predictor:  g_in = g1 + gs - dt/2 J_D(U^n)^T gs
-  return rev_launch<T>(c, U, c->gs, g1, c->gs, gin, dt, 0.5);
+  return rev_launch<T>(c, DH_K_REV1, U, c->gs, g1, c->gs, gin, dt, 0.5);
 }
 
 extern "C" {

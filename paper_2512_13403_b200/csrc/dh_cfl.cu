@@ -138,7 +138,7 @@ __global__ void cfl_finish_kernel(const CflParams<T> p) {
 }
 
 template <class T>
-cudaError_t launch_cfl(const CflParams<T>& p, int sm_count, cudaStream_t s) {
+cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s) {
   constexpr int W = Vec<T>::W;
   size_t work = (p.N % W == 0) ? p.N / W : p.N;
   size_t want = (work + 255) / 256;
@@ -146,13 +146,18 @@ cudaError_t launch_cfl(const CflParams<T>& p, int sm_count, cudaStream_t s) {
   int blocks = (int)(want < cap ? want : cap);
   if (blocks < 1) blocks = 1;
   cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
+  return cudaGetLastError();
+}
+
+template <class T>
+cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s) {
   cfl_finish_kernel<T><<<1, 1, 0, s>>>(p);
   return cudaGetLastError();
 }
 
-template cudaError_t launch_cfl<float>(const CflParams<float>&, int, cudaStream_t);
-template cudaError_t launch_cfl<double>(const CflParams<double>&, int, cudaStream_t);
+template cudaError_t launch_cfl_reduce<float>(const CflParams<float>&, int, cudaStream_t);
+template cudaError_t launch_cfl_reduce<double>(const CflParams<double>&, int, cudaStream_t);
+template cudaError_t launch_cfl_finish<float>(const CflParams<float>&, cudaStream_t);
+template cudaError_t launch_cfl_finish<double>(const CflParams<double>&, cudaStream_t);
 
 }  // namespace dh

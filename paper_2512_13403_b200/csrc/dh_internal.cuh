@@ -77,6 +77,15 @@ struct Ctx {
   CflResult* result_dev;
   CflResult* result_host;      // pinned
   unsigned long long launches;
+  // per-kernel event timing (dh_profile_enable / dh_profile_read)
+  int prof_on;
+  struct ProfRec* prof;        // pending (kind, start, stop) records
+  int prof_n, prof_cap;
+};
+
+struct ProfRec {
+  int kind;
+  cudaEvent_t a, b;
 };
 
 size_t elem_size(const Ctx* c);
@@ -86,6 +95,7 @@ template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int l
 template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
-template <class T> cudaError_t launch_cfl(const CflParams<T>& p, int sm_count, cudaStream_t s);   // 2 launches
+template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
+template <class T> cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s);
 
 }  // namespace dh

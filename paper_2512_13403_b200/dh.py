@@ -28,8 +28,9 @@ KERNELS = {"fused": 0, "gather": 1}
 SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
-    "dh_launch_count", "dh_last_error", "dh_version",
+    "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
 ]
+KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp"]
 
 _lib = None
 
@@ -66,10 +67,13 @@ def load(rebuild: bool = False):
     lib.dh_step_vjp_host.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_launch_count.restype = ctypes.c_ulonglong
     lib.dh_launch_count.argtypes = [vp]
+    lib.dh_profile_enable.argtypes = [vp, ci]
+    lib.dh_profile_read.argtypes = [vp, pd, ctypes.POINTER(ctypes.c_ulonglong)]
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
-               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host"):
+               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host", "dh_profile_enable",
+               "dh_profile_read"):
         getattr(lib, fn).restype = ci
     _lib = lib
     return lib
@@ -161,6 +165,19 @@ def dh_launch_count(ctx) -> int:
     return int(load().dh_launch_count(ctx))
 
 
+def dh_profile_enable(ctx, on: bool) -> None:
+    _check(load().dh_profile_enable(ctx, 1 if on else 0))
+
+
+def dh_profile_read(ctx) -> dict:
+    """{kernel kind: (milliseconds, launches)} recorded since the last read."""
+    n = len(KERNEL_KINDS)
+    ms = (ctypes.c_double * n)()
+    cnt = (ctypes.c_ulonglong * n)()
+    _check(load().dh_profile_read(ctx, ms, cnt))
+    return {k: (ms[i], int(cnt[i])) for i, k in enumerate(KERNEL_KINDS)}
+
+
 # ------------------------------------------------------------------------------------------- convenience
 class Solver:
     """A dh context bound to a grid; states are torch CUDA tensors [5, nz, ny, nx]."""
@@ -226,6 +243,12 @@ class Solver:
     def step_vjp_host(self, U_host, dt: float, g_out_host, g_in_host) -> None:
         dh_step_vjp_host(self.ctx, self._host(U_host, "U_host"), dt, self._host(g_out_host, "g_out_host"),
                          self._host(g_in_host, "g_in_host"))
+
+    def profile(self, on: bool) -> None:
+        dh_profile_enable(self.ctx, on)
+
+    def profile_read(self) -> dict:
+        return dh_profile_read(self.ctx)
 
     @property
     def launch_count(self) -> int:
