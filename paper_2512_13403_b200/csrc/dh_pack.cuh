@@ -1,0 +1,141 @@
+// dh_pack.cuh — two-cell "pack" arithmetic for the fused kernels (sm_100a).
+//
+// The fused stage kernels give every thread TWO cells adjacent in x and run the same instruction stream on
+// both.  For fp32 the add / mul / fma of such a pair is ONE packed instruction on sm_100 (PTX add/mul/fma
+// .f32x2 -> SASS FADD2 / FMUL2 / FFMA2): the fp32 pipe time is unchanged but the issue slots halve, which
+// is what binds this kernel ("Kernels").  min / max / MUFU / select stay per lane.  For fp64
+// the pack is two scalars.
+#pragma once
+#include "dh_math.cuh"
+
+namespace dh {
+
+#define DH_DI __device__ __forceinline__
+
+template <class T> struct P2 { T x, y; };
+template <> struct alignas(8) P2<float> { float x, y; };
+template <> struct alignas(16) P2<double> { double x, y; };
+
+struct B2 { bool x, y; };
+
+// ---- fp32: packed PTX ----------------------------------------------------------------------------
+DH_DI unsigned long long pk_(P2<float> a) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+  return r;
+}
+DH_DI P2<float> upk_(unsigned long long r) {
+  P2<float> a;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+  return a;
+}
+DH_DI P2<float> add2(P2<float> a, P2<float> b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b)));
+  return upk_(r);
+}
+DH_DI P2<float> sub2(P2<float> a, P2<float> b) {
+  unsigned long long r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b)));
+  return upk_(r);
+}
+DH_DI P2<float> mul2(P2<float> a, P2<float> b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b)));
+  return upk_(r);
+}
+DH_DI P2<float> fma2(P2<float> a, P2<float> b, P2<float> c) {   // a*b + c
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk_(a)), "l"(pk_(b)), "l"(pk_(c)));
+  return upk_(r);
+}
+// a*b - c and c - a*b: two scalar FFMA with a free operand negation (no packed negate exists)
+DH_DI P2<float> fms2(P2<float> a, P2<float> b, P2<float> c) { return {fmaf(a.x, b.x, -c.x), fmaf(a.y, b.y, -c.y)}; }
+DH_DI P2<float> fnma2(P2<float> a, P2<float> b, P2<float> c) { return {fmaf(-a.x, b.x, c.x), fmaf(-a.y, b.y, c.y)}; }
+
+// ---- fp64: two scalars ---------------------------------------------------------------------------
+DH_DI P2<double> add2(P2<double> a, P2<double> b) { return {a.x + b.x, a.y + b.y}; }
+DH_DI P2<double> sub2(P2<double> a, P2<double> b) { return {a.x - b.x, a.y - b.y}; }
+DH_DI P2<double> mul2(P2<double> a, P2<double> b) { return {a.x * b.x, a.y * b.y}; }
+DH_DI P2<double> fma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)}; }
+DH_DI P2<double> fms2(P2<double> a, P2<double> b, P2<double> c) { return {fma(a.x, b.x, -c.x), fma(a.y, b.y, -c.y)}; }
+DH_DI P2<double> fnma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(-a.x, b.x, c.x), fma(-a.y, b.y, c.y)}; }
+
+// ---- per-lane operations -------------------------------------------------------------------------
+DH_DI float rsqrt_(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+DH_DI double rsqrt_(double x) { return 1.0 / sqrt(x); }
+
+template <class T> DH_DI P2<T> bc2(T s) { return {s, s}; }
+template <class T> DH_DI P2<T> min2(P2<T> a, P2<T> b) { return {min_(a.x, b.x), min_(a.y, b.y)}; }
+template <class T> DH_DI P2<T> max2(P2<T> a, P2<T> b) { return {max_(a.x, b.x), max_(a.y, b.y)}; }
+template <class T> DH_DI P2<T> min2(P2<T> a, T b) { return {min_(a.x, b), min_(a.y, b)}; }
+template <class T> DH_DI P2<T> max2(P2<T> a, T b) { return {max_(a.x, b), max_(a.y, b)}; }
+template <class T> DH_DI P2<T> rcp2(P2<T> a) { return {rcp_(a.x), rcp_(a.y)}; }
+template <class T> DH_DI P2<T> rsqrt2(P2<T> a) { return {rsqrt_(a.x), rsqrt_(a.y)}; }
+template <class T> DH_DI P2<T> sel2(B2 m, P2<T> a, P2<T> b) { return {m.x ? a.x : b.x, m.y ? a.y : b.y}; }
+template <class T> DH_DI B2 ge2(P2<T> a, T b) { return {a.x >= b, a.y >= b}; }
+
+// ---- scheme pieces on packs ----------------------------------------------------------------------
+// primitives of two cells (Eq. 2); same arithmetic as prim() in dh_math.cuh
+template <class T>
+DH_DI void prim2(const P2<T> U[5], const Consts<T>& c, P2<T> W[5]) {
+  const P2<T> rho = max2(U[0], c.rho_floor);
+  const P2<T> r = rcp2(rho);
+  const P2<T> vx = mul2(U[1], r), vy = mul2(U[2], r), vz = mul2(U[3], r);
+  const P2<T> q = fma2(U[3], vz, fma2(U[2], vy, mul2(U[1], vx)));   // |m|^2 / rho
+  W[0] = rho; W[1] = vx; W[2] = vy; W[3] = vz;
+  W[4] = max2(mul2(bc2(c.gm1), fnma2(bc2(T(0.5)), q, U[4])), c.p_floor);
+}
+
+// limited slope of both cells: a = W_{+1} - W, b = W - W_{-1}  (Eq. A1)
+template <class T, int LIM>
+DH_DI P2<T> limit2(P2<T> a, P2<T> b) { return {limit<T, LIM>(a.x, b.x), limit<T, LIM>(a.y, b.y)}; }
+
+// HLLC flux of two faces with normal axis AX (Eq. A3 for the wave speeds); the same
+// arrangement as hllc() in dh_math.cuh: star state on the upwind side only, supersonic branches folded
+// into S_eff = min(S_L, 0) / max(S_R, 0), transverse momentum flux = v_t * F_mass, one rsqrt per sound
+// speed (c = gP * rsqrt(gP * rho)), E_K formed without a density reciprocal.
+template <class T, int AX>
+DH_DI void hllc2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F[5]) {
+  constexpr int n = 1 + AX, t1 = 1 + (AX + 1) % 3, t2 = 1 + (AX + 2) % 3;
+  const P2<T> g = bc2(c.gamma);
+  const P2<T> gPL = mul2(g, L[4]), gPR = mul2(g, R[4]);
+  const P2<T> cL = mul2(gPL, rsqrt2(mul2(gPL, L[0]))), cR = mul2(gPR, rsqrt2(mul2(gPR, R[0])));
+  const P2<T> uL = L[n], uR = R[n];
+  const P2<T> SL = min2(sub2(uL, cL), sub2(uR, cR));          // Eq. A3
+  const P2<T> SR = max2(add2(uL, cL), add2(uR, cR));
+  const P2<T> dL = sub2(SL, uL), dR = sub2(SR, uR);
+  const P2<T> aL = mul2(L[0], dL), aR = mul2(R[0], dR);
+  const P2<T> num = fnma2(aR, uR, fma2(aL, uL, sub2(R[4], L[4])));
+  const P2<T> Ss = mul2(num, rcp2(sub2(aL, aR)));             // contact speed S*
+  const B2 left = ge2(Ss, T(0));
+  const P2<T> rhoK = sel2(left, L[0], R[0]), uK = sel2(left, uL, uR);
+  const P2<T> v1 = sel2(left, L[t1], R[t1]), v2 = sel2(left, L[t2], R[t2]);
+  const P2<T> PK = sel2(left, L[4], R[4]), aK = sel2(left, aL, aR), dK = sel2(left, dL, dR);
+  const P2<T> Seff = sel2(left, min2(SL, T(0)), max2(SR, T(0)));   // 0 in the supersonic branches -> F = F_K
+  const P2<T> q = fma2(v2, v2, fma2(v1, v1, mul2(uK, uK)));
+  const P2<T> EK = fma2(mul2(bc2(T(0.5)), rhoK), q, mul2(bc2(c.inv_gm1), PK));
+  const P2<T> mK = mul2(rhoK, uK);
+  const P2<T> Y = sub2(Ss, uK);
+  const P2<T> inv = rcp2(sub2(dK, Y));                        // 1 / (S_K - S*)
+  const P2<T> fac = mul2(aK, inv);                            // rho*_K
+  const P2<T> Fm = fma2(Seff, sub2(fac, rhoK), mK);
+  const P2<T> Z = fma2(aK, Ss, PK);
+  const P2<T> Es = mul2(inv, fma2(Y, Z, mul2(dK, EK)));       // E*_K
+  F[0] = Fm;
+  F[n] = fma2(Seff, fms2(fac, Ss, mK), fma2(mK, uK, PK));
+  F[t1] = mul2(v1, Fm);
+  F[t2] = mul2(v2, Fm);
+  F[4] = fma2(Seff, sub2(Es, EK), mul2(uK, add2(EK, PK)));
+}
+
+// cooling of two finished cells (Eqs. 23-24); per lane
+template <class T>
+DH_DI void cool2(P2<T> U[5], T dt, const Consts<T>& c) {
+  T a[5] = {U[0].x, U[1].x, U[2].x, U[3].x, U[4].x};
+  T b[5] = {U[0].y, U[1].y, U[2].y, U[3].y, U[4].y};
+  U[4].x = cool_energy(a, dt, c);
+  U[4].y = cool_energy(b, dt, c);
+}
+
+}  // namespace dh
