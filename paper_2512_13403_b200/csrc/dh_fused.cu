@@ -34,7 +34,8 @@ template <int NW> struct Geo {
   static constexpr int PLANE = 5 * SR * SW;               // one buffered primitive plane (all 5 fields)
   static constexpr int XARR = 5 * TY * XP;
   static constexpr int YARR = 5 * (TY + 1) * TX;
-  static constexpr int TOTAL = 2 * PLANE + 2 * XARR + 2 * YARR;
+  static constexpr int STAGE = 5 * TY * TX;                // cp.async staging of one raw row-warp plane (all 5 fields)
+  static constexpr int TOTAL = 2 * PLANE + 2 * XARR + 2 * YARR + 2 * STAGE;
   static constexpr int NHALO = 4 * (SW / 2) + 2 * TY;     // halo packs per plane
   static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
 };
@@ -49,24 +50,31 @@ template <class T> DH_DI void sts2(T* p, P2<T> v) { *reinterpret_cast<P2<T>*>(p)
 template <class T> DH_DI P2<T> ldg2(const T* p) { return *reinterpret_cast<const P2<T>*>(p); }
 template <class T> DH_DI void stg2(T* p, P2<T> v) { *reinterpret_cast<P2<T>*>(p) = v; }
 
+// 8-byte (fp32 pack) / 16-byte (fp64 pack) asynchronous global -> shared copy of one pack (LDGSTS)
+template <class T> DH_DI void cp_async_pack(T* smem_dst, const T* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+DH_DI void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> DH_DI void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 // slopes of the two cells of a pack along x from the scalar neighbours wl (left of .x) and wr (right of .y);
 // returns the L (= W + s/2) and R (= W - s/2) states of both cells
 template <class T, int LIM>
 DH_DI void recon_x(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
   const T d0 = W.x - wl, d1 = W.y - W.x, d2 = wr - W.y;
-  const P2<T> s = {limit<T, LIM>(d1, d0), limit<T, LIM>(d2, d1)};
-  const P2<T> h = bc2(T(0.5));
-  L = fma2(h, s, W);
-  R = fnma2(h, s, W);
+  const P2<T> s = {limit1<T, LIM>(d1, d0), limit1<T, LIM>(d2, d1)};
+  L = fma2(bc2(T(0.5)), s, W);
+  R = fma2(bc2(T(-0.5)), s, W);
 }
 
 // slopes along y or z from the packs below (Wm) and above (Wp)
 template <class T, int LIM>
 DH_DI void recon_p(P2<T> Wm, P2<T> W, P2<T> Wp, P2<T>& L, P2<T>& R) {
   const P2<T> s = limit2<T, LIM>(sub2(Wp, W), sub2(W, Wm));
-  const P2<T> h = bc2(T(0.5));
-  L = fma2(h, s, W);
-  R = fnma2(h, s, W);
+  L = fma2(bc2(T(0.5)), s, W);
+  R = fma2(bc2(T(-0.5)), s, W);
 }
 
 }  // namespace
@@ -82,6 +90,8 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
   T* const Fxs = Rxs + G::XARR;                    // [5][TY][XP]     x flux through the LEFT face of lane l's pack
   T* const Rys = Fxs + G::XARR;                    // [5][TY+1][TX]   R states of row r (r = TY: halo row)
   T* const Fys = Rys + G::YARR;                    // [5][TY+1][TX]   y flux through the BOTTOM face of row r
+  T* const Ust = Fys + G::YARR;                    // [5][TY][TX]     raw U of the next plane (cp.async, private per thread)
+  T* const Bst = Ust + G::STAGE;                   // [5][TY][TX]     base state of plane p-1 (cp.async, private per thread)
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -93,7 +103,7 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
   const T tau = p.frac * dt;
   const P2<T> ncx = bc2(-tau * p.inv_dx[0]), ncy = bc2(-tau * p.inv_dx[1]);
   const P2<T> cz = bc2(tau * p.inv_dx[2]), ncz = bc2(-tau * p.inv_dx[2]);
-  const P2<T> half = bc2(T(0.5));
+  const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
   const Consts<T>& c = p.c;
 
   if (w < TY) {
@@ -103,30 +113,40 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
     const bool store_ok = (x0 + 2 * lane < nx) && (y0 + r < ny);
     const int so = (r + 2) * SW + 2 * lane + 2;    // own pack inside a shared plane
     const int xo = r * XP + lane, yo = r * TX + 2 * lane;
-    P2<T> Wprev[5], dprev[5], WLz[5], acc[5], Un[5];
+    T* const ust = Ust + yo;                       // this thread's staging slots (stride TY*TX per field)
+    T* const bst = Bst + yo;
+    constexpr int FS = TY * TX;
+    P2<T> Wprev[5], dprev[5], WLz[5], acc[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) Wprev[f] = dprev[f] = WLz[f] = acc[f] = bc2(T(0));
-    int pz = wrapm(z0 - 2, nz), pzm1 = pz, pzm2 = pz;
+    // element offsets of this thread's pack in planes p, p-1, p-2 (64-bit: 5 N words may exceed 2^32 bytes)
+    int pz = wrapm(z0 - 2, nz);
+    size_t op = (size_t)pz * NP + o, opm1 = op, opm2 = op;
 #pragma unroll
-    for (int f = 0; f < 5; ++f) Un[f] = ldg2(p.U + f * N + pz * NP + o);
+    for (int f = 0; f < 5; ++f) cp_async_pack(ust + f * FS, p.U + f * N + op);
+    cp_async_commit();
 
 #pragma unroll 1
     for (int it = 0; it < nit; ++it) {
+      const bool xy = (it >= 3) && (it <= zl + 2);   // x/y work on plane p-1 = z0 + it - 3
+      cp_async_wait<0>();
       P2<T> Uc[5];
 #pragma unroll
-      for (int f = 0; f < 5; ++f) Uc[f] = Un[f];
-      int pzn = pz + 1;
-      if (pzn == nz) pzn = 0;
-      if (it + 1 < nit) {
-#pragma unroll
-        for (int f = 0; f < 5; ++f) Un[f] = ldg2(p.U + f * N + pzn * NP + o);
-      }
-      const bool xy = (it >= 3) && (it <= zl + 2);   // x/y work on plane p-1 = z0 + it - 3
-      P2<T> Bv[5];
+      for (int f = 0; f < 5; ++f) Uc[f] = lds2(ust + f * FS);
+      // base state of plane p-1 first (needed in this iteration), then the raw state of plane p+1
       if (xy) {
 #pragma unroll
-        for (int f = 0; f < 5; ++f) Bv[f] = ldg2(p.B + f * N + pzm1 * NP + o);
+        for (int f = 0; f < 5; ++f) cp_async_pack(bst + f * FS, p.B + f * N + opm1);
       }
+      cp_async_commit();
+      int pzn = pz + 1;
+      size_t opn = op + NP;
+      if (pzn == nz) { pzn = 0; opn = o; }
+      if (it + 1 < nit) {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) cp_async_pack(ust + f * FS, p.U + f * N + opn);
+      }
+      cp_async_commit();
       // primitives of plane p -> shared (read by the neighbours in the next iteration)
       P2<T> Wp[5];
       prim2(Uc, c, Wp);
@@ -135,26 +155,41 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) sts2(Wb + f * SR * SW, Wp[f]);
       }
-      // z: slope of cell p-1, face between p-2 and p-1
-      P2<T> Fz[5];
+      // z: slope of cell p-1, face between p-2 and p-1; the face flux finishes plane p-2 and opens plane p-1
       {
-        P2<T> Rz[5], Lz[5];
+        P2<T> Rz[5], Fz[5];
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           const P2<T> a = sub2(Wp[f], Wprev[f]);
           const P2<T> s = limit2<T, LIM>(a, dprev[f]);
-          Lz[f] = fma2(half, s, Wprev[f]);
-          Rz[f] = fnma2(half, s, Wprev[f]);
+          Rz[f] = fma2(nhalf, s, Wprev[f]);
           dprev[f] = a;
+          Wp[f] = fma2(half, s, Wprev[f]);         // left state of the NEXT z face (kept in WLz below)
         }
         if (it >= 3) hllc2<T, 2>(WLz, Rz, c, Fz);
 #pragma unroll
-        for (int f = 0; f < 5; ++f) WLz[f] = Lz[f];
+        for (int f = 0; f < 5; ++f) WLz[f] = Wp[f];
+        if (it >= 4) {
+          P2<T> Uo[5];
+#pragma unroll
+          for (int f = 0; f < 5; ++f) Uo[f] = fma2(ncz, Fz[f], acc[f]);
+          if (p.cool) cool2(Uo, dt, c);
+          if (store_ok) {
+#pragma unroll
+            for (int f = 0; f < 5; ++f) stg2(p.out + f * N + opm2, Uo[f]);
+          }
+        }
+        if (xy) {
+          cp_async_wait<1>();                      // the base-state group; the next-plane group may still fly
+#pragma unroll
+          for (int f = 0; f < 5; ++f) acc[f] = fma2(cz, Fz[f], lds2(bst + f * FS));
+        }
       }
+      // the primitives of plane p were overwritten above: reload them (own smem slot, no hazard)
+      const T* Wq = Wsm + ((it - 1) & 1) * G::PLANE + so;
       // x / y, phase 1: slopes of the own cells of plane p-1, publish the R states
       P2<T> Lx[5], Rxo[5], Ly[5];
       if (xy) {
-        const T* Wq = Wsm + ((it - 1) & 1) * G::PLANE + so;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           const T* row = Wq + f * SR * SW;
@@ -182,33 +217,25 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
         for (int f = 0; f < 5; ++f) sts2(Fys + f * (TY + 1) * TX + yo + TX, Fy[f]);
       }
       __syncthreads();
-      // finish plane p-2 (its top z face is Fz) and store it
-      if (it >= 4) {
-        P2<T> Uo[5];
-#pragma unroll
-        for (int f = 0; f < 5; ++f) Uo[f] = fma2(ncz, Fz[f], acc[f]);
-        if (p.cool) cool2(Uo, dt, c);
-        if (store_ok) {
-#pragma unroll
-          for (int f = 0; f < 5; ++f) stg2(p.out + f * N + pzm2 * NP + o, Uo[f]);
-        }
-      }
-      // phase 3: partial update of plane p-1 (x, y differences and its bottom z face)
+      // phase 3: x and y differences into the partial update of plane p-1
       if (xy) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           const T fl = Fxs[f * TY * XP + xo];
           const P2<T> dFx = {Fx[f].x - fl, Fx[f].y - Fx[f].x};
           const P2<T> Fb = lds2(Fys + f * (TY + 1) * TX + yo);
-          P2<T> a = fma2(ncx, dFx, Bv[f]);
-          a = fma2(ncy, sub2(Fy[f], Fb), a);
-          acc[f] = fma2(cz, Fz[f], a);
+          acc[f] = fma2(ncy, sub2(Fy[f], Fb), fma2(ncx, dFx, acc[f]));
         }
       }
+      // plane p becomes plane p-1
+      {
+        const T* Wn = Wsm + (it & 1) * G::PLANE + so;
 #pragma unroll
-      for (int f = 0; f < 5; ++f) Wprev[f] = Wp[f];
-      pzm2 = pzm1;
-      pzm1 = pz;
+        for (int f = 0; f < 5; ++f) Wprev[f] = lds2(Wn + f * SR * SW);
+      }
+      opm2 = opm1;
+      opm1 = op;
+      op = opn;
       pz = pzn;
     }
   } else {
@@ -261,9 +288,9 @@ stage_fused_kernel(const StageParams<T> p, const int ZL) {
           recon_p<T, LIM>(lds2(col), lds2(col + SW), lds2(col + 2 * SW), LyB[f], Rt);
           // x: L state of the halo column -1, R state of the halo column TX, row rl
           const T* rw = pl + (rl + 2) * SW;
-          const T sl = limit<T, LIM>(rw[2] - rw[1], rw[1] - rw[0]);
+          const T sl = limit1<T, LIM>(rw[2] - rw[1], rw[1] - rw[0]);
           LxB[f] = fma(T(0.5), sl, rw[1]);
-          const T sr = limit<T, LIM>(rw[TX + 3] - rw[TX + 2], rw[TX + 2] - rw[TX + 1]);
+          const T sr = limit1<T, LIM>(rw[TX + 3] - rw[TX + 2], rw[TX + 2] - rw[TX + 1]);
           if (lane < TY) Rxs[f * TY * XP + rl * XP + 32] = fma(T(-0.5), sr, rw[TX + 2]);
         }
       }

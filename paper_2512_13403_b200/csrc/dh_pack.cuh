@@ -52,6 +52,18 @@ DH_DI P2<float> fma2(P2<float> a, P2<float> b, P2<float> c) {   // a*b + c
 // a*b - c and c - a*b: two scalar FFMA with a free operand negation (no packed negate exists)
 DH_DI P2<float> fms2(P2<float> a, P2<float> b, P2<float> c) { return {fmaf(a.x, b.x, -c.x), fmaf(a.y, b.y, -c.y)}; }
 DH_DI P2<float> fnma2(P2<float> a, P2<float> b, P2<float> c) { return {fmaf(-a.x, b.x, c.x), fmaf(-a.y, b.y, c.y)}; }
+// minmod(a, b) in three ALU-pipe instructions: FMNMX.xorsign.abs gives +-min(|a|,|b|) with the sign positive
+// exactly when a and b agree in sign; clamping at 0 kills the disagreeing case; the sign of a is put back.
+DH_DI float minmod_(float a, float b) {
+  float d;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  d = fmaxf(d, 0.0f);
+  return __uint_as_float(__float_as_uint(d) | (__float_as_uint(a) & 0x80000000u));
+}
+DH_DI double minmod_(double a, double b) {
+  const double mn = fmin(a, b), mx = fmax(a, b);
+  return fmin(fmax(mn, 0.0), mx);
+}
 
 // ---- fp64: two scalars ---------------------------------------------------------------------------
 DH_DI P2<double> add2(P2<double> a, P2<double> b) { return {a.x + b.x, a.y + b.y}; }
@@ -89,7 +101,12 @@ DH_DI void prim2(const P2<T> U[5], const Consts<T>& c, P2<T> W[5]) {
 
 // limited slope of both cells: a = W_{+1} - W, b = W - W_{-1}  (Eq. A1)
 template <class T, int LIM>
-DH_DI P2<T> limit2(P2<T> a, P2<T> b) { return {limit<T, LIM>(a.x, b.x), limit<T, LIM>(a.y, b.y)}; }
+DH_DI T limit1(T a, T b) {
+  if (LIM == 0) return minmod_(a, b);
+  return limit<T, LIM>(a, b);
+}
+template <class T, int LIM>
+DH_DI P2<T> limit2(P2<T> a, P2<T> b) { return {limit1<T, LIM>(a.x, b.x), limit1<T, LIM>(a.y, b.y)}; }
 
 // HLLC flux of two faces with normal axis AX (Eq. A3 for the wave speeds); the same
 // arrangement as hllc() in dh_math.cuh: star state on the upwind side only, supersonic branches folded
