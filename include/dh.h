@@ -64,8 +64,9 @@ enum {
   DH_OPT_T_FLOOR = 7,    /* default 0.01; E_floor = rho T_floor / (gamma-1) (Eq. 24 with R = 1) */
   DH_OPT_RHO_FLOOR = 8,  /* floors used only inside the primitive conversion, default 1e-10 */
   DH_OPT_P_FLOOR = 9,
-  DH_OPT_KERNEL = 10,    /* 0 (default): fused z-sweep stage kernels; 1: one-thread-per-cell gather kernels
-                            (same arithmetic, kept for cross-checking and as the fallback for odd grid sizes) */
+  DH_OPT_KERNEL = 10,    /* 0 (default): fused z-sweep stage kernel, 2x2 cells per thread; 1: one-thread-per-cell gather
+                            kernels (same arithmetic, kept for cross-checking and as the fallback for odd nx);
+                            2: the first fused z-sweep kernel (one pack per thread), kept for comparison */
   DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
   DH_OPT_COUNT_
 };

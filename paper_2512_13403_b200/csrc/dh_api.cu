@@ -170,7 +170,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_T_FLOOR: c->t_floor = v; break;
     case DH_OPT_RHO_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->rho_floor = v; break;
     case DH_OPT_P_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->p_floor = v; break;
-    case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0 or 1%s"); c->kernel = (int)v; break;
+    case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0, 1 or 2%s"); c->kernel = (int)v; break;
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
@@ -268,6 +268,14 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
   ProfScope ps(c, kind);
   bool done = false;
   if (c->kernel == 0) {
+    bool supported = false;
+    cudaError_t e = launch_stage_fused2<T>(p, c->limiter, c->sm_count, c->stream, &supported);
+    if (supported) {
+      if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
+      done = true;
+    }
+  }
+  if (!done && c->kernel != 1) {
     bool supported = false;
     cudaError_t e = launch_stage_fused<T>(p, c->limiter, c->sm_count, c->stream, &supported);
     if (supported) {

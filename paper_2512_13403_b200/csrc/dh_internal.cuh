@@ -93,6 +93,7 @@ size_t elem_size(const Ctx* c);
 // launchers (each returns the cudaError_t of the launch)
 template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, cudaStream_t s);
 template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
+template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);

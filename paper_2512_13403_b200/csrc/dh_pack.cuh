@@ -66,9 +66,11 @@ DH_DI double minmod_(double a, double b) {
 }
 
 // ---- fp64: two scalars ---------------------------------------------------------------------------
-DH_DI P2<double> add2(P2<double> a, P2<double> b) { return {a.x + b.x, a.y + b.y}; }
-DH_DI P2<double> sub2(P2<double> a, P2<double> b) { return {a.x - b.x, a.y - b.y}; }
-DH_DI P2<double> mul2(P2<double> a, P2<double> b) { return {a.x * b.x, a.y * b.y}; }
+// (the _rn intrinsics are never contracted into FMAs, so every call site rounds identically: a face flux has the
+// same bits whichever warp computes it, which is what makes the step translation-equivariant bitwise)
+DH_DI P2<double> add2(P2<double> a, P2<double> b) { return {__dadd_rn(a.x, b.x), __dadd_rn(a.y, b.y)}; }
+DH_DI P2<double> sub2(P2<double> a, P2<double> b) { return {__dsub_rn(a.x, b.x), __dsub_rn(a.y, b.y)}; }
+DH_DI P2<double> mul2(P2<double> a, P2<double> b) { return {__dmul_rn(a.x, b.x), __dmul_rn(a.y, b.y)}; }
 DH_DI P2<double> fma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(a.x, b.x, c.x), fma(a.y, b.y, c.y)}; }
 DH_DI P2<double> fms2(P2<double> a, P2<double> b, P2<double> c) { return {fma(a.x, b.x, -c.x), fma(a.y, b.y, -c.y)}; }
 DH_DI P2<double> fnma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(-a.x, b.x, c.x), fma(-a.y, b.y, c.y)}; }
@@ -77,6 +79,8 @@ DH_DI P2<double> fnma2(P2<double> a, P2<double> b, P2<double> c) { return {fma(-
 DH_DI float rsqrt_(float x) { float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 DH_DI double rsqrt_(double x) { return 1.0 / sqrt(x); }
 
+DH_DI float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+DH_DI double fma_(double a, double b, double c) { return fma(a, b, c); }
 template <class T> DH_DI P2<T> bc2(T s) { return {s, s}; }
 template <class T> DH_DI P2<T> min2(P2<T> a, P2<T> b) { return {min_(a.x, b.x), min_(a.y, b.y)}; }
 template <class T> DH_DI P2<T> max2(P2<T> a, P2<T> b) { return {max_(a.x, b.x), max_(a.y, b.y)}; }

@@ -22,7 +22,7 @@ OPTIONS = {
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
-KERNELS = {"fused": 0, "gather": 1}
+KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 
 # every symbol include/dh.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
