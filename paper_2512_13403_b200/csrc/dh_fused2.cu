@@ -40,7 +40,7 @@ template <int NRW> struct Geo2 {
   static constexpr int FY = 5 * (NRW + 1) * TX2;           // top-face y fluxes: slot 0 helper, slot r+1 thread row r
   static constexpr int XE = 5 * TY * XP2;                  // x exchange (R states or fluxes), one slot set per row
   static constexpr int STAGE = 5 * TY * TX2;               // cp.async staging of one raw plane of the tile
-  static constexpr int TOTAL = 2 * PLANE + 2 * FY + 4 * XE + 2 * STAGE;
+  static constexpr int TOTAL = 2 * PLANE + 2 * FY + 4 * XE + 3 * STAGE;
   static constexpr int XPK = (TY * 4 + 31) / 32;           // x-edge packs per helper lane (4 per row)
 };
 
@@ -74,7 +74,7 @@ DH_DI void recon_x2(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
 }  // namespace
 
 template <class T, int LIM, int NRW>
-__global__ void __launch_bounds__((NRW + 1) * 32, (sizeof(T) == 4 && NRW <= 4) ? 2 : 1)
+__global__ void __launch_bounds__((NRW + 1) * 32, 1)
 stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   using G = Geo2<NRW>;
   constexpr int TY = G::TY, SR = G::SR, FP = SR * SW2;       // FP: field pitch inside a shared plane
@@ -85,7 +85,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   T* const Rxs = Fys + 2 * G::FY;                  // [2][5][TY][XP2]     R state of the first cell of lane l; slot 32: helper
   T* const Fxs = Rxs + 2 * G::XE;                  // [2][5][TY][XP2]     x flux through the LEFT face of lane l; slot 0: helper
   T* const Ust = Fxs + 2 * G::XE;                  // [5][TY][TX2]        raw U of the next plane (cp.async, private slots)
-  T* const Bst = Ust + G::STAGE;                   // [5][TY][TX2]        base state of plane p-1 (cp.async, private slots)
+  T* const Bst = Ust + G::STAGE;                   // [2][5][TY][TX2]     base state, loaded one plane ahead (cp.async, private slots)
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -132,13 +132,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       P2<T> NA[5], NB[5];                          // plane p: raw, then primitive
 #pragma unroll
       for (int f = 0; f < 5; ++f) { NA[f] = lds2_(Ust + f * FS + stA); NB[f] = lds2_(Ust + f * FS + stB); }
-      // base state of plane p-1 first (needed in this iteration), then the raw state of plane p+1
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        cp_async_pack2(Bst + f * FS + stA, p.B + f * N + opm1 + oA);
-        cp_async_pack2(Bst + f * FS + stB, p.B + f * N + opm1 + oB);
-      }
-      cp_async_commit2();
+      // one plane ahead: the raw state of plane p+1 and the base state of plane p (used in the next iteration)
       int pzn = pz + 1;
       size_t opn = op + NP;
       if (pzn == nz) { pzn = 0; opn = 0; }
@@ -146,6 +140,8 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       for (int f = 0; f < 5; ++f) {
         cp_async_pack2(Ust + f * FS + stA, p.U + f * N + opn + oA);
         cp_async_pack2(Ust + f * FS + stB, p.U + f * N + opn + oB);
+        cp_async_pack2(Bst + bp * G::STAGE + f * FS + stA, p.B + f * N + op + oA);
+        cp_async_pack2(Bst + bp * G::STAGE + f * FS + stB, p.B + f * N + op + oB);
       }
       cp_async_commit2();
       {
@@ -180,9 +176,8 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
         if (st && ok_) {                                                                            \
           _Pragma("unroll") for (int f = 0; f < 5; ++f) stg2_(p.out + f * N + opm2 + o_, Uo[f]);    \
         }                                                                                           \
-        _Pragma("unroll") for (int f = 0; f < 5; ++f) acc_[f] = fma2(cz, Fz[f], lds2_(Bst + f * FS + st_)); \
+        _Pragma("unroll") for (int f = 0; f < 5; ++f) acc_[f] = fma2(cz, Fz[f], lds2_(Bst + bq * G::STAGE + f * FS + st_)); \
       }
-      cp_async_wait2<1>();                         // the base-state group; the next-plane group may still fly
       DH_ZPHASE(NA, WA, dA, LzA, accA, okA, oA, stA)
       DH_ZPHASE(NB, WB, dB, LzB, accB, okB, oB, stB)
 #undef DH_ZPHASE
@@ -381,10 +376,21 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
     configured = true;
   }
   const int bx = (p.nx + TX2 - 1) / TX2, by = (p.ny + G::TY - 1) / G::TY;
-  // z chunk: long enough that the 4 lead-in planes are cheap, short enough that the grid fills the GPU
-  int ZL = 64;
-  while (ZL > 8 && (long long)bx * by * ((p.nz + ZL - 1) / ZL) < 4LL * sm_count) ZL >>= 1;
-  const int bz = (p.nz + ZL - 1) / ZL;
+  // z chunks: every chunk pays 4 lead-in planes, and blocks run in waves of (blocks per SM) x sm_count;
+  // pick the chunk count that minimises waves x (planes per chunk + 4)
+  int dev = 0, per_sm = 1;
+  cudaGetDevice(&dev);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, NRW>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+  const long long slots = (long long)per_sm * sm_count, tiles = (long long)bx * by;
+  int bz = 1;
+  long long best = -1;
+  for (int cand = 1; cand <= p.nz / 4 && cand <= 65535; ++cand) {
+    const int zl_c = (p.nz + cand - 1) / cand;
+    if ((p.nz + zl_c - 1) / zl_c != cand) continue;
+    const long long cost = ((tiles * cand + slots - 1) / slots) * (zl_c + 4);
+    if (best < 0 || cost < best) { best = cost; bz = cand; }
+  }
+  const int ZL = (p.nz + bz - 1) / bz;
   dim3 grid(bx, by, bz), block((NRW + 1) * 32);
   stage_fused2_kernel<T, LIM, NRW><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
@@ -395,12 +401,15 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
 template <class T>
 cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported) {
   // packs are two cells adjacent in x: nx must be even; grid.y/z <= 65535
-  *supported = (p.nx % 2 == 0) && ((p.ny + 7) / 8 <= 65535);
+  *supported = (p.nx % 2 == 0) && ((p.ny + 5) / 6 <= 65535);
   if (!*supported) return cudaSuccess;
+  // fp32: 7 row warps + helper, one block per SM with the full register file (the kernel is bound by issue and
+  // register pressure, not occupancy: profiles/r01c); fp64 (parity only): 3 row warps so that shared memory fits
+  constexpr int NRW = sizeof(T) == 4 ? 7 : 3;
   switch (limiter) {
-    case 1: return launch_one2<T, 1, 4>(p, sm_count, s);
-    case 2: return launch_one2<T, 2, 4>(p, sm_count, s);
-    default: return launch_one2<T, 0, 4>(p, sm_count, s);
+    case 1: return launch_one2<T, 1, NRW>(p, sm_count, s);
+    case 2: return launch_one2<T, 2, NRW>(p, sm_count, s);
+    default: return launch_one2<T, 0, NRW>(p, sm_count, s);
   }
 }
 
