@@ -141,7 +141,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->acc, c->dt_dev, c->result_dev};
+  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->acc, c->dt_dev, c->result_dev};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
@@ -313,6 +313,56 @@ static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const v
   return DH_OK;
 }
 
+// Fused reversed stage (dh_rev.cu): per z slab, the face-adjoint sweep over the slab plus one plane on each side,
+// then the gather over the slab.  The scratch (20 words per cell of a slab) is allocated on first use.
+template <class T>
+static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+  const size_t NP = (size_t)c->nx * c->ny;
+  if (!c->rev_scratch) {
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)8 << 30; }
+    size_t budget = (size_t)12 << 30;
+    if (budget > free_b / 2) budget = free_b / 2;
+    const size_t per_plane = 20 * NP * elem_size(c);
+    long long planes = (long long)(budget / per_plane) - 2;
+    if (planes > c->nz) planes = c->nz;
+    if (planes < 1) return fail(DH_ERR_ALLOC, "dh_step_vjp: not enough device memory for the reverse-stage scratch%s");
+    int rc = lazy_alloc(c, &c->rev_scratch, (size_t)(planes + 2) * per_plane, "the reverse-stage scratch");
+    if (rc) return rc;
+    c->rev_slab = (int)planes;
+  }
+  const int SP = c->rev_slab + 2;
+  const int n[3] = {c->nx, c->ny, c->nz};
+  RevFaceParams<T> a;
+  a.U = (const T*)U; a.g = (const T*)g;
+  a.Wp = (T*)c->rev_scratch;
+  a.C = a.Wp + (size_t)5 * SP * NP;
+  a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
+  a.sp0 = 0; a.SP = SP;
+  for (int k = 0; k < 3; ++k) a.coef[k] = (T)(frac * dt * n[k] / c->L[k]);
+  a.c = make_consts<T>(c);
+  RevGatherParams<T> b;
+  b.U = (const T*)U; b.Wp = a.Wp; b.C = a.C; b.b1 = (const T*)b1; b.b2 = (const T*)b2; b.out = (T*)out;
+  b.nx = c->nx; b.ny = c->ny; b.nz = c->nz; b.sp0 = 1; b.SP = SP; b.c = a.c;
+  ProfScope ps(c, kind);
+  for (int z0 = 0; z0 < c->nz; z0 += c->rev_slab) {
+    const int nplanes = (c->nz - z0 < c->rev_slab) ? c->nz - z0 : c->rev_slab;
+    a.zs = z0 - 1; a.nout = nplanes + 2;
+    DH_CUDA(launch_rev_faces<T>(a, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
+    b.z0 = z0; b.nplanes = nplanes;
+    DH_CUDA(launch_rev_gather<T>(b, c->stream), "dh_step_vjp: gather kernel launch");
+    c->launches += 2;
+  }
+  return DH_OK;
+}
+
+template <class T>
+static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+  // the fused pair handles minmod on even nx; everything else takes the one-thread-per-cell gather kernel
+  if (c->kernel == 0 && c->limiter == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
+  return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
+}
+
 template <class T>
 static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
   int rc = lazy_alloc(c, &c->gs, state_bytes(c), "the U* cotangent state");
@@ -336,10 +386,10 @@ static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void*
     g1 = c->g1;
   }
   // reverse corrector:  gs = -dt J_D(U*)^T g1
-  rc = rev_launch<T>(c, DH_K_REV2, c->Us, g1, nullptr, nullptr, c->gs, dt, 1.0);
+  rc = rev_stage<T>(c, DH_K_REV2, c->Us, g1, nullptr, nullptr, c->gs, dt, 1.0);
   if (rc) return rc;
   // reverse predictor:  g_in = g1 + gs - dt/2 J_D(U^n)^T gs
-  return rev_launch<T>(c, DH_K_REV1, U, c->gs, g1, c->gs, gin, dt, 0.5);
+  return rev_stage<T>(c, DH_K_REV1, U, c->gs, g1, c->gs, gin, dt, 0.5);
 }
 
 extern "C" {

@@ -38,6 +38,35 @@ struct RevParams {
   Consts<T> c;
 };
 
+// Parameters of the two launches of a fused reversed stage (dh_rev.cu).  Scratch: Wp [5][SP][ny][nx] and
+// C [3][5][SP][ny][nx]; scratch plane sp0 holds grid plane zs (faces) / z0 (gather).
+template <class T>
+struct RevFaceParams {
+  const T* U;        // primal state the stage was evaluated at
+  const T* g;        // cotangent of the stage output
+  T* Wp;
+  T* C;
+  int nx, ny, nz;
+  int zs, nout;      // first output plane (unwrapped: may be -1) and number of output planes
+  int sp0, SP;
+  T coef[3];         // frac * dt / dx_a
+  Consts<T> c;
+};
+
+template <class T>
+struct RevGatherParams {
+  const T* U;
+  const T* Wp;
+  const T* C;
+  const T* b1;       // optional additive terms (nullptr = none)
+  const T* b2;
+  T* out;
+  int nx, ny, nz;
+  int z0, nplanes;   // planes z0 .. z0 + nplanes - 1 (all inside [0, nz))
+  int sp0, SP;
+  Consts<T> c;
+};
+
 // result block of the CFL reduction (device + pinned host mirror); all slots 8 bytes wide
 struct CflResult {
   double smax[3];    // T values widened
@@ -72,6 +101,8 @@ struct Ctx {
   void* Uhost_dev;             // device state for the HOST entry points
   void* gA;                    // device cotangent buffers for dh_step_vjp_host
   void* gB;
+  void* rev_scratch;           // 20 words per cell of a z slab (+2 planes), fused reverse stages
+  int rev_slab;                // planes per slab the scratch was sized for
   unsigned long long* acc;     // device accumulators of the CFL reduction
   void* dt_dev;                // device dt (T)
   CflResult* result_dev;
@@ -95,6 +126,8 @@ template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int l
 template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s);
+template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s);
+template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s);

@@ -1,0 +1,490 @@
+// dh_rev.cu — fused reverse-mode stage (step a7 of SURVEY.md §8(a), dt constant per PAPER.md:876).
+//
+// One reversed stage  out = b1 + b2 - tau J_D(U)^T g  (D(U) = sum_a (F_{a,+1/2} - F_{a,-1/2}) / dx_a, Eq. A4) is the
+// transpose of: primitives -> minmod slopes -> face states -> HLLC flux -> flux difference.  Written per axis for
+// cell i (coef = tau / dx_a):
+//     lambda_{i+1/2} = coef (g_{i+1} - g_i)                                   face cotangent
+//     (Lb, Rb)_{i+1/2} = J_HLLC(L_i, R_{i+1})^T lambda_{i+1/2}                one HLLC adjoint per face
+//     T_i = Lb_{i+1/2} + Rb_{i-1/2},   S_i = (Lb_{i+1/2} - Rb_{i-1/2}) / 2    state and slope cotangents
+//     minmod(a_i, b_i) passes S_i to a_i (if |a| <= |b|) or to b_i, or to neither (a b <= 0):
+//     Wb_i = T_i + [b-branch: +S_i | a-branch: -S_i]  +  (a-branch S_{i-1})  -  (b-branch S_{i+1})
+//     Ub_i = (dW/dU)_i^T Wb_i
+// The last two terms of Wb_i come from the neighbours' slopes, i.e. they depend on faces i-3/2 .. i+3/2.  Doing
+// everything in one kernel would make every tile recompute two extra layers of face adjoints around itself; the
+// one-thread-per-cell gather kernel (dh_naive.cu) does exactly that and spends 12 HLLC adjoints per cell.  Here
+// the work is split in two launches that share a scratch slab:
+//   A  rev_faces_kernel   fused z-sweep (same block shape as the first fused forward kernel): every face adjoint
+//                         once; writes per cell  Wp = sum_a (T_i + own-branch term)  and, per axis, c_i = S_i
+//                         masked by (a b > 0), with the branch flag stored in the mantissa LSB (<= 1 ulp);
+//   B  rev_gather_kernel  streaming: Wb_i = Wp_i + sum_a [a-branch c_{i-1}] - [b-branch c_{i+1}], then
+//                         Ub = prim_vjp(U, Wb) + b1 + b2.
+// Scratch is 20 words per cell of a z slab (+1 plane on each side); the API layer walks the slabs.  minmod only
+// (the branch flag is one bit); other limiters take the gather kernels.  No atomics; deterministic.
+#include "dh_internal.cuh"
+#include "dh_pack.cuh"
+
+namespace dh {
+
+namespace {
+
+constexpr int RTX = 64;        // cells per tile row = 32 lanes x 2
+constexpr int RSW = RTX + 4;   // row pitch of the shared planes (halo 2 on both sides)
+constexpr int RXP = 34;        // pitch of the x exchange arrays (33 used)
+
+template <int NW> struct GeoR {
+  static constexpr int TY = NW - 1;
+  static constexpr int SR = TY + 4;                       // rows of a shared plane
+  static constexpr int PLANE = 5 * SR * RSW;              // one buffered plane (all 5 fields)
+  static constexpr int XARR = 5 * TY * RXP;
+  static constexpr int YARR = 5 * (TY + 1) * RTX;
+  static constexpr int STAGE = 5 * TY * RTX;              // cp.async staging of one raw plane of the tile
+  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + STAGE;
+  static constexpr int NHALO = 4 * (RSW / 2) + 2 * TY;    // halo packs per plane
+  static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
+};
+
+DH_DI int wrapr(int i, int n) {   // i mod n for any i
+  int r = i % n;
+  return r < 0 ? r + n : r;
+}
+
+template <class T> DH_DI P2<T> rlds2(const T* p) { return *reinterpret_cast<const P2<T>*>(p); }
+template <class T> DH_DI void rsts2(T* p, P2<T> v) { *reinterpret_cast<P2<T>*>(p) = v; }
+template <class T> DH_DI P2<T> rldg2(const T* p) { return *reinterpret_cast<const P2<T>*>(p); }
+template <class T> DH_DI void rstg2(T* p, P2<T> v) { *reinterpret_cast<P2<T>*>(p) = v; }
+
+template <class T> DH_DI void rcp_async_pack(T* smem_dst, const T* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+DH_DI void rcp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+DH_DI void rcp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// branch flag in the mantissa LSB of the masked slope cotangent
+DH_DI float enc_flag(float v, bool pa) { return __uint_as_float((__float_as_uint(v) & ~1u) | (pa ? 1u : 0u)); }
+DH_DI double enc_flag(double v, bool pa) {
+  return __longlong_as_double((__double_as_longlong(v) & ~1ll) | (pa ? 1ll : 0ll));
+}
+DH_DI bool dec_flag(float v) { return (__float_as_uint(v) & 1u) != 0u; }
+DH_DI bool dec_flag(double v) { return (__double_as_longlong(v) & 1ll) != 0ll; }
+
+// minmod branch of slope (a, b): bit 0 = slope active (a b > 0), bit 1 = a-branch (|a| <= |b|)   (reading A7)
+template <class T> DH_DI int mm_mask(T a, T b) { return ((a * b > T(0)) ? 1 : 0) | ((abs_(a) <= abs_(b)) ? 2 : 0); }
+
+// cell cotangents of one axis from the two face adjoints: returns T + own-branch term, and the encoded c
+template <class T> DH_DI void cell_terms(T Lb, T Rbn, int m, T& wp, T& cenc) {
+  const T S = T(0.5) * (Lb - Rbn);
+  const bool on = (m & 1) != 0, pa = (m & 2) != 0;
+  wp = (Lb + Rbn) + (on ? (pa ? -S : S) : T(0));
+  cenc = enc_flag(on ? S : T(0), pa);
+}
+
+// HLLC adjoint of two faces: the scalar routine of dh_math.cuh on each half of the packs
+template <class T, int AX>
+DH_DI void hllc_vjp2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, const P2<T> Fb[5], P2<T> Lb[5], P2<T> Rb[5]) {
+  T l[5], r[5], fb[5], lb[5], rb[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { l[f] = L[f].x; r[f] = R[f].x; fb[f] = Fb[f].x; lb[f] = T(0); rb[f] = T(0); }
+  hllc_vjp<T, AX>(l, r, c, fb, lb, rb);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { Lb[f].x = lb[f]; Rb[f].x = rb[f]; l[f] = L[f].y; r[f] = R[f].y; fb[f] = Fb[f].y; lb[f] = T(0); rb[f] = T(0); }
+  hllc_vjp<T, AX>(l, r, c, fb, lb, rb);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { Lb[f].y = lb[f]; Rb[f].y = rb[f]; }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ kernel A
+template <class T, int NW>
+__global__ void __launch_bounds__(NW * 32, 1)
+rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
+  using G = GeoR<NW>;
+  constexpr int TY = G::TY, SR = G::SR, FP = SR * RSW, FS = TY * RTX;
+  constexpr int XF = TY * RXP, YF = (TY + 1) * RTX;       // field pitches of the exchange arrays
+  extern __shared__ __align__(16) unsigned char smem_rev[];
+  T* const Wsm = reinterpret_cast<T*>(smem_rev);   // [2][5][SR][RSW]  primitive planes p (it&1) and p-1
+  T* const Gsm = Wsm + 2 * G::PLANE;               // [2][5][SR][RSW]  cotangent planes p and p-1 (halo 1 used)
+  T* const Rxs = Gsm + 2 * G::PLANE;               // [5][TY][RXP]     R state of the first cell of lane l (l = 32: halo column)
+  T* const Bxs = Rxs + G::XARR;                    // [5][TY][RXP]     Rb of the face LEFT of lane l's pack (slot 0: helper)
+  T* const Rys = Bxs + G::XARR;                    // [5][TY+1][RTX]   R states of row r (r = TY: halo row)
+  T* const Bys = Rys + G::YARR;                    // [5][TY+1][RTX]   Rb of the face BELOW row r (slot 0: helper)
+  T* const Ust = Bys + G::YARR;                    // [5][TY][RTX]     raw U of the next plane (cp.async, private slots)
+
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int nx = p.nx, ny = p.ny, nz = p.nz;
+  const size_t NP = (size_t)nx * ny, N = NP * nz, SPN = (size_t)p.SP * NP;
+  const int x0 = blockIdx.x * RTX, y0 = blockIdx.y * TY;
+  const int zrel0 = blockIdx.z * ZL;               // first output plane of this block, relative to p.zs
+  const int zl = min(ZL, p.nout - zrel0);
+  const int nit = zl + 4;                          // planes z0-2 .. z0+zl+1
+  const P2<T> cx = bc2(p.coef[0]), cy = bc2(p.coef[1]), cz = bc2(p.coef[2]);
+  const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
+  const Consts<T>& c = p.c;
+  int pz = wrapr(p.zs + zrel0 - 2, nz);
+
+  if (w < TY) {
+    // ------------------------------------------------------------------------------------ row warp
+    const int r = w;
+    const size_t o = (size_t)wrapr(y0 + r, ny) * nx + wrapr(x0 + 2 * lane, nx);
+    const bool store_ok = (x0 + 2 * lane < nx) && (y0 + r < ny);
+    const int so = (r + 2) * RSW + 2 * lane + 2;   // own pack inside a shared plane
+    const int xo = r * RXP + lane, yo = r * RTX + 2 * lane;
+    T* const ust = Ust + yo;
+    P2<T> Wprev[5], dprev[5], Lz[5], gpp[5], RbzC[5], WxyC[5];
+    int mzC = 0;                                   // minmod branches (z) of the cell of plane p-2, 4 bits per field
+#pragma unroll
+    for (int f = 0; f < 5; ++f) Wprev[f] = dprev[f] = Lz[f] = gpp[f] = RbzC[f] = WxyC[f] = bc2(T(0));
+    size_t op = (size_t)pz * NP + o;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) rcp_async_pack(ust + f * FS, p.U + f * N + op);
+    rcp_async_commit();
+    rcp_async_wait_all();
+    // scratch offset of the plane finished in iteration `it` (plane p-2): advanced by NP per iteration
+    long long os2 = ((long long)p.sp0 + zrel0 - 4) * (long long)NP + (long long)o;
+
+#pragma unroll 1
+    for (int it = 0; it < nit; ++it) {
+      const int bp = it & 1, bq = bp ^ 1;
+      T* const Wp_s = Wsm + bp * G::PLANE;
+      const T* const Wq_s = Wsm + bq * G::PLANE;
+      const T* const Gq_s = Gsm + bq * G::PLANE;
+      const bool xy = (it >= 3) && (it <= zl + 2);   // x/y work on plane p-1 is wanted
+      P2<T> Uc[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) Uc[f] = rlds2(ust + f * FS);
+      // cotangent of plane p straight into its shared plane (read by the neighbours in the next iteration), and the
+      // raw state of plane p+1 into the staging slots; both are waited for at the end of the iteration
+      int pzn = pz + 1;
+      size_t opn = op + NP;
+      if (pzn == nz) { pzn = 0; opn = o; }
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        rcp_async_pack(Gsm + bp * G::PLANE + f * FP + so, p.g + f * N + op);
+        rcp_async_pack(ust + f * FS, p.U + f * N + opn);
+      }
+      rcp_async_commit();
+      P2<T> Wn[5];
+      prim2(Uc, c, Wn);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) rsts2(Wp_s + f * FP + so, Wn[f]);
+      P2<T> gq[5];                                  // own cotangent of plane p-1
+#pragma unroll
+      for (int f = 0; f < 5; ++f) gq[f] = rlds2(Gq_s + f * FP + so);
+
+      // ---- z: slope of plane p-1, adjoint of the face between p-2 and p-1, which completes the cell of plane p-2
+      {
+        P2<T> Rz[5], lam[5], Lb[5], Rb[5];
+        int mz = 0;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          const P2<T> a = sub2(Wn[f], Wprev[f]);
+          const P2<T> s = limit2<T, 0>(a, dprev[f]);
+          mz |= (mm_mask(a.x, dprev[f].x) | (mm_mask(a.y, dprev[f].y) << 2)) << (4 * f);
+          Rz[f] = fma2(nhalf, s, Wprev[f]);
+          Wn[f] = fma2(half, s, Wprev[f]);           // left state of the NEXT z face
+          dprev[f] = a;
+          lam[f] = mul2(cz, sub2(gq[f], gpp[f]));
+          gpp[f] = gq[f];
+        }
+        hllc_vjp2<T, 2>(Lz, Rz, c, lam, Lb, Rb);
+        const bool stz = (it >= 4) && store_ok;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          Lz[f] = Wn[f];
+          const int m = mzC >> (4 * f);
+          P2<T> wp, ce;
+          cell_terms(Lb[f].x, RbzC[f].x, m, wp.x, ce.x);
+          cell_terms(Lb[f].y, RbzC[f].y, m >> 2, wp.y, ce.y);
+          RbzC[f] = Rb[f];
+          if (stz) {
+            rstg2(p.Wp + f * SPN + os2, add2(wp, WxyC[f]));
+            rstg2(p.C + (10 + f) * SPN + os2, ce);
+          }
+        }
+        mzC = mz;
+      }
+
+      // ---- x / y on plane p-1, phase 1: slopes of the own cells, publish the R states
+      P2<T> Lx[5], Rxo[5], Ly[5];
+      int mx = 0, my = 0;
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const T* row = Wq_s + f * FP + so;
+        const P2<T> W = Wprev[f];
+        {
+          const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = row[2] - W.y;
+          const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
+          mx |= (mm_mask(d1, d0) | (mm_mask(d2, d1) << 2)) << (4 * f);
+          Lx[f] = fma2(half, s, W);
+          Rxo[f] = fma2(nhalf, s, W);
+          Rxs[f * XF + xo] = Rxo[f].x;
+        }
+        {
+          const P2<T> a = sub2(rlds2(row + RSW), W), b = sub2(W, rlds2(row - RSW));
+          const P2<T> s = limit2<T, 0>(a, b);
+          my |= (mm_mask(a.x, b.x) | (mm_mask(a.y, b.y) << 2)) << (4 * f);
+          Ly[f] = fma2(half, s, W);
+          rsts2(Rys + f * YF + yo, fma2(nhalf, s, W));
+        }
+      }
+      __syncthreads();
+      // ---- phase 2: adjoints of the own right (x) and top (y) faces, publish the R-side cotangents
+      P2<T> Lbx[5], Lby[5];
+      T RbxA[5];                                    // Rb of the face between the two own cells (belongs to the second cell)
+      {
+        P2<T> Rf[5], lam[5], Rb[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          Rf[f] = {Rxo[f].y, Rxs[f * XF + xo + 1]};
+          const T gr = Gq_s[f * FP + so + 2];
+          lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
+        }
+        hllc_vjp2<T, 0>(Lx, Rf, c, lam, Lbx, Rb);
+#pragma unroll
+        for (int f = 0; f < 5; ++f) { RbxA[f] = Rb[f].x; Bxs[f * XF + xo + 1] = Rb[f].y; }
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          Rf[f] = rlds2(Rys + f * YF + yo + RTX);
+          lam[f] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
+        }
+        hllc_vjp2<T, 1>(Ly, Rf, c, lam, Lby, Rb);
+#pragma unroll
+        for (int f = 0; f < 5; ++f) rsts2(Bys + f * YF + yo + RTX, Rb[f]);
+      }
+      rcp_async_wait_all();                         // cotangent plane p and the next raw plane have landed
+      __syncthreads();
+      // ---- phase 3: cell cotangents of plane p-1 for x and y (the z part joins them in the next iteration)
+      {
+        const bool stxy = xy && store_ok;
+        const long long os1 = os2 + (long long)NP;
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          P2<T> wx, cex, wy, cey;
+          cell_terms(Lbx[f].x, Bxs[f * XF + xo], mx >> (4 * f), wx.x, cex.x);
+          cell_terms(Lbx[f].y, RbxA[f], mx >> (4 * f + 2), wx.y, cex.y);
+          const P2<T> Rbn = rlds2(Bys + f * YF + yo);
+          cell_terms(Lby[f].x, Rbn.x, my >> (4 * f), wy.x, cey.x);
+          cell_terms(Lby[f].y, Rbn.y, my >> (4 * f + 2), wy.y, cey.y);
+          WxyC[f] = add2(wx, wy);
+          if (stxy) {
+            rstg2(p.C + f * SPN + os1, cex);
+            rstg2(p.C + (5 + f) * SPN + os1, cey);
+          }
+        }
+      }
+      // plane p becomes plane p-1
+#pragma unroll
+      for (int f = 0; f < 5; ++f) Wprev[f] = rlds2(Wp_s + f * FP + so);
+      os2 += (long long)NP;
+      op = opn;
+      pz = pzn;
+    }
+  } else {
+    // -------------------------------------------------------------------------------------- helper
+    constexpr int HP = G::HP, HC = RSW / 2;
+    int hg[HP], hs[HP];
+#pragma unroll
+    for (int k = 0; k < HP; ++k) {
+      const int idx = lane + 32 * k;
+      int row, cp;
+      if (idx < 4 * HC) {
+        const int hr = idx / HC;
+        cp = idx - hr * HC;
+        row = hr < 2 ? hr - 2 : TY + hr - 2;
+      } else {
+        const int kk = idx - 4 * HC;
+        row = kk >> 1;
+        cp = (kk & 1) ? HC - 1 : 0;
+      }
+      hg[k] = (idx < G::NHALO) ? wrapr(y0 + row, ny) * nx + wrapr(x0 - 2 + 2 * cp, nx) : -1;
+      hs[k] = (row + 2) * RSW + 2 * cp;
+    }
+    const int rl = lane < TY ? lane : TY - 1;      // row of the x pass (lanes >= TY repeat the last row, unused)
+
+#pragma unroll 1
+    for (int it = 0; it < nit; ++it) {
+      const int bp = it & 1, bq = bp ^ 1;
+      const T* const Wq_s = Wsm + bq * G::PLANE;
+      const T* const Gq_s = Gsm + bq * G::PLANE;
+      const size_t op = (size_t)pz * NP;
+      // halo of plane p: raw state to registers (converted below), cotangent straight into its shared plane
+      P2<T> Uh[HP][5];
+#pragma unroll
+      for (int k = 0; k < HP; ++k) {
+        if (hg[k] >= 0) {
+#pragma unroll
+          for (int f = 0; f < 5; ++f) {
+            Uh[k][f] = rldg2(p.U + f * N + op + hg[k]);
+            rcp_async_pack(Gsm + bp * G::PLANE + f * FP + hs[k], p.g + f * N + op + hg[k]);
+          }
+        }
+      }
+      rcp_async_commit();
+      P2<T> LyB[5];
+      T LxB[5];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const T* pl = Wq_s + f * FP;
+        // y: R state of the halo row TY, L state of the halo row -1
+        const T* col = pl + 2 * lane + 2;
+        {
+          const P2<T> Wm = rlds2(col + (TY + 1) * RSW), W = rlds2(col + (TY + 2) * RSW), Wu = rlds2(col + (TY + 3) * RSW);
+          const P2<T> s = limit2<T, 0>(sub2(Wu, W), sub2(W, Wm));
+          rsts2(Rys + f * YF + TY * RTX + 2 * lane, fma2(nhalf, s, W));
+        }
+        {
+          const P2<T> Wm = rlds2(col), W = rlds2(col + RSW), Wu = rlds2(col + 2 * RSW);
+          const P2<T> s = limit2<T, 0>(sub2(Wu, W), sub2(W, Wm));
+          LyB[f] = fma2(half, s, W);
+        }
+        // x: L state of the halo column -1, R state of the halo column RTX, row rl
+        const T* rw = pl + (rl + 2) * RSW;
+        const T sl = minmod_(rw[2] - rw[1], rw[1] - rw[0]);
+        LxB[f] = fma_(T(0.5), sl, rw[1]);
+        const T sr = minmod_(rw[RTX + 3] - rw[RTX + 2], rw[RTX + 2] - rw[RTX + 1]);
+        if (lane < TY) Rxs[f * XF + rl * RXP + 32] = fma_(T(-0.5), sr, rw[RTX + 2]);
+      }
+      __syncthreads();
+      {
+        P2<T> Lf[5], Rf[5], lam[5], Lb[5], Rb[5];
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          Rf[f] = rlds2(Rys + f * YF + 2 * lane);
+          const T* gc = Gq_s + f * FP + 2 * lane + 2;
+          lam[f] = mul2(cy, sub2(rlds2(gc + 2 * RSW), rlds2(gc + RSW)));
+        }
+        hllc_vjp2<T, 1>(LyB, Rf, c, lam, Lb, Rb);  // bottom y face of the tile
+#pragma unroll
+        for (int f = 0; f < 5; ++f) rsts2(Bys + f * YF + 2 * lane, Rb[f]);
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          Lf[f] = bc2(LxB[f]);
+          Rf[f] = bc2(Rxs[f * XF + rl * RXP]);
+          const T* gr = Gq_s + f * FP + (rl + 2) * RSW;
+          lam[f] = bc2(p.coef[0] * (gr[2] - gr[1]));
+        }
+        hllc_vjp2<T, 0>(Lf, Rf, c, lam, Lb, Rb);   // left x face of the tile, row rl
+        if (lane < TY) {
+#pragma unroll
+          for (int f = 0; f < 5; ++f) Bxs[f * XF + rl * RXP] = Rb[f].x;
+        }
+      }
+      // halo primitives of plane p -> shared
+      {
+        T* Wb = Wsm + bp * G::PLANE;
+#pragma unroll
+        for (int k = 0; k < HP; ++k) {
+          if (hg[k] >= 0) {
+            P2<T> Wh[5];
+            prim2(Uh[k], c, Wh);
+#pragma unroll
+            for (int f = 0; f < 5; ++f) rsts2(Wb + f * FP + hs[k], Wh[f]);
+          }
+        }
+      }
+      rcp_async_wait_all();
+      __syncthreads();
+      ++pz;
+      if (pz == nz) pz = 0;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ kernel B
+// One thread per pack (two x-adjacent cells) of a slab plane.
+template <class T>
+__global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T> p) {
+  const int ip = blockIdx.x * blockDim.x + threadIdx.x;       // pack index along x
+  const int i = 2 * ip, j = blockIdx.y, kz = blockIdx.z;      // kz: plane relative to p.z0
+  if (i >= p.nx) return;
+  const int nx = p.nx, ny = p.ny;
+  const size_t NP = (size_t)nx * ny, N = NP * p.nz, SPN = (size_t)p.SP * NP;
+  const size_t row = (size_t)j * nx, rowm = (size_t)(j == 0 ? ny - 1 : j - 1) * nx, rowp = (size_t)(j == ny - 1 ? 0 : j + 1) * nx;
+  const size_t sp = (size_t)(p.sp0 + kz) * NP;                // scratch plane of this cell; its z neighbours are sp -+ NP
+  const size_t cell = (size_t)(p.z0 + kz) * NP + row + i;     // p.z0 + kz < nz by construction
+  const int im = (i == 0 ? nx - 1 : i - 1), ipl = (i + 2 >= nx ? 0 : i + 2);
+  P2<T> Wb[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    P2<T> w = rldg2(p.Wp + f * SPN + sp + row + i);
+    // x: a-branch of the cell to the left, b-branch of the cell to the right
+    const T* Cx = p.C + f * SPN + sp + row;
+    const P2<T> cxo = rldg2(Cx + i);
+    const T cl = Cx[im], cr = Cx[ipl];
+    w.x += (dec_flag(cl) ? cl : T(0)) - (dec_flag(cxo.y) ? T(0) : cxo.y);
+    w.y += (dec_flag(cxo.x) ? cxo.x : T(0)) - (dec_flag(cr) ? T(0) : cr);
+    // y
+    const T* Cy = p.C + (5 + f) * SPN + sp + i;
+    const P2<T> cd = rldg2(Cy + rowm), cu = rldg2(Cy + rowp);
+    w.x += (dec_flag(cd.x) ? cd.x : T(0)) - (dec_flag(cu.x) ? T(0) : cu.x);
+    w.y += (dec_flag(cd.y) ? cd.y : T(0)) - (dec_flag(cu.y) ? T(0) : cu.y);
+    // z
+    const T* Cz = p.C + (10 + f) * SPN + sp + row + i;
+    const P2<T> cb = rldg2(Cz - NP), ct = rldg2(Cz + NP);
+    w.x += (dec_flag(cb.x) ? cb.x : T(0)) - (dec_flag(ct.x) ? T(0) : ct.x);
+    w.y += (dec_flag(cb.y) ? cb.y : T(0)) - (dec_flag(ct.y) ? T(0) : ct.y);
+    Wb[f] = w;
+  }
+  P2<T> U[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) U[f] = rldg2(p.U + f * N + cell);
+  T u[5], wb[5], ubx[5], uby[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { u[f] = U[f].x; wb[f] = Wb[f].x; }
+  prim_vjp(u, p.c, wb, ubx);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { u[f] = U[f].y; wb[f] = Wb[f].y; }
+  prim_vjp(u, p.c, wb, uby);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) {
+    P2<T> v = {ubx[f], uby[f]};
+    if (p.b1) v = add2(v, rldg2(p.b1 + f * N + cell));
+    if (p.b2) v = add2(v, rldg2(p.b2 + f * N + cell));
+    rstg2(p.out + f * N + cell, v);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ launchers
+template <class T>
+cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
+  constexpr int NW = 8;
+  using G = GeoR<NW>;
+  const size_t smem = (size_t)G::TOTAL * sizeof(T);
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int bx = (p.nx + RTX - 1) / RTX, by = (p.ny + G::TY - 1) / G::TY;
+  // z chunks: waves of sm_count blocks (one block per SM), 4 lead-in planes per chunk
+  const long long tiles = (long long)bx * by;
+  int bz = 1;
+  long long best = -1;
+  for (int cand = 1; cand <= (p.nout + 3) / 4 && cand <= 65535; ++cand) {
+    const int zl_c = (p.nout + cand - 1) / cand;
+    if ((p.nout + zl_c - 1) / zl_c != cand) continue;
+    const long long cost = ((tiles * cand + sm_count - 1) / sm_count) * (zl_c + 4);
+    if (best < 0 || cost < best) { best = cost; bz = cand; }
+  }
+  const int ZL = (p.nout + bz - 1) / bz;
+  dim3 grid(bx, by, bz), block(NW * 32);
+  rev_faces_kernel<T, NW><<<grid, block, smem, s>>>(p, ZL);
+  return cudaGetLastError();
+}
+
+template <class T>
+cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s) {
+  dim3 block(128), grid((p.nx / 2 + 127) / 128, p.ny, p.nplanes);
+  rev_gather_kernel<T><<<grid, block, 0, s>>>(p);
+  return cudaGetLastError();
+}
+
+template cudaError_t launch_rev_faces<float>(const RevFaceParams<float>&, int, cudaStream_t);
+template cudaError_t launch_rev_faces<double>(const RevFaceParams<double>&, int, cudaStream_t);
+template cudaError_t launch_rev_gather<float>(const RevGatherParams<float>&, cudaStream_t);
+template cudaError_t launch_rev_gather<double>(const RevGatherParams<double>&, cudaStream_t);
+
+}  // namespace dh
