@@ -171,6 +171,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_RHO_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->rho_floor = v; break;
     case DH_OPT_P_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->p_floor = v; break;
     case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0, 1 or 2%s"); c->kernel = (int)v; break;
+    case DH_OPT_REV_SLAB: if (v < 0 || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: rev_slab must be a non-negative integer%s"); c->rev_slab_opt = (int)v; break;
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
@@ -190,6 +191,7 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_P_FLOOR: *out = c->p_floor; break;
     case DH_OPT_KERNEL: *out = c->kernel; break;
     case DH_OPT_LIMITER: *out = c->limiter; break;
+    case DH_OPT_REV_SLAB: *out = c->rev_slab_opt; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
   return DH_OK;
@@ -318,14 +320,23 @@ static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const v
 template <class T>
 static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
   const size_t NP = (size_t)c->nx * c->ny;
+  const int want = c->rev_slab_opt > 0 ? (c->rev_slab_opt < c->nz ? c->rev_slab_opt : c->nz) : 0;
+  if (c->rev_scratch && want > 0 && want != c->rev_slab) {      // the option changed: resize
+    DH_CUDA(cudaStreamSynchronize(c->stream), "dh_step_vjp: synchronize");
+    cudaFree(c->rev_scratch);
+    c->rev_scratch = nullptr;
+  }
   if (!c->rev_scratch) {
-    size_t free_b = 0, total_b = 0;
-    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)8 << 30; }
-    size_t budget = (size_t)12 << 30;
-    if (budget > free_b / 2) budget = free_b / 2;
     const size_t per_plane = 20 * NP * elem_size(c);
-    long long planes = (long long)(budget / per_plane) - 2;
-    if (planes > c->nz) planes = c->nz;
+    long long planes = want;
+    if (planes == 0) {
+      size_t free_b = 0, total_b = 0;
+      if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)8 << 30; }
+      size_t budget = (size_t)12 << 30;
+      if (budget > free_b / 2) budget = free_b / 2;
+      planes = (long long)(budget / per_plane) - 2;
+      if (planes > c->nz) planes = c->nz;
+    }
     if (planes < 1) return fail(DH_ERR_ALLOC, "dh_step_vjp: not enough device memory for the reverse-stage scratch%s");
     int rc = lazy_alloc(c, &c->rev_scratch, (size_t)(planes + 2) * per_plane, "the reverse-stage scratch");
     if (rc) return rc;

@@ -103,6 +103,7 @@ struct Ctx {
   void* gB;
   void* rev_scratch;           // 20 words per cell of a z slab (+2 planes), fused reverse stages
   int rev_slab;                // planes per slab the scratch was sized for
+  int rev_slab_opt;            // DH_OPT_REV_SLAB (0 = automatic)
   unsigned long long* acc;     // device accumulators of the CFL reduction
   void* dt_dev;                // device dt (T)
   CflResult* result_dev;

@@ -19,7 +19,7 @@ DH_F32, DH_F64 = 0, 1
 DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, -4
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
-    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11,
+    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
