@@ -179,6 +179,13 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
         _Pragma("unroll") for (int f = 0; f < 5; ++f) acc_[f] = fma2(cz, Fz[f], lds2_(Bst + bq * G::STAGE + f * FS + st_)); \
       }
       DH_ZPHASE(NA, WA, dA, LzA, accA, okA, oA, stA)
+      // x neighbours of plane p-1, loaded here so that their latency hides behind the second z phase
+      T xl[5][2], xr[5][2];
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        const T* rowA = Wq_s + f * FP + soA;
+        xl[f][0] = rowA[-1]; xr[f][0] = rowA[2]; xl[f][1] = rowA[SW2 - 1]; xr[f][1] = rowA[SW2 + 2];
+      }
       DH_ZPHASE(NB, WB, dB, LzB, accB, okB, oB, stB)
 #undef DH_ZPHASE
 
@@ -189,9 +196,8 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
         P2<T> LxA[5], RxA[5], LxB[5], RxB[5];
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          const T* rowA = Wq_s + f * FP + soA;
-          recon_x2<T, LIM>(WA[f], rowA[-1], rowA[2], LxA[f], RxA[f]);
-          recon_x2<T, LIM>(WB[f], rowA[SW2 - 1], rowA[SW2 + 2], LxB[f], RxB[f]);
+          recon_x2<T, LIM>(WA[f], xl[f][0], xr[f][0], LxA[f], RxA[f]);
+          recon_x2<T, LIM>(WB[f], xl[f][1], xr[f][1], LxB[f], RxB[f]);
           Rx_s[f * XEP + xeA] = RxA[f].x;
           Rx_s[f * XEP + xeB] = RxB[f].x;
         }
