@@ -51,6 +51,7 @@ def parse_args():
     ap.add_argument("--cooling", type=int, default=0, help="1: configs[3]'s cooling source in the corrector epilogue")
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
+    ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -228,26 +229,34 @@ def run_dh(a):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def fwd_step():
-        s.cfl_dt_async(U)
-        s.step_devdt(U)
+    def fwd_step(k=1):
+        # k x (CFL dt + RK2 step), dt never leaves the device
+        if a.no_chain:
+            for _ in range(k):
+                s.cfl_dt_async(U)
+                s.step_devdt(U)
+        else:
+            s.advance(U, k, sync=False)
 
     # a state that fits in the 126 MB L2 (n <= 128) is evicted between iterations by writing a 512 MB buffer;
     # the flush is outside the per-iteration event pairs
     fits_l2 = 5 * 4 * N <= 4 * 126e6
     flush = torch.empty(128 * 1024 * 1024, device=dev, dtype=torch.float32) if fits_l2 else None
 
-    def timed(fn, iters):
-        """K calls bracketed by barrier + synchronize on both sides, CUDA events on the launching stream; the
-        max over ranks is taken by the caller."""
+    def timed(fn, iters, batched=False):
+        """K steps bracketed by barrier + synchronize on both sides, CUDA events on the launching stream; the
+        max over ranks is taken by the caller.  batched: fn(K) issues all K steps in one library call."""
         barrier()
         l0 = s.launch_count
         t0 = time.time()
         if flush is None:
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            for _ in range(iters):
-                fn()
+            if batched:
+                fn(iters)
+            else:
+                for _ in range(iters):
+                    fn()
             e1.record()
             barrier()
             ms = e0.elapsed_time(e1)
@@ -273,12 +282,11 @@ def run_dh(a):
         return float(t.item())
 
     # ---- forward: warm-up, then the timed region with per-kernel events and the clock sampler running
-    for _ in range(W):
-        fwd_step()
+    fwd_step(W) if flush is None else [fwd_step() for _ in range(W)]
     dt_w = s.poll()                                        # raises on a non-finite state
     s.profile(True)
     sampler = ClockSampler(local) if rank == 0 else None
-    ms_fwd, launches, t0, t1 = timed(fwd_step, K)
+    ms_fwd, launches, t0, t1 = timed(fwd_step, K, batched=True)
     clocks = sampler.stop(t0, t1) if sampler else None
     prof = s.profile_read()
     dt_last = s.poll()
@@ -306,7 +314,8 @@ def run_dh(a):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
                        "cfl": 0.4, "limiter": "minmod", "riemann": "hllc", "integrator": "rk2 predictor/corrector",
-                       "cooling": bool(a.cooling), "kernel": a.kernel, "parallelism": f"replicas x{world}",
+                       "cooling": bool(a.cooling), "kernel": a.kernel,
+                       "call": "dh_cfl_dt_async + dh_step_devdt per step" if a.no_chain else "dh_advance(U, K): K x (CFL reduce, dt epilogue, predictor, corrector)", "parallelism": f"replicas x{world}",
                        "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
                        if fits_l2 else f"inputs larger than L2 ({5 * 4 * N / 1e6:.0f} MB per state vs 126 MB), no flush",
                        "dt_last": dt_last},

@@ -109,6 +109,14 @@ int dh_cfl_dt_async(dh_ctx* ctx, const void* U);
 /* Synchronise the stream and report (dt of the last CFL, non-finite flag -> DH_ERR_NONFINITE). */
 int dh_poll_status(dh_ctx* ctx, double* dt_out);
 
+/* nsteps x (Eq. A8 time step + RK2 step) in place, everything on the device: per step the CFL reduction, its
+ * one-thread dt epilogue, the predictor and the corrector; dt never visits the host.  (Reducing the wave speeds of
+ * U^{n+1} inside the corrector instead was built and measured: the estimate-then-exact candidate test costs the
+ * corrector more than the 20 B/cell pass it saves.)
+ * U: DEVICE.  dt_last_out: HOST or NULL; if non-NULL the call synchronises and reports the last dt / a non-finite
+ * state like dh_poll_status, otherwise it is asynchronous and dh_poll_status may be called later. */
+int dh_advance(dh_ctx* ctx, void* U, int nsteps, double* dt_last_out);
+
 /* Vector-Jacobian product of the full step (dt held constant):
  *   gU_in = (dU^{n+1}/dU^n)^T gU_out   evaluated at U = U^n (the PRE-step state) and dt.
  * Nothing is stored by dh_step: U* is recomputed, then the two stages are reversed by gather-form kernels

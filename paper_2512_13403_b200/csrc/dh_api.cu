@@ -245,12 +245,13 @@ static int cfl_launch(dh_ctx* c, const void* U) {
   {
     ProfScope ps(c, DH_K_CFL_REDUCE);
     DH_CUDA(launch_cfl_reduce<T>(p, c->sm_count, c->stream), "dh_cfl_dt: reduction kernel launch");
+    c->launches += 1;
   }
   {
     ProfScope ps(c, DH_K_CFL_FINISH);
     DH_CUDA(launch_cfl_finish<T>(p, c->stream), "dh_cfl_dt: epilogue kernel launch");
   }
-  c->launches += 2;
+  c->launches += 1;
   return DH_OK;
 }
 
@@ -445,17 +446,27 @@ int dh_step_vjp(dh_ctx* c, const void* U, double dt, const void* gout, void* gin
   return c->dtype == DH_F32 ? vjp_impl<float>(c, U, dt, gout, gin) : vjp_impl<double>(c, U, dt, gout, gin);
 }
 
+int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
+  if (!c || !U || nsteps < 0) return fail(DH_ERR_ARG, "dh_advance: bad argument%s");
+  if (U == c->Us) return fail(DH_ERR_ARG, "dh_advance: U aliases library scratch%s");
+  const bool f32 = c->dtype == DH_F32;
+  for (int s = 0; s < nsteps; ++s) {
+    int rc = f32 ? cfl_launch<float>(c, U) : cfl_launch<double>(c, U);
+    if (rc) return rc;
+    rc = f32 ? step_impl<float>(c, U, 0.0, true) : step_impl<double>(c, U, 0.0, true);
+    if (rc) return rc;
+  }
+  if (dt_last_out) return dh_poll_status(c, dt_last_out);
+  return DH_OK;
+}
+
 int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {
   if (!c || !U_host || nsteps < 0) return fail(DH_ERR_ARG, "dh_run_host: bad argument%s");
   int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
   if (rc) return rc;
   DH_CUDA(cudaMemcpyAsync(c->Uhost_dev, U_host, state_bytes(c), cudaMemcpyHostToDevice, c->stream), "dh_run_host: H2D");
-  for (int s = 0; s < nsteps; ++s) {
-    rc = dh_cfl_dt_async(c, c->Uhost_dev);
-    if (rc) return rc;
-    rc = dh_step_devdt(c, c->Uhost_dev);
-    if (rc) return rc;
-  }
+  rc = dh_advance(c, c->Uhost_dev, nsteps, nullptr);
+  if (rc) return rc;
   DH_CUDA(cudaMemcpyAsync(U_host, c->Uhost_dev, state_bytes(c), cudaMemcpyDeviceToHost, c->stream), "dh_run_host: D2H");
   return dh_poll_status(c, dt_last_out);
 }

@@ -28,7 +28,7 @@ KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
-    "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
+    "dh_advance", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
 ]
 KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp"]
 
@@ -64,6 +64,7 @@ def load(rebuild: bool = False):
     lib.dh_step_devdt.argtypes = [vp, vp]
     lib.dh_step_vjp.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_run_host.argtypes = [vp, vp, ci, pd]
+    lib.dh_advance.argtypes = [vp, vp, ci, pd]
     lib.dh_step_vjp_host.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_launch_count.restype = ctypes.c_ulonglong
     lib.dh_launch_count.argtypes = [vp]
@@ -72,7 +73,7 @@ def load(rebuild: bool = False):
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
-               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host", "dh_profile_enable",
+               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_advance", "dh_step_vjp_host", "dh_profile_enable",
                "dh_profile_read"):
         getattr(lib, fn).restype = ci
     _lib = lib
@@ -148,6 +149,16 @@ def dh_step_devdt(ctx, U_ptr: int) -> None:
 
 def dh_step_vjp(ctx, U_ptr: int, dt: float, gout_ptr: int, gin_ptr: int) -> None:
     _check(load().dh_step_vjp(ctx, ctypes.c_void_p(U_ptr), float(dt), ctypes.c_void_p(gout_ptr), ctypes.c_void_p(gin_ptr)))
+
+
+def dh_advance(ctx, U_ptr: int, nsteps: int, sync: bool = True):
+    """nsteps x (CFL dt + RK2 step) on the device; returns the last dt if `sync`, else None (asynchronous)."""
+    if sync:
+        out = ctypes.c_double()
+        _check(load().dh_advance(ctx, ctypes.c_void_p(U_ptr), int(nsteps), ctypes.byref(out)))
+        return out.value
+    _check(load().dh_advance(ctx, ctypes.c_void_p(U_ptr), int(nsteps), None))
+    return None
 
 
 def dh_run_host(ctx, U_host_ptr: int, nsteps: int) -> float:
@@ -227,6 +238,9 @@ class Solver:
 
     def step(self, U, dt: float) -> None:
         dh_step(self.ctx, self._dev(U, "U"), dt)
+
+    def advance(self, U, nsteps: int, sync: bool = True):
+        return dh_advance(self.ctx, self._dev(U, "U"), nsteps, sync)
 
     def step_devdt(self, U) -> None:
         dh_step_devdt(self.ctx, self._dev(U, "U"))

@@ -372,6 +372,39 @@ def test_device_resident_dt_path_matches_host_dt_path():
 
 
 # ------------------------------------------------------------------------------------ error behaviour
+@pytest.mark.parametrize("cooling", [0, 1])
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+def test_advance_is_bitwise_the_host_driven_loop(dtype, cooling):
+    """dh_advance (device-resident dt for every step) equals the loop of dh_cfl_dt + dh_step bit for bit, and its
+    last dt equals the oracle's dt of the state before the last step."""
+    U = random_state((20, 30, 132), 91, 5 / 3, dtype, mach=1.5).cuda()
+    s = _solver(U, 5 / 3, cooling=cooling, lambda0=0.5)
+    a, b = U.clone(), U.clone()
+    dts = []
+    for _ in range(4):
+        before = a.clone()
+        dts.append(s.cfl_dt(a))
+        s.step(a, dts[-1])
+    dt_last = s.advance(b, 4)
+    assert dt_last == dts[-1]
+    assert torch.equal(a, b)
+    p = oracle_params(U.cpu(), 5 / 3, cooling=bool(cooling), lambda0=0.5)
+    dt_ora, _ = oracle.cfl_dt(before.cpu().numpy(), p)
+    assert dt_last == dt_ora
+    # the slots are left re-armed: a stand-alone reduction afterwards is unaffected
+    assert s.cfl_dt(a) == s.cfl_dt(b)
+
+
+def test_advance_detects_nonfinite_state():
+    from paper_2512_13403_b200 import dh
+    U = random_state((8, 8, 64), 93, 1.4, torch.float32).cuda()
+    s = _solver(U, 1.4)
+    U[4, 3, 3, 10] = float("nan")
+    with pytest.raises(dh.DhError) as e:
+        s.advance(U, 2)
+    assert e.value.code == dh.DH_ERR_NONFINITE
+
+
 def test_error_codes():
     from paper_2512_13403_b200 import dh
     with pytest.raises(dh.DhError):
