@@ -38,7 +38,7 @@ template <int NW> struct GeoR {
   static constexpr int XARR = 5 * TY * RXP;
   static constexpr int YARR = 5 * (TY + 1) * RTX;
   static constexpr int STAGE = 5 * TY * RTX;              // cp.async staging of one raw plane of the tile
-  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + STAGE;
+  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + 3 * STAGE;
   static constexpr int NHALO = 4 * (RSW / 2) + 2 * TY;    // halo packs per plane
   static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
 };
@@ -101,6 +101,122 @@ DH_DI void hllc_vjp2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, con
   }
 }
 
+template <class T> DH_DI P2<T> neg2(P2<T> a) { return {-a.x, -a.y}; }
+template <class T> DH_DI P2<T> zsel2(B2 m, P2<T> a) { return {m.x ? a.x : T(0), m.y ? a.y : T(0)}; }
+
+// HLLC adjoint of two faces at once: hllc_vjp() of dh_math.cuh statement by statement on packs, so that the
+// multiplies / adds / FMAs issue as packed fp32 instructions; selects, compares and MUFU stay per lane.
+template <class T, int AX>
+DH_DI void hllc_vjp2p(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, const P2<T> Fb[5], P2<T> Lb[5], P2<T> Rb[5]) {
+  constexpr int n = 1 + AX, t1 = 1 + (AX + 1) % 3, t2 = 1 + (AX + 2) % 3;
+  const P2<T> g = bc2(c.gamma), ig = bc2(c.inv_gm1), hf = bc2(T(0.5));
+  // ---- forward recompute
+  const P2<T> rL = rcp2(L[0]), rR = rcp2(R[0]);
+  const P2<T> cL2 = mul2(mul2(g, L[4]), rL), cR2 = mul2(mul2(g, R[4]), rR);
+  const P2<T> cL = {sqrt_(cL2.x), sqrt_(cL2.y)}, cR = {sqrt_(cR2.x), sqrt_(cR2.y)};
+  const P2<T> uL = L[n], uR = R[n];
+  const P2<T> sLa = sub2(uL, cL), sLb = sub2(uR, cR), sRa = add2(uL, cL), sRb = add2(uR, cR);
+  const B2 pickLa = {sLa.x <= sLb.x, sLa.y <= sLb.y}, pickRa = {sRa.x >= sRb.x, sRa.y >= sRb.y};
+  const P2<T> SL = sel2(pickLa, sLa, sLb), SR = sel2(pickRa, sRa, sRb);
+  const P2<T> dL = sub2(SL, uL), dR = sub2(SR, uR);
+  const P2<T> aL = mul2(L[0], dL), aR = mul2(R[0], dR);
+  const P2<T> num = fma2(neg2(aR), uR, fma2(aL, uL, sub2(R[4], L[4])));
+  const P2<T> iden = rcp2(sub2(aL, aR));
+  const P2<T> Ss = mul2(num, iden);
+  const B2 left = ge2(Ss, T(0)), right = {!left.x, !left.y};
+  const P2<T> rhoK = sel2(left, L[0], R[0]), uK = sel2(left, uL, uR), v1 = sel2(left, L[t1], R[t1]), v2 = sel2(left, L[t2], R[t2]);
+  const P2<T> PK = sel2(left, L[4], R[4]), SK = sel2(left, SL, SR), aK = sel2(left, aL, aR), rK = sel2(left, rL, rR);
+  const B2 seff_on = {left.x ? (SK.x < T(0)) : (SK.x > T(0)), left.y ? (SK.y < T(0)) : (SK.y > T(0))};
+  const P2<T> Seff = zsel2(seff_on, SK);
+  const P2<T> e = fma2(mul2(PK, rK), ig, mul2(hf, fma2(v2, v2, fma2(v1, v1, mul2(uK, uK)))));
+  const P2<T> EK = mul2(rhoK, e), mK = mul2(rhoK, uK);
+  const P2<T> inv = rcp2(sub2(SK, Ss));
+  const P2<T> fac = mul2(aK, inv);
+  const P2<T> Fm = fma2(Seff, sub2(fac, rhoK), mK);
+  const P2<T> Y = sub2(Ss, uK), Z = fma2(aK, Ss, PK);
+  const P2<T> X = fma2(Y, Z, mul2(aK, e));
+  const P2<T> Es = mul2(inv, X);
+  // ---- reverse
+  const P2<T> Fmb = fma2(Fb[t2], v2, fma2(Fb[t1], v1, Fb[0]));     // F_t = v_t * F_m
+  P2<T> v1b = mul2(Fb[t1], Fm), v2b = mul2(Fb[t2], Fm);
+  P2<T> uKb = mul2(Fb[4], add2(EK, PK));                            // F_E = uK (EK + PK) + Seff (Es - EK)
+  P2<T> EKb = mul2(Fb[4], sub2(uK, Seff));
+  P2<T> PKb = mul2(Fb[4], uK);
+  P2<T> Seffb = mul2(Fb[4], sub2(Es, EK));
+  const P2<T> Esb = mul2(Fb[4], Seff);
+  P2<T> invb = mul2(Esb, X);                                        // Es = inv * X,  X = aK e + Y Z
+  const P2<T> Xb = mul2(Esb, inv);
+  P2<T> aKb = mul2(Xb, e);
+  P2<T> eb = mul2(Xb, aK);
+  const P2<T> Yb = mul2(Xb, Z), Zb = mul2(Xb, Y);
+  P2<T> Ssb = Yb;
+  uKb = sub2(uKb, Yb);
+  aKb = fma2(Zb, Ss, aKb);
+  Ssb = fma2(Zb, aK, Ssb);
+  PKb = add2(PKb, Zb);
+  P2<T> mKb = mul2(Fb[n], sub2(uK, Seff));                          // F_n = mK uK + PK + Seff (fac Ss - mK)
+  uKb = fma2(Fb[n], mK, uKb);
+  PKb = add2(PKb, Fb[n]);
+  Seffb = fma2(Fb[n], fma2(fac, Ss, neg2(mK)), Seffb);
+  const P2<T> FnS = mul2(Fb[n], Seff);
+  P2<T> facb = mul2(FnS, Ss);
+  Ssb = fma2(FnS, fac, Ssb);
+  mKb = add2(mKb, Fmb);                                             // F_m = mK + Seff (fac - rhoK)
+  Seffb = fma2(Fmb, sub2(fac, rhoK), Seffb);
+  facb = fma2(Fmb, Seff, facb);
+  P2<T> rhoKb = neg2(mul2(Fmb, Seff));
+  aKb = fma2(facb, inv, aKb);                                       // fac = aK inv; inv = 1 / (SK - Ss)
+  invb = fma2(facb, aK, invb);
+  const P2<T> wb = neg2(mul2(mul2(invb, inv), inv));
+  P2<T> SKb = wb;
+  Ssb = sub2(Ssb, wb);
+  rhoKb = fma2(mKb, uK, rhoKb);                                     // mK = rhoK uK; EK = rhoK e; e = PK rK / (gamma-1) + q/2
+  uKb = fma2(mKb, rhoK, uKb);
+  rhoKb = fma2(EKb, e, rhoKb);
+  eb = fma2(EKb, rhoK, eb);
+  const P2<T> ebg = mul2(eb, ig);
+  PKb = fma2(ebg, rK, PKb);
+  const P2<T> rKb = mul2(ebg, PK);
+  uKb = fma2(eb, uK, uKb);
+  v1b = fma2(eb, v1, v1b);
+  v2b = fma2(eb, v2, v2b);
+  SKb = add2(SKb, zsel2(seff_on, Seffb));                           // Seff = SK on its active branch
+  // un-select K
+  P2<T> rhoLb = zsel2(left, rhoKb), rhoRb = zsel2(right, rhoKb), uLb = zsel2(left, uKb), uRb = zsel2(right, uKb);
+  P2<T> PLb = zsel2(left, PKb), PRb = zsel2(right, PKb), SLb = zsel2(left, SKb), SRb = zsel2(right, SKb);
+  P2<T> aLb = zsel2(left, aKb), aRb = zsel2(right, aKb), rLb = zsel2(left, rKb), rRb = zsel2(right, rKb);
+  Lb[t1] = zsel2(left, v1b); Rb[t1] = zsel2(right, v1b);
+  Lb[t2] = zsel2(left, v2b); Rb[t2] = zsel2(right, v2b);
+  const P2<T> numb = mul2(Ssb, iden);                               // Ss = num / den
+  const P2<T> denb = neg2(mul2(mul2(Ssb, Ss), iden));
+  aLb = add2(aLb, fma2(numb, uL, denb));
+  aRb = sub2(aRb, fma2(numb, uR, denb));
+  PRb = add2(PRb, numb);
+  PLb = sub2(PLb, numb);
+  uLb = fma2(numb, aL, uLb);
+  uRb = fma2(neg2(numb), aR, uRb);
+  rhoLb = fma2(aLb, dL, rhoLb);                                     // aL = rhoL dL, dL = SL - uL (and R)
+  rhoRb = fma2(aRb, dR, rhoRb);
+  const P2<T> dLb = mul2(aLb, L[0]), dRb = mul2(aRb, R[0]);
+  SLb = add2(SLb, dLb); uLb = sub2(uLb, dLb);
+  SRb = add2(SRb, dRb); uRb = sub2(uRb, dRb);
+  const B2 npRa = {!pickRa.x, !pickRa.y}, npLa = {!pickLa.x, !pickLa.y};   // SR = max(...), SL = min(...)
+  uLb = add2(uLb, add2(zsel2(pickRa, SRb), zsel2(pickLa, SLb)));
+  uRb = add2(uRb, add2(zsel2(npRa, SRb), zsel2(npLa, SLb)));
+  const P2<T> cLb = sub2(zsel2(pickRa, SRb), zsel2(pickLa, SLb));
+  const P2<T> cRb = sub2(zsel2(npRa, SRb), zsel2(npLa, SLb));
+  const P2<T> tLb = mul2(mul2(cLb, hf), rcp2(cL)), tRb = mul2(mul2(cRb, hf), rcp2(cR));   // cK = sqrt(gamma PK rK)
+  const P2<T> tLg = mul2(tLb, g), tRg = mul2(tRb, g);
+  PLb = fma2(tLg, rL, PLb);
+  PRb = fma2(tRg, rR, PRb);
+  rLb = fma2(tLg, L[4], rLb);
+  rRb = fma2(tRg, R[4], rRb);
+  rhoLb = fma2(neg2(rLb), mul2(rL, rL), rhoLb);                     // rK = 1 / rhoK
+  rhoRb = fma2(neg2(rRb), mul2(rR, rR), rhoRb);
+  Lb[0] = rhoLb; Lb[n] = uLb; Lb[4] = PLb;
+  Rb[0] = rhoRb; Rb[n] = uRb; Rb[4] = PRb;
+}
+
 }  // namespace
 
 // ------------------------------------------------------------------------------------------------ kernel A
@@ -139,10 +255,12 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
     const int so = (r + 2) * RSW + 2 * lane + 2;   // own pack inside a shared plane
     const int xo = r * RXP + lane, yo = r * RTX + 2 * lane;
     T* const ust = Ust + yo;
-    P2<T> Wprev[5], dprev[5], Lz[5], gpp[5], RbzC[5], WxyC[5];
+    T* const pk1 = Ust + G::STAGE + yo;            // parked carries (private slots): Rb of the lower z face, x+y cell terms
+    T* const pk2 = Ust + 2 * G::STAGE + yo;
+    P2<T> Wprev[5], dprev[5], Lz[5], gpp[5];
     int mzC = 0;                                   // minmod branches (z) of the cell of plane p-2, 4 bits per field
 #pragma unroll
-    for (int f = 0; f < 5; ++f) Wprev[f] = dprev[f] = Lz[f] = gpp[f] = RbzC[f] = WxyC[f] = bc2(T(0));
+    for (int f = 0; f < 5; ++f) { Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0)); rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); }
     size_t op = (size_t)pz * NP + o;
 #pragma unroll
     for (int f = 0; f < 5; ++f) rcp_async_pack(ust + f * FS, p.U + f * N + op);
@@ -195,18 +313,19 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           lam[f] = mul2(cz, sub2(gq[f], gpp[f]));
           gpp[f] = gq[f];
         }
-        hllc_vjp2<T, 2>(Lz, Rz, c, lam, Lb, Rb);
+        hllc_vjp2p<T, 2>(Lz, Rz, c, lam, Lb, Rb);
         const bool stz = (it >= 4) && store_ok;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           Lz[f] = Wn[f];
           const int m = mzC >> (4 * f);
           P2<T> wp, ce;
-          cell_terms(Lb[f].x, RbzC[f].x, m, wp.x, ce.x);
-          cell_terms(Lb[f].y, RbzC[f].y, m >> 2, wp.y, ce.y);
-          RbzC[f] = Rb[f];
+          const P2<T> RbzC = rlds2(pk1 + f * FS);
+          cell_terms(Lb[f].x, RbzC.x, m, wp.x, ce.x);
+          cell_terms(Lb[f].y, RbzC.y, m >> 2, wp.y, ce.y);
+          rsts2(pk1 + f * FS, Rb[f]);
           if (stz) {
-            rstg2(p.Wp + f * SPN + os2, add2(wp, WxyC[f]));
+            rstg2(p.Wp + f * SPN + os2, add2(wp, rlds2(pk2 + f * FS)));
             rstg2(p.C + (10 + f) * SPN + os2, ce);
           }
         }
@@ -248,7 +367,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           const T gr = Gq_s[f * FP + so + 2];
           lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
         }
-        hllc_vjp2<T, 0>(Lx, Rf, c, lam, Lbx, Rb);
+        hllc_vjp2p<T, 0>(Lx, Rf, c, lam, Lbx, Rb);
 #pragma unroll
         for (int f = 0; f < 5; ++f) { RbxA[f] = Rb[f].x; Bxs[f * XF + xo + 1] = Rb[f].y; }
 #pragma unroll
@@ -256,7 +375,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           Rf[f] = rlds2(Rys + f * YF + yo + RTX);
           lam[f] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
         }
-        hllc_vjp2<T, 1>(Ly, Rf, c, lam, Lby, Rb);
+        hllc_vjp2p<T, 1>(Ly, Rf, c, lam, Lby, Rb);
 #pragma unroll
         for (int f = 0; f < 5; ++f) rsts2(Bys + f * YF + yo + RTX, Rb[f]);
       }
@@ -274,7 +393,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           const P2<T> Rbn = rlds2(Bys + f * YF + yo);
           cell_terms(Lby[f].x, Rbn.x, my >> (4 * f), wy.x, cey.x);
           cell_terms(Lby[f].y, Rbn.y, my >> (4 * f + 2), wy.y, cey.y);
-          WxyC[f] = add2(wx, wy);
+          rsts2(pk2 + f * FS, add2(wx, wy));
           if (stxy) {
             rstg2(p.C + f * SPN + os1, cex);
             rstg2(p.C + (5 + f) * SPN + os1, cey);
@@ -456,7 +575,7 @@ __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T
 // ------------------------------------------------------------------------------------------------ launchers
 template <class T>
 cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
-  constexpr int NW = 8;
+  constexpr int NW = sizeof(T) == 4 ? 8 : 6;      // fp64 (parity only): 5 row warps so that shared memory fits
   using G = GeoR<NW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
   static bool configured = false;
