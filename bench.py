@@ -47,7 +47,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="dh", choices=["dh", "reference"])
-    ap.add_argument("--n", type=int, default=1024, help="grid size per axis (default 1024: BASELINE configs[4])")
+    ap.add_argument("--n", "--grid", dest="n", type=int, default=1024, help="grid size per axis (default 1024: BASELINE configs[4])")
     ap.add_argument("--cooling", type=int, default=0, help="1: configs[3]'s cooling source in the corrector epilogue")
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
@@ -195,6 +195,24 @@ def run_reference(a):
     print(json.dumps(line), flush=True)
 
 
+# ---------------------------------------------------------------------------------------- multi-rank helpers
+def reduce_max_ms(ms: float, world: int, device=None) -> float:
+    """Replicas only: the time of a multi-rank run is the slowest rank's device time."""
+    if world == 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([ms], device=device if device is not None else "cpu", dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(cells_per_rank: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job throughput: every rank advances its own replica, so the cells add up and the time is the max."""
+    return world * cells_per_rank * steps / (ms_max * 1e-3)
+
+
 # --------------------------------------------------------------------------------------------------- dh leg
 def run_dh(a):
     import torch
@@ -275,11 +293,7 @@ def run_dh(a):
         return ms, s.launch_count - l0, t0, t1
 
     def max_over_ranks(ms):
-        if world == 1:
-            return ms
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return reduce_max_ms(ms, world, dev)
 
     # ---- forward: warm-up, then the timed region with per-kernel events and the clock sampler running
     fwd_step(W) if flush is None else [fwd_step() for _ in range(W)]
@@ -291,7 +305,7 @@ def run_dh(a):
     prof = s.profile_read()
     dt_last = s.poll()
     ms_fwd = max_over_ranks(ms_fwd)
-    value = world * N * K / (ms_fwd * 1e-3)
+    value = aggregate_value(N, K, world, ms_fwd)
 
     peak, peak_src = measured_peak()
     gbs = lambda words, ms, cnt: (words * 4.0 * N * cnt) / (ms * 1e-3) / 1e9 if ms > 0 else None
