@@ -38,7 +38,7 @@ template <int NW> struct GeoR {
   static constexpr int XARR = 5 * TY * RXP;
   static constexpr int YARR = 5 * (TY + 1) * RTX;
   static constexpr int STAGE = 5 * TY * RTX;              // cp.async staging of one raw plane of the tile
-  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + 3 * STAGE;
+  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + 6 * STAGE;
   static constexpr int NHALO = 4 * (RSW / 2) + 2 * TY;    // halo packs per plane
   static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
 };
@@ -69,15 +69,24 @@ DH_DI double enc_flag(double v, bool pa) {
 DH_DI bool dec_flag(float v) { return (__float_as_uint(v) & 1u) != 0u; }
 DH_DI bool dec_flag(double v) { return (__double_as_longlong(v) & 1ll) != 0ll; }
 
-// minmod branch of slope (a, b): bit 0 = slope active (a b > 0), bit 1 = a-branch (|a| <= |b|)   (reading A7)
-template <class T> DH_DI int mm_mask(T a, T b) { return ((a * b > T(0)) ? 1 : 0) | ((abs_(a) <= abs_(b)) ? 2 : 0); }
-
-// cell cotangents of one axis from the two face adjoints: returns T + own-branch term, and the encoded c
-template <class T> DH_DI void cell_terms(T Lb, T Rbn, int m, T& wp, T& cenc) {
-  const T S = T(0.5) * (Lb - Rbn);
-  const bool on = (m & 1) != 0, pa = (m & 2) != 0;
-  wp = (Lb + Rbn) + (on ? (pa ? -S : S) : T(0));
-  cenc = enc_flag(on ? S : T(0), pa);
+// minmod branch of slope (a, b) as a factor: 0 if the slope is inactive (a b <= 0), -1/2 on the a-branch
+// (|a| <= |b|), +1/2 on the b-branch (reading A7).  With D = Lb - Rbn (so S = D / 2): the cell's own-branch term is
+// k D, the masked slope cotangent is |k| D, and the a-branch flag is the sign bit of k.
+template <class T> DH_DI T kfac(T a, T b) {
+  const T k = (abs_(a) <= abs_(b)) ? T(-0.5) : T(0.5);
+  return (a * b > T(0)) ? k : T(0);
+}
+template <class T> DH_DI P2<T> kfac2(P2<T> a, P2<T> b) { return {kfac(a.x, b.x), kfac(a.y, b.y)}; }
+DH_DI float enc_sign(float v, float k) { return __uint_as_float((__float_as_uint(v) & ~1u) | (__float_as_uint(k) >> 31)); }
+DH_DI double enc_sign(double v, double k) {
+  return __longlong_as_double((__double_as_longlong(v) & ~1ll) | (long long)((unsigned long long)__double_as_longlong(k) >> 63));
+}
+// cell cotangents of one axis from the two face adjoints of two cells: wp = T + own-branch term, ce = encoded c
+template <class T> DH_DI void cell_terms2(P2<T> Lb, P2<T> Rbn, P2<T> k, P2<T>& wp, P2<T>& ce) {
+  const P2<T> D = sub2(Lb, Rbn);
+  wp = fma2(k, D, add2(Lb, Rbn));
+  const P2<T> c = mul2(P2<T>{abs_(k.x), abs_(k.y)}, D);
+  ce = {enc_sign(c.x, k.x), enc_sign(c.y, k.y)};
 }
 
 // HLLC adjoint of two faces: the scalar routine of dh_math.cuh on each half of the packs.  The loop over the halves
@@ -257,10 +266,12 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
     T* const ust = Ust + yo;
     T* const pk1 = Ust + G::STAGE + yo;            // parked carries (private slots): Rb of the lower z face, x+y cell terms
     T* const pk2 = Ust + 2 * G::STAGE + yo;
+    T* const pkx = Ust + 3 * G::STAGE + yo;           // parked minmod branch factors of the own cells: x, y, z
+    T* const pky = Ust + 4 * G::STAGE + yo;
+    T* const pkz = Ust + 5 * G::STAGE + yo;
     P2<T> Wprev[5], dprev[5], Lz[5], gpp[5];
-    int mzC = 0;                                   // minmod branches (z) of the cell of plane p-2, 4 bits per field
 #pragma unroll
-    for (int f = 0; f < 5; ++f) { Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0)); rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); }
+    for (int f = 0; f < 5; ++f) { Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0)); rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); rsts2(pkz + f * FS, bc2(T(0))); }
     size_t op = (size_t)pz * NP + o;
 #pragma unroll
     for (int f = 0; f < 5; ++f) rcp_async_pack(ust + f * FS, p.U + f * N + op);
@@ -301,12 +312,12 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
       // ---- z: slope of plane p-1, adjoint of the face between p-2 and p-1, which completes the cell of plane p-2
       {
         P2<T> Rz[5], lam[5], Lb[5], Rb[5];
-        int mz = 0;
+        P2<T> kz[5];
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           const P2<T> a = sub2(Wn[f], Wprev[f]);
           const P2<T> s = limit2<T, 0>(a, dprev[f]);
-          mz |= (mm_mask(a.x, dprev[f].x) | (mm_mask(a.y, dprev[f].y) << 2)) << (4 * f);
+          kz[f] = kfac2(a, dprev[f]);
           Rz[f] = fma2(nhalf, s, Wprev[f]);
           Wn[f] = fma2(half, s, Wprev[f]);           // left state of the NEXT z face
           dprev[f] = a;
@@ -318,23 +329,19 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           Lz[f] = Wn[f];
-          const int m = mzC >> (4 * f);
           P2<T> wp, ce;
-          const P2<T> RbzC = rlds2(pk1 + f * FS);
-          cell_terms(Lb[f].x, RbzC.x, m, wp.x, ce.x);
-          cell_terms(Lb[f].y, RbzC.y, m >> 2, wp.y, ce.y);
+          cell_terms2(Lb[f], rlds2(pk1 + f * FS), rlds2(pkz + f * FS), wp, ce);   // cell of plane p-2: parked Rb and factor
           rsts2(pk1 + f * FS, Rb[f]);
+          rsts2(pkz + f * FS, kz[f]);
           if (stz) {
             rstg2(p.Wp + f * SPN + os2, add2(wp, rlds2(pk2 + f * FS)));
             rstg2(p.C + (10 + f) * SPN + os2, ce);
           }
         }
-        mzC = mz;
       }
 
       // ---- x / y on plane p-1, phase 1: slopes of the own cells, publish the R states
       P2<T> Lx[5], Rxo[5], Ly[5];
-      int mx = 0, my = 0;
 #pragma unroll
       for (int f = 0; f < 5; ++f) {
         const T* row = Wq_s + f * FP + so;
@@ -342,7 +349,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         {
           const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = row[2] - W.y;
           const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
-          mx |= (mm_mask(d1, d0) | (mm_mask(d2, d1) << 2)) << (4 * f);
+          rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
           Lx[f] = fma2(half, s, W);
           Rxo[f] = fma2(nhalf, s, W);
           Rxs[f * XF + xo] = Rxo[f].x;
@@ -350,7 +357,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         {
           const P2<T> a = sub2(rlds2(row + RSW), W), b = sub2(W, rlds2(row - RSW));
           const P2<T> s = limit2<T, 0>(a, b);
-          my |= (mm_mask(a.x, b.x) | (mm_mask(a.y, b.y) << 2)) << (4 * f);
+          rsts2(pky + f * FS, kfac2(a, b));
           Ly[f] = fma2(half, s, W);
           rsts2(Rys + f * YF + yo, fma2(nhalf, s, W));
         }
@@ -388,11 +395,8 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           P2<T> wx, cex, wy, cey;
-          cell_terms(Lbx[f].x, Bxs[f * XF + xo], mx >> (4 * f), wx.x, cex.x);
-          cell_terms(Lbx[f].y, RbxA[f], mx >> (4 * f + 2), wx.y, cex.y);
-          const P2<T> Rbn = rlds2(Bys + f * YF + yo);
-          cell_terms(Lby[f].x, Rbn.x, my >> (4 * f), wy.x, cey.x);
-          cell_terms(Lby[f].y, Rbn.y, my >> (4 * f + 2), wy.y, cey.y);
+          cell_terms2(Lbx[f], P2<T>{Bxs[f * XF + xo], RbxA[f]}, rlds2(pkx + f * FS), wx, cex);
+          cell_terms2(Lby[f], rlds2(Bys + f * YF + yo), rlds2(pky + f * FS), wy, cey);
           rsts2(pk2 + f * FS, add2(wx, wy));
           if (stxy) {
             rstg2(p.C + f * SPN + os1, cex);
