@@ -13,8 +13,9 @@
 // everything in one kernel would make every tile recompute two extra layers of face adjoints around itself; the
 // one-thread-per-cell gather kernel (dh_naive.cu) does exactly that and spends 12 HLLC adjoints per cell.  Here
 // the work is split in two launches that share a scratch slab:
-//   A  rev_faces_kernel   fused z-sweep (same block shape as the first fused forward kernel): every face adjoint
-//                         once; writes per cell  Wp = sum_a (T_i + own-branch term)  and, per axis, c_i = S_i
+//   A  rev_faces_kernel   fused z-sweep (7 row warps x one pack + helper; z in registers, x / y through shared planes,
+//                         R states of the neighbouring cells recomputed locally, ONE block barrier per plane): every
+//                         face adjoint once; writes per cell  Wp = sum_a (T_i + own-branch term)  and, per axis, c_i = S_i
 //                         masked by (a b > 0), with the branch flag stored in the mantissa LSB (<= 1 ulp);
 //   B  rev_gather_kernel  streaming: Wb_i = Wp_i + sum_a [a-branch c_{i-1}] - [b-branch c_{i+1}], then
 //                         Ub = prim_vjp(U, Wb) + b1 + b2.
@@ -61,11 +62,7 @@ template <class T> DH_DI void rcp_async_pack(T* smem_dst, const T* gmem_src) {
 DH_DI void rcp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 DH_DI void rcp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
-// branch flag in the mantissa LSB of the masked slope cotangent
-DH_DI float enc_flag(float v, bool pa) { return __uint_as_float((__float_as_uint(v) & ~1u) | (pa ? 1u : 0u)); }
-DH_DI double enc_flag(double v, bool pa) {
-  return __longlong_as_double((__double_as_longlong(v) & ~1ll) | (pa ? 1ll : 0ll));
-}
+// branch flag in the mantissa LSB of the masked slope cotangent (written by enc_sign below)
 DH_DI bool dec_flag(float v) { return (__float_as_uint(v) & 1u) != 0u; }
 DH_DI bool dec_flag(double v) { return (__double_as_longlong(v) & 1ll) != 0ll; }
 
@@ -238,11 +235,9 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
   extern __shared__ __align__(16) unsigned char smem_rev[];
   T* const Wsm = reinterpret_cast<T*>(smem_rev);   // [2][5][SR][RSW]  primitive planes p (it&1) and p-1
   T* const Gsm = Wsm + 2 * G::PLANE;               // [2][5][SR][RSW]  cotangent planes p and p-1 (halo 1 used)
-  T* const Rxs = Gsm + 2 * G::PLANE;               // [5][TY][RXP]     R state of the first cell of lane l (l = 32: halo column)
-  T* const Bxs = Rxs + G::XARR;                    // [5][TY][RXP]     Rb of the face LEFT of lane l's pack (slot 0: helper)
-  T* const Rys = Bxs + G::XARR;                    // [5][TY+1][RTX]   R states of row r (r = TY: halo row)
-  T* const Bys = Rys + G::YARR;                    // [5][TY+1][RTX]   Rb of the face BELOW row r (slot 0: helper)
-  T* const Ust = Bys + G::YARR;                    // [5][TY][RTX]     raw U of the next plane (cp.async, private slots)
+  T* const Rxs = Gsm + 2 * G::PLANE;               // [2][5][TY][RXP]   Rb of the face LEFT of lane l's pack (slot 0: helper), by iteration parity
+  T* const Rys = Rxs + 2 * G::XARR;                // [2][5][TY+1][RTX] Rb of the face BELOW row r (slot 0: helper), by iteration parity
+  T* const Ust = Rys + 2 * G::YARR;                    // [5][TY][RTX]     raw U of the next plane (cp.async, private slots)
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -340,51 +335,47 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         }
       }
 
-      // ---- x / y on plane p-1, phase 1: slopes of the own cells, publish the R states
-      P2<T> Lx[5], Rxo[5], Ly[5];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        const T* row = Wq_s + f * FP + so;
-        const P2<T> W = Wprev[f];
-        {
-          const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = row[2] - W.y;
-          const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
-          rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
-          Lx[f] = fma2(half, s, W);
-          Rxo[f] = fma2(nhalf, s, W);
-          Rxs[f * XF + xo] = Rxo[f].x;
-        }
-        {
-          const P2<T> a = sub2(rlds2(row + RSW), W), b = sub2(W, rlds2(row - RSW));
-          const P2<T> s = limit2<T, 0>(a, b);
-          rsts2(pky + f * FS, kfac2(a, b));
-          Ly[f] = fma2(half, s, W);
-          rsts2(Rys + f * YF + yo, fma2(nhalf, s, W));
-        }
-      }
-      __syncthreads();
-      // ---- phase 2: adjoints of the own right (x) and top (y) faces, publish the R-side cotangents
+      // ---- x / y on plane p-1: slopes of the own cells and of the next cell along the axis (recomputed from the shared
+      // plane, so no R-state exchange and no barrier before the face adjoints), adjoints of the own right (x) and top (y)
+      // faces, publish the R-side cotangents
+      T* const Bx_s = Rxs + bp * G::XARR;           // [2][5][TY][RXP]  (Rxs, Bxs are contiguous: two buffers)
+      T* const By_s = Rys + bp * G::YARR;           // [2][5][TY+1][RTX]
       P2<T> Lbx[5], Lby[5];
       T RbxA[5];                                    // Rb of the face between the two own cells (belongs to the second cell)
       {
-        P2<T> Rf[5], lam[5], Rb[5];
+        P2<T> Lf[5], Rf[5], lam[5], Rb[5];
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          Rf[f] = {Rxo[f].y, Rxs[f * XF + xo + 1]};
+          const T* row = Wq_s + f * FP + so;
+          const P2<T> W = Wprev[f];
+          const T wr = row[2], wr2 = row[3];
+          const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = wr - W.y;
+          const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
+          rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
+          Lf[f] = fma2(half, s, W);
+          const T Rown = fma_(T(-0.5), s.y, W.y);                         // R state of the second own cell
+          const T Rnext = fma_(T(-0.5), minmod_(wr2 - wr, d2), wr);       // R state of the cell right of the pack
+          Rf[f] = {Rown, Rnext};
           const T gr = Gq_s[f * FP + so + 2];
           lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
         }
-        hllc_vjp2p<T, 0>(Lx, Rf, c, lam, Lbx, Rb);
+        hllc_vjp2p<T, 0>(Lf, Rf, c, lam, Lbx, Rb);
 #pragma unroll
-        for (int f = 0; f < 5; ++f) { RbxA[f] = Rb[f].x; Bxs[f * XF + xo + 1] = Rb[f].y; }
+        for (int f = 0; f < 5; ++f) { RbxA[f] = Rb[f].x; Bx_s[f * XF + xo + 1] = Rb[f].y; }
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          Rf[f] = rlds2(Rys + f * YF + yo + RTX);
+          const T* row = Wq_s + f * FP + so;
+          const P2<T> W = Wprev[f], Wu = rlds2(row + RSW), Wu2 = rlds2(row + 2 * RSW);
+          const P2<T> a = sub2(Wu, W), b = sub2(W, rlds2(row - RSW));
+          const P2<T> s = limit2<T, 0>(a, b);
+          rsts2(pky + f * FS, kfac2(a, b));
+          Lf[f] = fma2(half, s, W);
+          Rf[f] = fma2(nhalf, limit2<T, 0>(sub2(Wu2, Wu), a), Wu);        // R state of the row above
           lam[f] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
         }
-        hllc_vjp2p<T, 1>(Ly, Rf, c, lam, Lby, Rb);
+        hllc_vjp2p<T, 1>(Lf, Rf, c, lam, Lby, Rb);
 #pragma unroll
-        for (int f = 0; f < 5; ++f) rsts2(Bys + f * YF + yo + RTX, Rb[f]);
+        for (int f = 0; f < 5; ++f) rsts2(By_s + f * YF + yo + RTX, Rb[f]);
       }
       rcp_async_wait_all();                         // cotangent plane p and the next raw plane have landed
       __syncthreads();
@@ -395,8 +386,8 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           P2<T> wx, cex, wy, cey;
-          cell_terms2(Lbx[f], P2<T>{Bxs[f * XF + xo], RbxA[f]}, rlds2(pkx + f * FS), wx, cex);
-          cell_terms2(Lby[f], rlds2(Bys + f * YF + yo), rlds2(pky + f * FS), wy, cey);
+          cell_terms2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, rlds2(pkx + f * FS), wx, cex);
+          cell_terms2(Lby[f], rlds2(By_s + f * YF + yo), rlds2(pky + f * FS), wy, cey);
           rsts2(pk2 + f * FS, add2(wx, wy));
           if (stxy) {
             rstg2(p.C + f * SPN + os1, cex);
@@ -452,53 +443,38 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         }
       }
       rcp_async_commit();
-      P2<T> LyB[5];
-      T LxB[5];
-#pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        const T* pl = Wq_s + f * FP;
-        // y: R state of the halo row TY, L state of the halo row -1
-        const T* col = pl + 2 * lane + 2;
-        {
-          const P2<T> Wm = rlds2(col + (TY + 1) * RSW), W = rlds2(col + (TY + 2) * RSW), Wu = rlds2(col + (TY + 3) * RSW);
-          const P2<T> s = limit2<T, 0>(sub2(Wu, W), sub2(W, Wm));
-          rsts2(Rys + f * YF + TY * RTX + 2 * lane, fma2(nhalf, s, W));
-        }
-        {
-          const P2<T> Wm = rlds2(col), W = rlds2(col + RSW), Wu = rlds2(col + 2 * RSW);
-          const P2<T> s = limit2<T, 0>(sub2(Wu, W), sub2(W, Wm));
-          LyB[f] = fma2(half, s, W);
-        }
-        // x: L state of the halo column -1, R state of the halo column RTX, row rl
-        const T* rw = pl + (rl + 2) * RSW;
-        const T sl = minmod_(rw[2] - rw[1], rw[1] - rw[0]);
-        LxB[f] = fma_(T(0.5), sl, rw[1]);
-        const T sr = minmod_(rw[RTX + 3] - rw[RTX + 2], rw[RTX + 2] - rw[RTX + 1]);
-        if (lane < TY) Rxs[f * XF + rl * RXP + 32] = fma_(T(-0.5), sr, rw[RTX + 2]);
-      }
-      __syncthreads();
+      // the two faces nobody in the tile owns, plane p-1: bottom y face row and left x face column (row rl).  L and R
+      // states come from the shared plane of the previous iteration; only the R-side cotangents are needed here.
+      T* const Bx_s = Rxs + bp * G::XARR;
+      T* const By_s = Rys + bp * G::YARR;
       {
         P2<T> Lf[5], Rf[5], lam[5], Lb[5], Rb[5];
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          Rf[f] = rlds2(Rys + f * YF + 2 * lane);
+          const T* col = Wq_s + f * FP + 2 * lane + 2;
+          const P2<T> Wm2 = rlds2(col), Wm1 = rlds2(col + RSW), W0 = rlds2(col + 2 * RSW), W1 = rlds2(col + 3 * RSW);
+          const P2<T> d0 = sub2(W0, Wm1);
+          Lf[f] = fma2(half, limit2<T, 0>(d0, sub2(Wm1, Wm2)), Wm1);
+          Rf[f] = fma2(nhalf, limit2<T, 0>(sub2(W1, W0), d0), W0);
           const T* gc = Gq_s + f * FP + 2 * lane + 2;
           lam[f] = mul2(cy, sub2(rlds2(gc + 2 * RSW), rlds2(gc + RSW)));
         }
-        hllc_vjp2<T, 1>(LyB, Rf, c, lam, Lb, Rb);  // bottom y face of the tile
+        hllc_vjp2<T, 1>(Lf, Rf, c, lam, Lb, Rb);   // bottom y face of the tile
 #pragma unroll
-        for (int f = 0; f < 5; ++f) rsts2(Bys + f * YF + 2 * lane, Rb[f]);
+        for (int f = 0; f < 5; ++f) rsts2(By_s + f * YF + 2 * lane, Rb[f]);
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          Lf[f] = bc2(LxB[f]);
-          Rf[f] = bc2(Rxs[f * XF + rl * RXP]);
+          const T* rw = Wq_s + f * FP + (rl + 2) * RSW;
+          const T dc = rw[2] - rw[1];
+          Lf[f] = bc2(fma_(T(0.5), minmod_(dc, rw[1] - rw[0]), rw[1]));
+          Rf[f] = bc2(fma_(T(-0.5), minmod_(rw[3] - rw[2], dc), rw[2]));
           const T* gr = Gq_s + f * FP + (rl + 2) * RSW;
           lam[f] = bc2(p.coef[0] * (gr[2] - gr[1]));
         }
         hllc_vjp2<T, 0>(Lf, Rf, c, lam, Lb, Rb);   // left x face of the tile, row rl
         if (lane < TY) {
 #pragma unroll
-          for (int f = 0; f < 5; ++f) Bxs[f * XF + rl * RXP] = Rb[f].x;
+          for (int f = 0; f < 5; ++f) Bx_s[f * XF + rl * RXP] = Rb[f].x;
         }
       }
       // halo primitives of plane p -> shared
