@@ -342,40 +342,50 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
       T* const By_s = Rys + bp * G::YARR;           // [2][5][TY+1][RTX]
       P2<T> Lbx[5], Lby[5];
       T RbxA[5];                                    // Rb of the face between the two own cells (belongs to the second cell)
-      {
-        P2<T> Lf[5], Rf[5], lam[5], Rb[5];
+      // One copy of the (large) packed adjoint serves both axes: the y pass hands it the state with the components
+      // permuted so that the face normal is component 1 (the loop is not unrolled; it keeps the plane-loop body small
+      // enough for the instruction cache, see profiles/r01c).
+      constexpr int PY[5] = {0, 3, 1, 2, 4};        // field f of a y face goes to slot PY[f]: (rho, vy, vz, vx, P)
+#pragma unroll 1
+      for (int ax = 0; ax < 2; ++ax) {
+        P2<T> Lf[5], Rf[5], lam[5], Lb[5], Rb[5];
+        if (ax == 0) {
 #pragma unroll
-        for (int f = 0; f < 5; ++f) {
-          const T* row = Wq_s + f * FP + so;
-          const P2<T> W = Wprev[f];
-          const T wr = row[2], wr2 = row[3];
-          const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = wr - W.y;
-          const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
-          rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
-          Lf[f] = fma2(half, s, W);
-          const T Rown = fma_(T(-0.5), s.y, W.y);                         // R state of the second own cell
-          const T Rnext = fma_(T(-0.5), minmod_(wr2 - wr, d2), wr);       // R state of the cell right of the pack
-          Rf[f] = {Rown, Rnext};
-          const T gr = Gq_s[f * FP + so + 2];
-          lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
+          for (int f = 0; f < 5; ++f) {
+            const T* row = Wq_s + f * FP + so;
+            const P2<T> W = Wprev[f];
+            const T wr = row[2], wr2 = row[3];
+            const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = wr - W.y;
+            const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
+            rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
+            Lf[f] = fma2(half, s, W);
+            const T Rown = fma_(T(-0.5), s.y, W.y);                         // R state of the second own cell
+            const T Rnext = fma_(T(-0.5), minmod_(wr2 - wr, d2), wr);       // R state of the cell right of the pack
+            Rf[f] = {Rown, Rnext};
+            const T gr = Gq_s[f * FP + so + 2];
+            lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
+          }
+        } else {
+#pragma unroll
+          for (int f = 0; f < 5; ++f) {
+            const T* row = Wq_s + f * FP + so;
+            const P2<T> W = Wprev[f], Wu = rlds2(row + RSW), Wu2 = rlds2(row + 2 * RSW);
+            const P2<T> a = sub2(Wu, W), b = sub2(W, rlds2(row - RSW));
+            const P2<T> s = limit2<T, 0>(a, b);
+            rsts2(pky + f * FS, kfac2(a, b));
+            Lf[PY[f]] = fma2(half, s, W);
+            Rf[PY[f]] = fma2(nhalf, limit2<T, 0>(sub2(Wu2, Wu), a), Wu);    // R state of the row above
+            lam[PY[f]] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
+          }
         }
-        hllc_vjp2p<T, 0>(Lf, Rf, c, lam, Lbx, Rb);
+        hllc_vjp2p<T, 0>(Lf, Rf, c, lam, Lb, Rb);
+        if (ax == 0) {
 #pragma unroll
-        for (int f = 0; f < 5; ++f) { RbxA[f] = Rb[f].x; Bx_s[f * XF + xo + 1] = Rb[f].y; }
+          for (int f = 0; f < 5; ++f) { Lbx[f] = Lb[f]; RbxA[f] = Rb[f].x; Bx_s[f * XF + xo + 1] = Rb[f].y; }
+        } else {
 #pragma unroll
-        for (int f = 0; f < 5; ++f) {
-          const T* row = Wq_s + f * FP + so;
-          const P2<T> W = Wprev[f], Wu = rlds2(row + RSW), Wu2 = rlds2(row + 2 * RSW);
-          const P2<T> a = sub2(Wu, W), b = sub2(W, rlds2(row - RSW));
-          const P2<T> s = limit2<T, 0>(a, b);
-          rsts2(pky + f * FS, kfac2(a, b));
-          Lf[f] = fma2(half, s, W);
-          Rf[f] = fma2(nhalf, limit2<T, 0>(sub2(Wu2, Wu), a), Wu);        // R state of the row above
-          lam[f] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
+          for (int f = 0; f < 5; ++f) { Lby[f] = Lb[PY[f]]; rsts2(By_s + f * YF + yo + RTX, Rb[PY[f]]); }
         }
-        hllc_vjp2p<T, 1>(Lf, Rf, c, lam, Lby, Rb);
-#pragma unroll
-        for (int f = 0; f < 5; ++f) rsts2(By_s + f * YF + yo + RTX, Rb[f]);
       }
       rcp_async_wait_all();                         // cotangent plane p and the next raw plane have landed
       __syncthreads();
