@@ -9,9 +9,10 @@ One JSON line on stdout (rank 0).  Contract and the meaning of every key: DESIGN
 
 * workload (default): BASELINE.json configs[4] — 1024^3 fp32 periodic decaying turbulence, rms Mach 2, no
   cooling (21.5 GB per state, far larger than the 126 MB L2, so no L2 flush is needed between iterations).
-* a "step" = dh_cfl_dt_async + dh_step_devdt (CFL reduction, predictor stage, corrector stage; dt never leaves
-  the device).  `value` = cells * K / time, inputs resident in HBM.  The VJP of the step (dh_step_vjp) is timed
-  in the same run and reported under "vjp".
+* a "step" = CFL reduction + dt epilogue + predictor stage + corrector stage; the K timed steps are one
+  dh_advance(U, K) call (dt never leaves the device; --no-chain issues dh_cfl_dt_async + dh_step_devdt per step
+  instead).  `value` = cells * K / time, inputs resident in HBM.  The VJP of the step (dh_step_vjp) is timed in the
+  same run and reported under "vjp".
 * "e2e" = the same step through dh_run_host: pinned HOST buffer -> device, CFL + step, device -> HOST, all
   inside the timed region.
 * N > 1: the path does not shard in this build ("replicas only"): every rank runs the same-shaped
