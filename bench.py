@@ -53,6 +53,7 @@ def parse_args():
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
     ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
+    ap.add_argument("--adjoint", type=int, default=0, help="also time dh_adjoint over this many steps (checkpointed multi-step adjoint)")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -365,6 +366,29 @@ def run_dh(a):
                                                    for k, v in pv.items() if v[1] > 0}}}
         line["gpu_launches"] += launches_v
         del g, gin
+        torch.cuda.empty_cache()
+
+    # ---- multi-step adjoint: forward sweep with checkpoints + reverse sweep with recomputation
+    if a.adjoint > 0:
+        import math
+        every = max(1, int(round(math.sqrt(a.adjoint))))
+        Ua = U.clone()
+        ga = workloads.cotangent(U.shape, seed=3005 + rank, dtype=torch.float32, device=dev)
+        s.adjoint(Ua, ga, a.adjoint, every)                  # warm-up: allocates the checkpoints
+        Ua.copy_(U)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        s.adjoint(Ua, ga, a.adjoint, every)
+        e1.record()
+        barrier()
+        ms_a = max_over_ranks(e0.elapsed_time(e1))
+        nck = -(-a.adjoint // every)
+        line["adjoint"] = {"steps": a.adjoint, "checkpoint_every": every, "ms": ms_a,
+                           "value": world * N * a.adjoint / (ms_a * 1e-3), "unit": "cell-step-adjoints/s",
+                           "states_held": nck + every + 1,
+                           "work": "forward sweep (CFL + step) + recomputation of every segment + one VJP per step"}
+        del Ua, ga
         torch.cuda.empty_cache()
 
     # ---- end to end: pinned HOST state -> dh_run_host (H2D, CFL + step, D2H) -> HOST, all inside the timed region

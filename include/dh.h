@@ -124,6 +124,18 @@ int dh_advance(dh_ctx* ctx, void* U, int nsteps, double* dt_last_out);
  * U or gU_out.  Asynchronous on the context's stream. */
 int dh_step_vjp(dh_ctx* ctx, const void* U, double dt, const void* gU_out, void* gU_in);
 
+/* Adjoint of `nsteps` steps with sparse checkpoints and recomputation of short segments (§2.3;
+ * SURVEY.md §8(f) item 1).  Forward: U_0 -> U_n in place, dt_k from Eq. A8 before every step (device resident), every
+ * `every`-th state and all dt_k kept.  Reverse: walking the segments backwards, the states of a segment are recomputed
+ * from its checkpoint and dh_step_vjp is applied step by step with dt_k held constant.
+ *   U:  DEVICE, in: U_0, out: U_n.      gU: DEVICE, in: dL/dU_n, out: dL/dU_0 (overwritten); must not alias U.
+ *   every >= 1: checkpoint spacing; the library allocates ceil(nsteps / every) + every + 1 states on first use
+ *   (about 2 sqrt(nsteps) states for every ~ sqrt(nsteps)) and keeps them until dh_destroy.
+ *   dts_out: HOST array of nsteps doubles, or NULL.
+ * Synchronises the stream once (after the forward sweep, to fetch the dt sequence); returns DH_ERR_NONFINITE if a
+ * CFL reduction of the forward sweep found a non-finite state. */
+int dh_adjoint(dh_ctx* ctx, void* U, void* gU, int nsteps, int every, double* dts_out);
+
 /* HOST-buffer entry points (used for end-to-end measurements): U_host is a HOST array (pinned memory gives
  * asynchronous copies) of the same layout.  The library copies it to a device state it owns, runs
  * `nsteps` x (CFL dt + step) with the device-resident dt, copies the result back and synchronises.

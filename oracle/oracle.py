@@ -226,3 +226,18 @@ def window_step_vjp(U_full, dt, g_full, p, lo, size, halo=8):
     sel = (slice(None), idx[0][:, None, None], idx[1][None, :, None], idx[2][None, None, :])
     out = step_vjp(np.asarray(U_full)[sel], dt, np.asarray(g_full)[sel], p)
     return out[:, halo:-halo, halo:-halo, halo:-halo]
+
+
+def adjoint(U0, nsteps, g_final, p, cfl=0.4):
+    """Adjoint of `nsteps` steps: the plain composition, no checkpoints.  Forward: dt_k from Eq. A8
+    (in the array's own dtype, like cfl_dt) then one step, all states kept; reverse: step_vjp applied backwards with
+    every dt_k held constant.  Returns (U_n, dL/dU_0, [dt_k])."""
+    states, dts = [np.array(U0, copy=True)], []
+    for _ in range(nsteps):
+        dt, _ = cfl_dt(states[-1], p, cfl)
+        dts.append(dt)
+        states.append(step(states[-1], dt, p).astype(states[-1].dtype))
+    g = np.asarray(g_final, dtype=np.float64)
+    for k in range(nsteps - 1, -1, -1):
+        g = step_vjp(states[k], dts[k], g, p)
+    return states[-1], g, dts

@@ -141,10 +141,11 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->acc, c->dt_dev, c->result_dev};
+  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
+  if (c->adj_dts_host) cudaFreeHost(c->adj_dts_host);
   prof_drop(c);
   free(c->prof);
   delete c;
@@ -457,6 +458,81 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
     if (rc) return rc;
   }
   if (dt_last_out) return dh_poll_status(c, dt_last_out);
+  return DH_OK;
+}
+
+int dh_adjoint(dh_ctx* c, void* U, void* gU, int nsteps, int every, double* dts_out) {
+  if (!c || !U || !gU || nsteps < 0 || every < 1) return fail(DH_ERR_ARG, "dh_adjoint: bad argument%s");
+  if (U == gU || U == c->Us || gU == c->Us) return fail(DH_ERR_ARG, "dh_adjoint: U and gU must be distinct caller arrays%s");
+  if (nsteps == 0) return DH_OK;
+  if (every > nsteps) every = nsteps;
+  const size_t sb = state_bytes(c);
+  const int nck = (nsteps + every - 1) / every;                 // checkpoints: states before steps 0, every, 2 every, ...
+  const size_t need = (size_t)nck + (size_t)every + 1;          // + one segment of states + one cotangent
+  if (c->adj_states && c->adj_count < need) {
+    DH_CUDA(cudaStreamSynchronize(c->stream), "dh_adjoint: synchronize");
+    cudaFree(c->adj_states);
+    c->adj_states = nullptr;
+  }
+  if (!c->adj_states) {
+    int rc = lazy_alloc(c, &c->adj_states, need * sb, "the checkpoints of dh_adjoint");
+    if (rc) return rc;
+    c->adj_count = need;
+  }
+  if (c->adj_dts_cap < nsteps) {
+    DH_CUDA(cudaStreamSynchronize(c->stream), "dh_adjoint: synchronize");
+    if (c->adj_dts_dev) cudaFree(c->adj_dts_dev);
+    if (c->adj_dts_host) cudaFreeHost(c->adj_dts_host);
+    c->adj_dts_dev = nullptr; c->adj_dts_host = nullptr; c->adj_dts_cap = 0;
+    if (cudaMalloc((void**)&c->adj_dts_dev, 2 * (size_t)nsteps * 8) != cudaSuccess ||
+        cudaMallocHost((void**)&c->adj_dts_host, 2 * (size_t)nsteps * 8) != cudaSuccess) {
+      cudaGetLastError();
+      return fail(DH_ERR_ALLOC, "dh_adjoint: allocation of the dt sequence failed%s");
+    }
+    c->adj_dts_cap = nsteps;
+  }
+  char* const base = (char*)c->adj_states;
+  auto ckpt = [&](int i) { return (void*)(base + (size_t)i * sb); };
+  auto seg = [&](int j) { return (void*)(base + ((size_t)nck + j) * sb); };
+  void* gtmp = (void*)(base + ((size_t)nck + every) * sb);
+  const bool f32 = c->dtype == DH_F32;
+  // ---- forward sweep: checkpoints and the dt sequence (dt never visits the host inside the loop)
+  for (int k = 0; k < nsteps; ++k) {
+    if (k % every == 0) DH_CUDA(cudaMemcpyAsync(ckpt(k / every), U, sb, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: checkpoint");
+    int rc = f32 ? cfl_launch<float>(c, U) : cfl_launch<double>(c, U);
+    if (rc) return rc;
+    DH_CUDA(cudaMemcpyAsync(c->adj_dts_dev + k, &c->result_dev->dt, 8, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: dt");
+    DH_CUDA(cudaMemcpyAsync(c->adj_dts_dev + nsteps + k, &c->result_dev->nonfinite, 8, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: flag");
+    rc = f32 ? step_impl<float>(c, U, 0.0, true) : step_impl<double>(c, U, 0.0, true);
+    if (rc) return rc;
+  }
+  DH_CUDA(cudaMemcpyAsync(c->adj_dts_host, c->adj_dts_dev, 2 * (size_t)nsteps * 8, cudaMemcpyDeviceToHost, c->stream), "dh_adjoint: dt sequence");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_adjoint: synchronize");
+  for (int k = 0; k < nsteps; ++k) {
+    unsigned long long flag;
+    memcpy(&flag, c->adj_dts_host + nsteps + k, 8);
+    if (flag) return fail(DH_ERR_NONFINITE, "dh_adjoint: non-finite state in the forward sweep%s");
+    if (dts_out) dts_out[k] = c->adj_dts_host[k];
+  }
+  // ---- reverse sweep, segment by segment: recompute the states before each step of the segment, then pull the
+  //      cotangent back through the steps in reverse order
+  void* g = gU;
+  void* gn = gtmp;
+  for (int ic = nck - 1; ic >= 0; --ic) {
+    const int k0 = ic * every, len = (nsteps - k0 < every) ? nsteps - k0 : every;
+    DH_CUDA(cudaMemcpyAsync(seg(0), ckpt(ic), sb, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: segment start");
+    for (int j = 1; j < len; ++j) {
+      DH_CUDA(cudaMemcpyAsync(seg(j), seg(j - 1), sb, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: segment copy");
+      int rc = dh_step(c, seg(j), c->adj_dts_host[k0 + j - 1]);
+      if (rc) return rc;
+    }
+    for (int j = len - 1; j >= 0; --j) {
+      int rc = dh_step_vjp(c, seg(j), c->adj_dts_host[k0 + j], g, gn);
+      if (rc) return rc;
+      void* t = g; g = gn; gn = t;
+    }
+  }
+  if (g != gU) DH_CUDA(cudaMemcpyAsync(gU, g, sb, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: result copy");
   return DH_OK;
 }
 

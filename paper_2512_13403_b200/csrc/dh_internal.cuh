@@ -104,6 +104,11 @@ struct Ctx {
   void* rev_scratch;           // 20 words per cell of a z slab (+2 planes), fused reverse stages
   int rev_slab;                // planes per slab the scratch was sized for
   int rev_slab_opt;            // DH_OPT_REV_SLAB (0 = automatic)
+  void* adj_states;            // dh_adjoint: checkpoints, one segment of states, one cotangent
+  size_t adj_count;            // states allocated there
+  double* adj_dts_dev;         // dh_adjoint: dt sequence (device, T widened by the CFL epilogue)
+  double* adj_dts_host;        // pinned mirror
+  int adj_dts_cap;
   unsigned long long* acc;     // device accumulators of the CFL reduction
   void* dt_dev;                // device dt (T)
   CflResult* result_dev;

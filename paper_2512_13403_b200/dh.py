@@ -28,7 +28,7 @@ KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
-    "dh_advance", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
+    "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
 ]
 KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp"]
 
@@ -65,6 +65,7 @@ def load(rebuild: bool = False):
     lib.dh_step_vjp.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_run_host.argtypes = [vp, vp, ci, pd]
     lib.dh_advance.argtypes = [vp, vp, ci, pd]
+    lib.dh_adjoint.argtypes = [vp, vp, vp, ci, ci, pd]
     lib.dh_step_vjp_host.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_launch_count.restype = ctypes.c_ulonglong
     lib.dh_launch_count.argtypes = [vp]
@@ -73,7 +74,7 @@ def load(rebuild: bool = False):
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
-               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_advance", "dh_step_vjp_host", "dh_profile_enable",
+               "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_advance", "dh_adjoint", "dh_step_vjp_host", "dh_profile_enable",
                "dh_profile_read"):
         getattr(lib, fn).restype = ci
     _lib = lib
@@ -161,6 +162,13 @@ def dh_advance(ctx, U_ptr: int, nsteps: int, sync: bool = True):
     return None
 
 
+def dh_adjoint(ctx, U_ptr: int, gU_ptr: int, nsteps: int, every: int) -> list:
+    """Adjoint of nsteps steps with checkpoints every `every` steps; returns the dt sequence."""
+    dts = (ctypes.c_double * max(nsteps, 1))()
+    _check(load().dh_adjoint(ctx, ctypes.c_void_p(U_ptr), ctypes.c_void_p(gU_ptr), int(nsteps), int(every), dts))
+    return [dts[i] for i in range(nsteps)]
+
+
 def dh_run_host(ctx, U_host_ptr: int, nsteps: int) -> float:
     out = ctypes.c_double()
     _check(load().dh_run_host(ctx, ctypes.c_void_p(U_host_ptr), int(nsteps), ctypes.byref(out)))
@@ -241,6 +249,10 @@ class Solver:
 
     def advance(self, U, nsteps: int, sync: bool = True):
         return dh_advance(self.ctx, self._dev(U, "U"), nsteps, sync)
+
+    def adjoint(self, U, gU, nsteps: int, every: int) -> list:
+        """U: U_0 -> U_n in place; gU: dL/dU_n -> dL/dU_0 in place; returns the dt sequence."""
+        return dh_adjoint(self.ctx, self._dev(U, "U"), self._dev(gU, "gU"), nsteps, every)
 
     def step_devdt(self, U) -> None:
         dh_step_devdt(self.ctx, self._dev(U, "U"))

@@ -582,3 +582,44 @@ def test_step_and_vjp_are_bitwise_reproducible(dtype):
         grads.append(s.step_vjp(U, dt, g).clone())
     assert torch.equal(outs[0], outs[1]) and torch.equal(outs[0], outs[2])
     assert torch.equal(grads[0], grads[1]) and torch.equal(grads[0], grads[2])
+
+
+# ------------------------------------------------------------------ multi-step adjoint
+@pytest.mark.parametrize("every", [1, 2, 5, 7])
+def test_adjoint_checkpointed_fp64_matches_oracle_composition(every):
+    """dh_adjoint (sparse checkpoints + recomputed segments) against the oracle's plain composition of step_vjp,
+    5 steps on a ragged fp64 grid: first dt bit-identical (the later ones to 1e-13: their inputs differ by rounding),
+    final state and gradient pointwise."""
+    U = random_state((9, 10, 70), 301, 5 / 3, torch.float64)
+    p = oracle_params(U, 5 / 3)
+    g = np.random.default_rng(302).normal(size=tuple(U.shape))
+    Un_ref, g0_ref, dts_ref = oracle.adjoint(U.numpy(), 5, g, p)
+    s = _solver(U, 5 / 3)
+    Ud, gd = U.cuda(), torch.from_numpy(g).cuda()
+    dts = s.adjoint(Ud, gd, 5, every)
+    assert dts[0] == dts_ref[0]                           # identical input: bit-identical; later states differ by rounding
+    assert np.allclose(dts, dts_ref, rtol=1e-13, atol=0)
+    assert max_rel_err(Ud.cpu().numpy(), Un_ref) <= 5e-12
+    err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
+    assert err.max() <= 1e-11, float(err.max())
+
+
+def test_adjoint_is_bitwise_the_manual_loop_fp32():
+    """Checkpointing must not change a bit: dh_adjoint equals cfl_dt + step forward and step_vjp backward done by
+    hand with every state kept (fp32, cooling on, several tiles)."""
+    U0 = random_state((12, 20, 132), 303, 5 / 3, torch.float32).cuda()
+    s = _solver(U0, 5 / 3, cooling=1, lambda0=0.3)
+    g = torch.randn_like(U0)
+    states, dts = [U0.clone()], []
+    for _ in range(6):
+        dts.append(s.cfl_dt(states[-1]))
+        nxt = states[-1].clone()
+        s.step(nxt, dts[-1])
+        states.append(nxt)
+    gm = g.clone()
+    for k in range(5, -1, -1):
+        gm = s.step_vjp(states[k], dts[k], gm).clone()
+    Ua, ga = U0.clone(), g.clone()
+    assert s.adjoint(Ua, ga, 6, 4) == dts
+    assert torch.equal(Ua, states[-1])
+    assert torch.equal(ga, gm)

@@ -160,3 +160,32 @@ def test_stage_vjp_matches_dense_jacobian_on_tiny_grid():
         dD = (oracle.flux_divergence(U + e, p) - oracle.flux_divergence(U - e, p)) / (2 * eps)
         flat[m] = -tau * float((g * dD).sum())
     assert np.abs(got - want).max() <= 5e-8 * max(1.0, np.abs(want).max())
+
+
+def test_multistep_adjoint_against_finite_differences():
+    """oracle.adjoint (composition of step_vjp with the dt sequence frozen) against central finite
+    differences of L(U_0) = <g, H_dt3(H_dt2(H_dt1(U_0)))> along random directions, 6^3 fp64."""
+    rng = np.random.default_rng(77)
+    shape = (6, 6, 6)
+    rho = rng.uniform(0.8, 1.5, shape)
+    v = rng.normal(0, 0.3, (3,) + shape)
+    P = rng.uniform(0.8, 1.5, shape)
+    gamma = 1.4
+    U0 = np.stack([rho, rho * v[0], rho * v[1], rho * v[2], P / (gamma - 1) + 0.5 * rho * (v ** 2).sum(0)])
+    p = oracle.params(gamma=gamma, shape=U0.shape)
+    g = rng.normal(size=U0.shape)
+    Un, g0, dts = oracle.adjoint(U0, 3, g, p)
+    assert len(dts) == 3 and all(d > 0 for d in dts)
+
+    def run(U):
+        for d in dts:                                      # dt sequence held constant
+            U = oracle.step(U, d, p)
+        return U
+
+    assert np.array_equal(run(U0), Un)
+    for _ in range(3):
+        w = rng.normal(size=U0.shape)
+        eps = 1e-6
+        fd = float(((run(U0 + eps * w) - run(U0 - eps * w)) * g).sum() / (2 * eps))
+        an = float((g0 * w).sum())
+        assert abs(fd - an) <= 2e-6 * max(abs(fd), abs(an), 1e-3), (fd, an)
