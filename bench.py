@@ -328,6 +328,21 @@ def run_dh(a):
                 "step_GB/s": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9,
                 "step_frac": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9 / peak}
 
+    # the same kernel against its dispatch (operand-read) bound: modelled dispatch cycles per launch from the
+    # committed capture (profiles/r01f_dispatch_model.md) / (schedulers x SM clock x measured launch time)
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            disp = json.load(f).get(f"dispatch_cycles_{n}")
+    except Exception:
+        disp = None
+    if disp is not None:
+        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+        mhz = (clocks or {}).get("sm_mhz") or 1965.0
+        peak_disp = 4 * sm_count * mhz * 1e6                       # dispatch cycles per second, all schedulers
+        ach = disp / (st_ms / max(st_cnt, 1) * 1e-3)
+        roofline["alu"] = {"bound": "alu", "what": "dispatch (register operand read) cycles of the stage kernel",
+                           "achieved": ach, "peak": peak_disp, "unit": "dispatch cycles/s", "frac": ach / peak_disp,
+                           "peak_source": f"4 schedulers x {sm_count} SMs x {mhz:.0f} MHz (sampled clock)"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
