@@ -59,6 +59,10 @@ template <class T> DH_DI void cp_async_pack2(T* smem_dst, const T* gmem_src) {
   if (sizeof(T) == 4) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
   else asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+template <class T> DH_DI void cp_async_quad2(T* smem_dst, const T* gmem_src) {   // 4 x fp32: 16 bytes
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
 DH_DI void cp_async_commit2() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N> DH_DI void cp_async_wait2() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
@@ -73,7 +77,7 @@ DH_DI void recon_x2(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
 
 }  // namespace
 
-template <class T, int LIM, int NRW>
+template <class T, int LIM, int NRW, bool V16>
 __global__ void __launch_bounds__((NRW + 1) * 32, 1)
 stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   using G = Geo2<NRW>;
@@ -116,10 +120,21 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
     P2<T> WA[5], dA[5], LzA[5], accA[5], WB[5], dB[5], LzB[5], accB[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) WA[f] = dA[f] = LzA[f] = accA[f] = WB[f] = dB[f] = LzB[f] = accB[f] = bc2(T(0));
+    // V16 (fp32, nx % 4 == 0): a lane pair shares the staging work: the even lane copies the 4 cells of row A that the
+    // pair owns, the odd lane those of row B, as ONE 16-byte cp.async each (half the LDGSTS count; a __syncwarp
+    // makes the partner's copy visible)
+    const int q4 = 4 * (lane >> 1);
+    const size_t oQ = (size_t)wrapm2(y0 + jA + (lane & 1), ny) * nx + wrapm2(x0 + q4, nx);
+    const int stQ = (jA + (lane & 1)) * TX2 + q4;
+    if (V16) {
 #pragma unroll
-    for (int f = 0; f < 5; ++f) {
-      cp_async_pack2(Ust + f * FS + stA, p.U + f * N + op + oA);
-      cp_async_pack2(Ust + f * FS + stB, p.U + f * N + op + oB);
+      for (int f = 0; f < 5; ++f) cp_async_quad2(Ust + f * FS + stQ, p.U + f * N + op + oQ);
+    } else {
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        cp_async_pack2(Ust + f * FS + stA, p.U + f * N + op + oA);
+        cp_async_pack2(Ust + f * FS + stB, p.U + f * N + op + oB);
+      }
     }
     cp_async_commit2();
 
@@ -129,6 +144,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       T* const Wp_s = Wsm + bp * G::PLANE;
       const T* const Wq_s = Wsm + bq * G::PLANE;
       cp_async_wait2<0>();
+      if (V16) __syncwarp();
       P2<T> NA[5], NB[5];                          // plane p: raw, then primitive
 #pragma unroll
       for (int f = 0; f < 5; ++f) { NA[f] = lds2_(Ust + f * FS + stA); NB[f] = lds2_(Ust + f * FS + stB); }
@@ -136,12 +152,21 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       int pzn = pz + 1;
       size_t opn = op + NP;
       if (pzn == nz) { pzn = 0; opn = 0; }
+      if (V16) {
+        __syncwarp();                              // the partner has read its half of the slots written below
 #pragma unroll
-      for (int f = 0; f < 5; ++f) {
-        cp_async_pack2(Ust + f * FS + stA, p.U + f * N + opn + oA);
-        cp_async_pack2(Ust + f * FS + stB, p.U + f * N + opn + oB);
-        cp_async_pack2(Bst + bp * G::STAGE + f * FS + stA, p.B + f * N + op + oA);
-        cp_async_pack2(Bst + bp * G::STAGE + f * FS + stB, p.B + f * N + op + oB);
+        for (int f = 0; f < 5; ++f) {
+          cp_async_quad2(Ust + f * FS + stQ, p.U + f * N + opn + oQ);
+          cp_async_quad2(Bst + bp * G::STAGE + f * FS + stQ, p.B + f * N + op + oQ);
+        }
+      } else {
+#pragma unroll
+        for (int f = 0; f < 5; ++f) {
+          cp_async_pack2(Ust + f * FS + stA, p.U + f * N + opn + oA);
+          cp_async_pack2(Ust + f * FS + stB, p.U + f * N + opn + oB);
+          cp_async_pack2(Bst + bp * G::STAGE + f * FS + stA, p.B + f * N + op + oA);
+          cp_async_pack2(Bst + bp * G::STAGE + f * FS + stB, p.B + f * N + op + oB);
+        }
       }
       cp_async_commit2();
       {
@@ -371,13 +396,13 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
 
 namespace {
 
-template <class T, int LIM, int NRW>
+template <class T, int LIM, int NRW, bool V16>
 cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   using G = Geo2<NRW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
   static bool configured = false;     // per instantiation; the attribute is per function and sticks
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, NRW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, NRW, V16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
@@ -386,7 +411,7 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   // pick the chunk count that minimises waves x (planes per chunk + 4)
   int dev = 0, per_sm = 1;
   cudaGetDevice(&dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, NRW>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, NRW, V16>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
   const long long slots = (long long)per_sm * sm_count, tiles = (long long)bx * by;
   int bz = 1;
   long long best = -1;
@@ -398,7 +423,7 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   }
   const int ZL = (p.nz + bz - 1) / bz;
   dim3 grid(bx, by, bz), block((NRW + 1) * 32);
-  stage_fused2_kernel<T, LIM, NRW><<<grid, block, smem, s>>>(p, ZL);
+  stage_fused2_kernel<T, LIM, NRW, V16><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
 }
 
@@ -412,10 +437,17 @@ cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int sm_cou
   // fp32: 7 row warps + helper, one block per SM with the full register file (the kernel is bound by issue and
   // register pressure, not occupancy: profiles/r01c); fp64 (parity only): 3 row warps so that shared memory fits
   constexpr int NRW = sizeof(T) == 4 ? 7 : 3;
+  if (sizeof(T) == 4 && p.nx % 4 == 0) {             // 16-byte staging copies
+    switch (limiter) {
+      case 1: return launch_one2<T, 1, NRW, true>(p, sm_count, s);
+      case 2: return launch_one2<T, 2, NRW, true>(p, sm_count, s);
+      default: return launch_one2<T, 0, NRW, true>(p, sm_count, s);
+    }
+  }
   switch (limiter) {
-    case 1: return launch_one2<T, 1, NRW>(p, sm_count, s);
-    case 2: return launch_one2<T, 2, NRW>(p, sm_count, s);
-    default: return launch_one2<T, 0, NRW>(p, sm_count, s);
+    case 1: return launch_one2<T, 1, NRW, false>(p, sm_count, s);
+    case 2: return launch_one2<T, 2, NRW, false>(p, sm_count, s);
+    default: return launch_one2<T, 0, NRW, false>(p, sm_count, s);
   }
 }
 
