@@ -69,7 +69,7 @@ enum {
                             2: the first fused z-sweep kernel (one pack per thread), kept for comparison */
   DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
   DH_OPT_REV_SLAB = 12,  /* planes per z slab of the fused reverse stages' scratch (20 words per cell of a slab);
-                            0 (default): as many as fit in min(12 GiB, half of the free device memory) */
+                            0 (default): as many as fit in min(32 GiB, half of the free device memory) */
   DH_OPT_COUNT_
 };
 

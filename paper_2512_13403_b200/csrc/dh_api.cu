@@ -334,7 +334,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
     if (planes == 0) {
       size_t free_b = 0, total_b = 0;
       if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)8 << 30; }
-      size_t budget = (size_t)12 << 30;
+      size_t budget = (size_t)32 << 30;
       if (budget > free_b / 2) budget = free_b / 2;
       planes = (long long)(budget / per_plane) - 2;
       if (planes > c->nz) planes = c->nz;
