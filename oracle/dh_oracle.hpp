@@ -33,7 +33,7 @@ struct Params {
   double p_floor;
   int limiter;        // 0 minmod (A4), 1 van Leer, 2 MC, 3 piecewise-constant
   int riemann;        // 0 HLLC, 1 HLL, 2 Rusanov/LF
-  int integrator;     // 0 predictor/corrector A6-A7, 1 Heun
+  int integrator;     // 0 predictor/corrector A6-A7, 1 Heun, 2 SSPRK3
   int cooling;        // 0 off, 1 on: Eq. 23 with N_sub=1, reading A9
   double lambda0;     // Lambda(T) = lambda0 * T^alpha (reading A10)
   double alpha;
@@ -311,6 +311,8 @@ void apply_cooling(const Grid& g, const Params& p, double dt, S* U) {
 // integrator 0 (default, reading A1/A2): U* = U^n - dt/2 D(U^n);  U^{n+1} = U^n - dt D(U*)
 //                                        (Eqs. A6-A7 form, applied unsplit, Eq. A4)
 // integrator 1: Heun RK2: U1 = U^n - dt D(U^n);  U^{n+1} = (U^n + U1 - dt D(U1)) / 2
+// integrator 2: SSPRK3 (the paper names the scheme, the stages are the Shu-Osher form):
+//               U1 = U^n - dt D(U^n);  U2 = 3/4 U^n + 1/4 (U1 - dt D(U1));  U^{n+1} = 1/3 U^n + 2/3 (U2 - dt D(U2))
 // then cooling once (reading A8).
 // ------------------------------------------------------------------------------------------------
 template <class S>
@@ -322,10 +324,17 @@ void step(const Grid& g, const Params& p, const S* U, double dt, S* Uout) {
     for (size_t c = 0; c < M; ++c) Us[c] = U[c] - (0.5 * dt) * D[c];
     flux_divergence(g, p, Us.data(), D.data());
     for (size_t c = 0; c < M; ++c) Uout[c] = U[c] - dt * D[c];
-  } else {
+  } else if (p.integrator == 1) {
     for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];
     flux_divergence(g, p, Us.data(), D.data());
     for (size_t c = 0; c < M; ++c) Uout[c] = 0.5 * (U[c] + (Us[c] - dt * D[c]));
+  } else {
+    std::vector<S> U2(M);
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];
+    flux_divergence(g, p, Us.data(), D.data());
+    for (size_t c = 0; c < M; ++c) U2[c] = 0.75 * U[c] + 0.25 * (Us[c] - dt * D[c]);
+    flux_divergence(g, p, U2.data(), D.data());
+    for (size_t c = 0; c < M; ++c) Uout[c] = (1.0 / 3.0) * U[c] + (2.0 / 3.0) * (U2[c] - dt * D[c]);
   }
   if (p.cooling) apply_cooling(g, p, dt, Uout);
 }
@@ -425,6 +434,27 @@ inline void step_vjp(const Grid& g, const Params& p, const double* U, double dt,
     // U* = U - dt/2 D(U):  Ubar += U*bar - dt/2 J_D(U)^T U*bar
     for (size_t c = 0; c < M; ++c) gin[c] = g1[c] + gs[c];
     stage_vjp_accumulate(g, p, U, 0.5 * dt, gs.data(), gin);
+  } else if (p.integrator == 2) {
+    // SSPRK3: Ua = U - dt D(U); Ub = 3/4 U + 1/4 (Ua - dt D(Ua)); U1 = 1/3 U + 2/3 (Ub - dt D(Ub))
+    std::vector<double> Ub(M), Da(M);
+    for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];
+    flux_divergence(g, p, Us.data(), Da.data());
+    for (size_t c = 0; c < M; ++c) Ub[c] = 0.75 * U[c] + 0.25 * (Us[c] - dt * Da[c]);
+    if (p.cooling) {
+      std::vector<double> U1(M);
+      flux_divergence(g, p, Ub.data(), D.data());
+      for (size_t c = 0; c < M; ++c) U1[c] = (1.0 / 3.0) * U[c] + (2.0 / 3.0) * (Ub[c] - dt * D[c]);
+      cooling_vjp(g, p, dt, U1.data(), gout, g1.data());
+    } else {
+      for (size_t c = 0; c < M; ++c) g1[c] = gout[c];
+    }
+    std::vector<double> a(M), b(M), gb(M), ga(M);
+    for (size_t c = 0; c < M; ++c) { a[c] = (2.0 / 3.0) * g1[c]; gb[c] = a[c]; }   // Ubbar = 2/3 g1 ...
+    stage_vjp_accumulate(g, p, Ub.data(), dt, a.data(), gb.data());                // ... - dt J_D(Ub)^T (2/3 g1)
+    for (size_t c = 0; c < M; ++c) { b[c] = 0.25 * gb[c]; ga[c] = b[c]; }          // Uabar = 1/4 Ubbar ...
+    stage_vjp_accumulate(g, p, Us.data(), dt, b.data(), ga.data());                // ... - dt J_D(Ua)^T (1/4 Ubbar)
+    for (size_t c = 0; c < M; ++c) gin[c] = (1.0 / 3.0) * g1[c] + 0.75 * gb[c] + ga[c];
+    stage_vjp_accumulate(g, p, U, dt, ga.data(), gin);                             // ... - dt J_D(U)^T Uabar
   } else {
     // Heun: Ua = U - dt D(U); U1 = (U + Ua - dt D(Ua)) / 2
     for (size_t c = 0; c < M; ++c) Us[c] = U[c] - dt * D[c];

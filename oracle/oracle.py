@@ -26,7 +26,7 @@ _lib = None
 
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2, "constant": 3}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}
-INTEGRATORS = {"vl2": 0, "heun": 1}
+INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}
 
 
 class _Params(ctypes.Structure):

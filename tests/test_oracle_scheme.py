@@ -86,7 +86,7 @@ def test_smooth_advected_wave_is_second_order():
     assert math.log2(errs[0] / errs[1]) > 1.5, errs
 
 
-@pytest.mark.parametrize("integrator", ["vl2", "heun"])
+@pytest.mark.parametrize("integrator", ["vl2", "heun", "ssprk3"])
 def test_uniform_state_is_preserved_bitwise(integrator):
     g = 5 / 3
     shape = (6, 5, 7)
@@ -161,6 +161,40 @@ def test_two_stage_form_matches_its_definition_with_numpy():
     U1 = U - dt * oracle.flux_divergence(U, ph)
     want = 0.5 * (U + U1 - dt * oracle.flux_divergence(U1, ph))
     assert np.allclose(oracle.step(U, dt, ph), want, rtol=0, atol=1e-15)
+    p3 = oracle.params(shape=U.shape, integrator="ssprk3")
+    U1 = U - dt * oracle.flux_divergence(U, p3)
+    U2 = 0.75 * U + 0.25 * (U1 - dt * oracle.flux_divergence(U1, p3))
+    want = U / 3 + (2 / 3) * (U2 - dt * oracle.flux_divergence(U2, p3))
+    assert np.allclose(oracle.step(U, dt, p3), want, rtol=0, atol=1e-15)
+
+
+@pytest.mark.parametrize("integrator,order", [("vl2", 2), ("heun", 2), ("ssprk3", 3)])
+def test_temporal_order_of_the_integrators(integrator, order):
+    """PAPER.md:843-845 ("second-order RK2 (Heun's method), third-order SSPRK3"): with the spatial operator frozen
+    (first-order reconstruction on a smooth supersonic flow, where D is a smooth function of U) the error of one step
+    against a finely sub-stepped solution falls as dt^(order+1): halving dt divides it by 2^(order+1).  A wrong stage
+    weight lowers the order and fails this."""
+    n, g = 8, 5 / 3
+    x = (np.arange(n) + 0.5) / n
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    rho = 1.0 + 0.1 * np.sin(2 * np.pi * X) * np.cos(2 * np.pi * Y)
+    v = [3.0 + 0.1 * np.sin(2 * np.pi * Z), 2.5 + 0.1 * np.cos(2 * np.pi * X), 2.8 + 0.1 * np.sin(2 * np.pi * Y)]
+    P = 0.6 + 0.05 * np.cos(2 * np.pi * (X + Z))
+    U = _cons(rho, v, P, g)
+    p = oracle.params(gamma=g, shape=U.shape, limiter="constant", integrator=integrator)
+    T = 0.2 * oracle.cfl_dt(U, p)[0]
+
+    def run(k):
+        V = U.copy()
+        for _ in range(k):
+            V = oracle.step(V, T / k, p)
+        return V
+
+    ref = run(64)
+    e1, e2 = np.abs(run(1) - ref).max(), np.abs(run(2) - ref).max()
+    # global error over the fixed interval T: e(dt) ~ dt^order
+    rate = math.log2(e1 / e2)
+    assert abs(rate - order) < 0.25, (e1, e2, rate)
 
 
 def test_flux_divergence_of_1d_profile_by_hand():

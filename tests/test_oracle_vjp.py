@@ -24,6 +24,8 @@ CASES = [
     dict(riemann="rusanov"),
     dict(integrator="heun"),
     dict(integrator="heun", cooling=True, lambda0=0.5),
+    dict(integrator="ssprk3"),
+    dict(integrator="ssprk3", cooling=True, lambda0=0.5),
 ]
 
 
@@ -45,7 +47,8 @@ def test_vjp_equals_transposed_dual_number_jvp(kw):
         assert abs(lhs - rhs) <= 1e-13 * (np.abs(g * Jv).sum() + np.abs(gin * v).sum())
 
 
-@pytest.mark.parametrize("kw", [dict(), dict(cooling=True, lambda0=0.5)], ids=["hydro", "cooling"])
+@pytest.mark.parametrize("kw", [dict(), dict(cooling=True, lambda0=0.5), dict(integrator="heun"), dict(integrator="ssprk3")],
+                         ids=["hydro", "cooling", "heun", "ssprk3"])
 def test_vjp_against_central_finite_differences(kw):
     """BASELINE requirement: 8^3 fp64, <g, (H(U+eps v) - H(U-eps v)) / 2 eps> vs <J^T g, v>.
     The scheme is piecewise smooth (limiter / HLLC / floor switches); eps is small enough that for these
@@ -86,7 +89,7 @@ def test_vjp_fd_single_components():
         assert abs(fd - gin[f, k, j, i]) <= 2e-7 * max(1.0, abs(fd)), (f, k, j, i, fd, gin[f, k, j, i])
 
 
-@pytest.mark.parametrize("integrator", ["vl2", "heun"])
+@pytest.mark.parametrize("integrator", ["vl2", "heun", "ssprk3"])
 def test_vjp_of_constant_cotangent_is_itself(integrator):
     """sum_i U_f is invariant under the step (no cooling) => J^T 1_f = 1_f exactly up to rounding."""
     shape = (6, 7, 8)
