@@ -38,7 +38,7 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/s per RK2 step (forward: CFL dt + predictor + corrector)"
 UNIT = "cell-updates/s"
 FWD_WORDS, VJP_WORDS = 25, 45          # algorithmic words per cell: SURVEY.md §8(d), DESIGN.md §"Kernels"
-STAGE_WORDS = {"stage1": 10, "stage2": 15, "rev2": 15, "rev1": 20, "cfl_reduce": 5}
+STAGE_WORDS = {"stage1": 10, "stage2": 15, "rev2": 15, "rev1": 20, "cfl_reduce": 5, "lincomb": 15}
 FALLBACK_HBM_GBS = 6650.0              # /opt/skills/guides/B200_PROFILING.md, used only without MEASURED_PEAKS.json
 
 
@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
     ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
+    ap.add_argument("--integrator", choices=["vl2", "heun", "ssprk3"], default="vl2",
+                    help="vl2 = the predictor / corrector of Eqs. A6-A7 (BASELINE's metric); heun, ssprk3: SURVEY 8(f) item 2")
     ap.add_argument("--adjoint", type=int, default=0, help="also time dh_adjoint over this many steps (checkpointed multi-step adjoint)")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -245,7 +247,9 @@ def run_dh(a):
     U_cpu_block = U[:, :m, :m, :m].contiguous().cpu().numpy() if (rank == 0 and world == 1 and not a.no_cpu) else None
 
     s = dh.Solver(n, n, n, gamma=wl.gamma, dtype=torch.float32, kernel=a.kernel, cooling=int(a.cooling),
-                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor)
+                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator)
+    # algorithmic words per cell of one step: CFL 5 + per stage (5 in [+ 5 base] + 5 out) + per combination 15
+    fwd_words = {"vl2": FWD_WORDS, "heun": 5 + 10 + 15 + 15, "ssprk3": 5 + 10 + 15 + 15 + 15 + 15}[a.integrator]
 
     def barrier():
         if world > 1:
@@ -325,8 +329,8 @@ def run_dh(a):
                 "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
                                    "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
                                for k, v in prof.items() if v[1] > 0},
-                "step_GB/s": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9,
-                "step_frac": FWD_WORDS * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9 / peak}
+                "step_GB/s": fwd_words * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9,
+                "step_frac": fwd_words * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9 / peak}
 
     # the same kernel against its dispatch (operand-read) bound: modelled dispatch cycles per launch from the
     # committed capture (profiles/r01f_dispatch_model.md) / (schedulers x SM clock x measured launch time)
@@ -347,7 +351,7 @@ def run_dh(a):
             "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
-                       "cfl": 0.4, "limiter": "minmod", "riemann": "hllc", "integrator": "rk2 predictor/corrector",
+                       "cfl": 0.4, "limiter": "minmod", "riemann": "hllc", "integrator": {"vl2": "rk2 predictor/corrector", "heun": "heun rk2", "ssprk3": "ssprk3"}[a.integrator],
                        "cooling": bool(a.cooling), "kernel": a.kernel,
                        "call": "dh_cfl_dt_async + dh_step_devdt per step" if a.no_chain else "dh_advance(U, K): K x (CFL reduce, dt epilogue, predictor, corrector)", "parallelism": f"replicas x{world}",
                        "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
@@ -371,11 +375,12 @@ def run_dh(a):
         ms_v = max_over_ranks(ms_v)
         if not bool(torch.isfinite(gin[:, :2]).all()):
             raise RuntimeError("non-finite VJP result")
+        vjp_words = {"vl2": VJP_WORDS, "heun": 10 + 15 + 10 + 20 + 20, "ssprk3": 10 + 15 + 15 + 15 + 10 + 20 + 10 + 20 + 15 + 20}[a.integrator]
         line["vjp"] = {"value": world * N * Kv / (ms_v * 1e-3), "unit": "cell-VJPs/s", "steps": Kv, "ms_per_step": ms_v / Kv,
                        "gpu_launches": launches_v,
-                       "roofline": {"bound": "hbm", "achieved": VJP_WORDS * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9, "peak": peak,
-                                    "unit": "GB/s", "frac": VJP_WORDS * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9 / peak,
-                                    "words_per_cell": VJP_WORDS,
+                       "roofline": {"bound": "hbm", "achieved": vjp_words * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9, "peak": peak,
+                                    "unit": "GB/s", "frac": vjp_words * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9 / peak,
+                                    "words_per_cell": vjp_words,
                                     "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
                                                        "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
                                                    for k, v in pv.items() if v[1] > 0}}}

@@ -70,6 +70,11 @@ enum {
   DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
   DH_OPT_REV_SLAB = 12,  /* planes per z slab of the fused reverse stages' scratch (20 words per cell of a slab);
                             0 (default): as many as fit in min(32 GiB, half of the free device memory) */
+  DH_OPT_INTEGRATOR = 13,/* 0 (default): the predictor / corrector of Eqs. A6-A7;
+                            1: Heun's RK2  U1 = U - dt D(U);  U' = 1/2 U + 1/2 (U1 - dt D(U1));
+                            2: SSPRK3  U1 = U - dt D(U);  U2 = 3/4 U + 1/4 (U1 - dt D(U1));
+                               U' = 1/3 U + 2/3 (U2 - dt D(U2)).  Same stage kernels; the convex combinations are
+                               formed by a streaming kernel (DH_K_LINCOMB); dh_step_vjp / dh_adjoint follow the option */
   DH_OPT_COUNT_
 };
 
@@ -160,7 +165,8 @@ enum {
   DH_K_REV2 = 4,         /* reverse corrector */
   DH_K_REV1 = 5,         /* reverse predictor */
   DH_K_COOL_VJP = 6,     /* pointwise cooling adjoint */
-  DH_K_COUNT_ = 7
+  DH_K_LINCOMB = 7,      /* out = a X + b Y: base states / scaled cotangents of Heun and SSPRK3 */
+  DH_K_COUNT_ = 8
 };
 int dh_profile_enable(dh_ctx* ctx, int on);
 int dh_profile_read(dh_ctx* ctx, double* ms_out, unsigned long long* launches_out);

@@ -115,7 +115,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->gamma = gamma;
   c->cfl = 0.4;
   c->L[0] = c->L[1] = c->L[2] = 1.0;
-  c->cooling = 0; c->kernel = 0; c->limiter = 0;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->integrator = 0;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
@@ -141,7 +141,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
+  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
@@ -174,6 +174,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0, 1 or 2%s"); c->kernel = (int)v; break;
     case DH_OPT_REV_SLAB: if (v < 0 || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: rev_slab must be a non-negative integer%s"); c->rev_slab_opt = (int)v; break;
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
+    case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
   return DH_OK;
@@ -193,6 +194,7 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_KERNEL: *out = c->kernel; break;
     case DH_OPT_LIMITER: *out = c->limiter; break;
     case DH_OPT_REV_SLAB: *out = c->rev_slab_opt; break;
+    case DH_OPT_INTEGRATOR: *out = c->integrator; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
   return DH_OK;
@@ -292,8 +294,49 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
   return DH_OK;
 }
 
+// out = a X + b Y over a whole state (Y may be NULL); the base states and scaled cotangents of Heun / SSPRK3
+template <class T>
+static int lincomb(dh_ctx* c, void* out, double a, const void* X, double b, const void* Y) {
+  ProfScope ps(c, DH_K_LINCOMB);
+  DH_CUDA(launch_lincomb<T>((T*)out, (T)a, (const T*)X, (T)b, (const T*)Y, 5 * c->N, c->sm_count, c->stream), "lincomb kernel launch");
+  c->launches += 1;
+  return DH_OK;
+}
+
+// The stage states of Heun / SSPRK3 up to (not including) the last stage: c->Us = U1, (SSPRK3) c->Uc = U2, and
+// c->Ub = the base state of the last stage.  *last_in = the state the last stage differentiates, *last_frac its weight.
+template <class T>
+static int rk_prefix(dh_ctx* c, const void* U, double dt, bool devdt, const void** last_in, double* last_frac) {
+  int rc = lazy_alloc(c, &c->Ub, state_bytes(c), "the base-state combination");
+  if (rc) return rc;
+  rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 1.0, false);              // U1 = U - dt D(U)
+  if (rc) return rc;
+  if (c->integrator == 1) {                                                                // Heun
+    rc = lincomb<T>(c, c->Ub, 0.5, U, 0.5, c->Us);
+    *last_in = c->Us; *last_frac = 0.5;
+    return rc;
+  }
+  rc = lazy_alloc(c, &c->Uc, state_bytes(c), "the second stage state");
+  if (rc) return rc;
+  rc = lincomb<T>(c, c->Ub, 0.75, U, 0.25, c->Us);
+  if (rc) return rc;
+  rc = stage_launch<T>(c, DH_K_STAGE1, c->Us, c->Ub, c->Uc, dt, devdt, 0.25, false);      // U2 = 3/4 U + 1/4 (U1 - dt D(U1))
+  if (rc) return rc;
+  rc = lincomb<T>(c, c->Ub, 1.0 / 3.0, U, 2.0 / 3.0, c->Uc);
+  *last_in = c->Uc; *last_frac = 2.0 / 3.0;
+  return rc;
+}
+
 template <class T>
 static int step_impl(dh_ctx* c, void* U, double dt, bool devdt) {
+  if (c->integrator != 0) {
+    // Heun / SSPRK3 in Shu-Osher form: every stage is  out = B - w dt D(state)
+    const void* last_in = nullptr;
+    double w = 0.0;
+    int rc = rk_prefix<T>(c, U, dt, devdt, &last_in, &w);
+    if (rc) return rc;
+    return stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, c->cooling != 0);
+  }
   // predictor: U* = U^n - dt/2 D(U^n)   (Eq. A6);  corrector, in place: U^{n+1} = U^n - dt D(U*)   (Eq. A7)
   int rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 0.5, false);
   if (rc) return rc;
@@ -376,8 +419,58 @@ static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const vo
   return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
 }
 
+// VJP of a Heun / SSPRK3 step.  With a = w g (w the last stage's weight) the last stage gives
+// Xbar = a - dt J_D(X)^T a for its input X, and so on down to U; the U-weights of the base states add w_U g terms.
+template <class T>
+static int vjp_rk(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
+  int rc = lazy_alloc(c, &c->gs, state_bytes(c), "the stage cotangent");
+  if (rc) return rc;
+  const void* last_in = nullptr;
+  double w = 0.0;
+  rc = rk_prefix<T>(c, U, dt, false, &last_in, &w);                // recompute the stage states (nothing was stored)
+  if (rc) return rc;
+  const void* g1 = gout;
+  if (c->cooling) {
+    rc = lazy_alloc(c, &c->U1, state_bytes(c), "the pre-cooling state");
+    if (rc) return rc;
+    rc = lazy_alloc(c, &c->g1, state_bytes(c), "the pre-cooling cotangent");
+    if (rc) return rc;
+    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, c->U1, dt, false, w, false);
+    if (rc) return rc;
+    ProfScope ps(c, DH_K_COOL_VJP);
+    DH_CUDA(launch_cool_vjp<T>((const T*)c->U1, (const T*)gout, (T*)c->g1, c->N, (T)dt, make_consts<T>(c), c->stream),
+            "dh_step_vjp: cooling reverse kernel launch");
+    c->launches += 1;
+    g1 = c->g1;
+  }
+  void* const h = c->Ub;                                           // the base state is dead: scaled cotangents live there
+  if (c->integrator == 1) {
+    // Heun: U' = 1/2 U + 1/2 (U1 - dt D(U1)), U1 = U - dt D(U)
+    rc = lincomb<T>(c, h, 0.5, g1, 0.0, nullptr);
+    if (rc) return rc;
+    rc = rev_stage<T>(c, DH_K_REV2, c->Us, g1, h, nullptr, c->gs, dt, 0.5);          // U1bar = h - dt/2 J_D(U1)^T g1
+    if (rc) return rc;
+    return rev_stage<T>(c, DH_K_REV1, U, c->gs, h, c->gs, gin, dt, 1.0);             // Ubar = h + U1bar - dt J_D(U)^T U1bar
+  }
+  // SSPRK3: U' = 1/3 U + 2/3 (U2 - dt D(U2)), U2 = 3/4 U + 1/4 (U1 - dt D(U1)), U1 = U - dt D(U)
+  rc = lazy_alloc(c, &c->ga, state_bytes(c), "the first stage cotangent");
+  if (rc) return rc;
+  rc = lincomb<T>(c, h, 2.0 / 3.0, g1, 0.0, nullptr);
+  if (rc) return rc;
+  rc = rev_stage<T>(c, DH_K_REV2, c->Uc, g1, h, nullptr, c->gs, dt, 2.0 / 3.0);      // U2bar = 2/3 g1 - 2/3 dt J_D(U2)^T g1
+  if (rc) return rc;
+  rc = lincomb<T>(c, h, 0.25, c->gs, 0.0, nullptr);
+  if (rc) return rc;
+  rc = rev_stage<T>(c, DH_K_REV1, c->Us, c->gs, h, nullptr, c->ga, dt, 0.25);        // U1bar = 1/4 U2bar - 1/4 dt J_D(U1)^T U2bar
+  if (rc) return rc;
+  rc = lincomb<T>(c, h, 1.0 / 3.0, g1, 0.75, c->gs);
+  if (rc) return rc;
+  return rev_stage<T>(c, DH_K_REV1, U, c->ga, h, c->ga, gin, dt, 1.0);               // Ubar = 1/3 g1 + 3/4 U2bar + U1bar - dt J_D(U)^T U1bar
+}
+
 template <class T>
 static int vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
+  if (c->integrator != 0) return vjp_rk<T>(c, U, dt, gout, gin);
   int rc = lazy_alloc(c, &c->gs, state_bytes(c), "the U* cotangent state");
   if (rc) return rc;
   // recompute U* = U^n - dt/2 D(U^n)  (nothing was stored by dh_step)

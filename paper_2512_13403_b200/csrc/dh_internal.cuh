@@ -90,12 +90,15 @@ struct Ctx {
   int nx, ny, nz, dtype;
   size_t N;
   double gamma, cfl, L[3];
-  int cooling, kernel, limiter;
+  int cooling, kernel, limiter, integrator;
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
   int sm_count;
   void* Us;                    // U* scratch (always)
   void* gs;                    // cotangent of U* (first VJP)
+  void* Ub;                    // base-state combination (Heun / SSPRK3); reused as the scaled cotangent in their VJP
+  void* Uc;                    // second stage state of SSPRK3
+  void* ga;                    // cotangent of the first stage state (SSPRK3 VJP)
   void* U1;                    // pre-cooling state, cooling VJP only
   void* g1;                    // cotangent of U1, cooling VJP only
   void* Uhost_dev;             // device state for the HOST entry points
@@ -135,6 +138,7 @@ template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limit
 template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
+template <class T> cudaError_t launch_lincomb(T* out, T a, const T* X, T b, const T* Y, size_t n, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s);
 

@@ -19,9 +19,10 @@ DH_F32, DH_F64 = 0, 1
 DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, -4
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
-    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12,
+    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
+INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
 KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 
 # every symbol include/dh.h declares (checked by tests/test_abi.py)
@@ -30,7 +31,7 @@ SYMBOLS = [
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
 ]
-KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp"]
+KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb"]
 
 _lib = None
 
@@ -218,6 +219,8 @@ class Solver:
         for k, v in options.items():
             if k == "limiter" and isinstance(v, str):
                 v = LIMITERS[v]
+            if k == "integrator" and isinstance(v, str):
+                v = INTEGRATORS[v]
             if k == "kernel" and isinstance(v, str):
                 v = KERNELS[v]
             dh_set_option(self.ctx, OPTIONS[k], float(v))

@@ -623,3 +623,55 @@ def test_adjoint_is_bitwise_the_manual_loop_fp32():
     assert s.adjoint(Ua, ga, 6, 4) == dts
     assert torch.equal(Ua, states[-1])
     assert torch.equal(ga, gm)
+
+
+# ------------------------------------------------------------------ Heun / SSPRK3
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("cooling", [0, 1])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("integrator", ["heun", "ssprk3"])
+def test_step_parity_other_integrators(integrator, dtype, cooling, kernel):
+    """One step of Heun's RK2 / SSPRK3 (same stage kernels, convex combinations by the lincomb kernel) against the
+    oracle on a grid with several ragged tiles; dt bit-identical, state to the step tolerance."""
+    gamma = 5 / 3
+    U = random_state((13, 17, 132), 410, gamma, dtype)
+    okw = dict(integrator=integrator, **(dict(cooling=True, lambda0=0.5) if cooling else {}))
+    skw = dict(integrator=integrator, kernel=kernel, **(dict(cooling=1, lambda0=0.5) if cooling else {}))
+    p = oracle_params(U, gamma, **okw)
+    s = _solver(U, gamma, **skw)
+    Ud = U.cuda()
+    dt = s.cfl_dt(Ud)
+    assert dt == oracle.cfl_dt(U.numpy(), p)[0]
+    s.step(Ud, dt)
+    err = max_rel_err(Ud.cpu().numpy(), oracle.step(U.numpy(), dt, p))
+    assert err <= TOL[dtype], err
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("cooling", [0, 1])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("integrator", ["heun", "ssprk3"])
+def test_vjp_parity_other_integrators(integrator, dtype, cooling, kernel):
+    U = random_state((9, 17, 70), 411, 5 / 3, dtype)
+    okw = dict(integrator=integrator, **(dict(cooling=True, lambda0=0.5) if cooling else {}))
+    skw = dict(integrator=integrator, kernel=kernel, **(dict(cooling=1, lambda0=0.5) if cooling else {}))
+    _vjp_case(U, 5 / 3, 12, dtype, okw, skw, 1e-12 if dtype == torch.float64 else 1e-4)
+
+
+@pytest.mark.parametrize("integrator", ["heun", "ssprk3"])
+def test_advance_and_adjoint_follow_the_integrator_option(integrator):
+    """dh_advance / dh_adjoint with Heun / SSPRK3: 4 steps fp64 against the oracle's loop and its composed adjoint."""
+    U = random_state((9, 10, 70), 412, 5 / 3, torch.float64)
+    p = oracle_params(U, 5 / 3, integrator=integrator)
+    g = np.random.default_rng(413).normal(size=tuple(U.shape))
+    Un_ref, g0_ref, dts_ref = oracle.adjoint(U.numpy(), 4, g, p)
+    s = _solver(U, 5 / 3, integrator=integrator)
+    Ua = U.cuda()
+    s.advance(Ua, 4)
+    assert max_rel_err(Ua.cpu().numpy(), Un_ref) <= 5e-12
+    Ud, gd = U.cuda(), torch.from_numpy(g).cuda()
+    dts = s.adjoint(Ud, gd, 4, 3)
+    assert dts[0] == dts_ref[0] and np.allclose(dts, dts_ref, rtol=1e-13, atol=0)
+    assert torch.equal(Ud, Ua)
+    err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
+    assert err.max() <= 1e-11, float(err.max())
