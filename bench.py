@@ -359,6 +359,7 @@ def run_dh(a):
                        "dt_last": dt_last},
             "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
     s.profile(False)
+    line["config"]["cfl_candidate_path"] = s.cfl_stats()      # dh_advance: dt's from candidate lists / fallbacks / packs
 
     # ---- VJP of the step, same state, seeded Gaussian cotangent on all five fields (configs[4])
     if not a.no_vjp:

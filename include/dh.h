@@ -75,6 +75,10 @@ enum {
                             2: SSPRK3  U1 = U - dt D(U);  U2 = 3/4 U + 1/4 (U1 - dt D(U1));
                                U' = 1/3 U + 2/3 (U2 - dt D(U2)).  Same stage kernels; the convex combinations are
                                formed by a streaming kernel (DH_K_LINCOMB); dh_step_vjp / dh_adjoint follow the option */
+  DH_OPT_FUSE_CFL = 14,  /* 1 (default) / 0: inside dh_advance, from the second step on, the last stage of a step appends the
+                            packs of its result whose estimated wave speed reaches 0.97 x the previous maximum to a list,
+                            and the next dt comes from the exact recipe on that list (the full reduction runs only
+                            when the list cannot settle the maxima).  dt and the states are bit-identical either way */
   DH_OPT_COUNT_
 };
 
@@ -170,6 +174,12 @@ enum {
 };
 int dh_profile_enable(dh_ctx* ctx, int on);
 int dh_profile_read(dh_ctx* ctx, double* ms_out, unsigned long long* launches_out);
+
+/* Counters of the CFL candidate path of dh_advance (DH_OPT_FUSE_CFL) since dh_create, copied to the HOST array
+ * out[3] after a synchronize of the context's stream: out[0] = dt's taken from a candidate list, out[1] = of those,
+ * the ones that fell back to the full reduction (list overflow, or a maximum below the threshold), out[2] = packs
+ * evaluated with the exact recipe.  All zero before the first dh_advance of more than one step. */
+int dh_cfl_stats(dh_ctx* ctx, unsigned long long* out);
 
 /* Message describing the last error on the calling thread ("" if none). */
 const char* dh_last_error(void);

@@ -115,7 +115,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->gamma = gamma;
   c->cfl = 0.4;
   c->L[0] = c->L[1] = c->L[2] = 1.0;
-  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->integrator = 0;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->integrator = 0; c->fuse_cfl = 1;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
@@ -141,7 +141,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
+  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
@@ -175,6 +175,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_REV_SLAB: if (v < 0 || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: rev_slab must be a non-negative integer%s"); c->rev_slab_opt = (int)v; break;
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
+    case DH_OPT_FUSE_CFL: c->fuse_cfl = (v != 0.0); break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
   return DH_OK;
@@ -195,6 +196,7 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_LIMITER: *out = c->limiter; break;
     case DH_OPT_REV_SLAB: *out = c->rev_slab_opt; break;
     case DH_OPT_INTEGRATOR: *out = c->integrator; break;
+    case DH_OPT_FUSE_CFL: *out = c->fuse_cfl; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
   return DH_OK;
@@ -230,8 +232,10 @@ int dh_profile_read(dh_ctx* c, double* ms_out, unsigned long long* launches_out)
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------ CFL
+// cand: the state was written by a last stage that pushed its CFL candidates (dh_advance): exact recipe on those
+// packs, then the full reduction only if they do not settle the maxima
 template <class T>
-static int cfl_launch(dh_ctx* c, const void* U) {
+static int cfl_launch(dh_ctx* c, const void* U, bool cand = false) {
   CflParams<T> p;
   p.U = (const T*)U;
   p.N = c->N;
@@ -245,10 +249,16 @@ static int cfl_launch(dh_ctx* c, const void* U) {
   p.acc = c->acc;
   p.dt_dev = (T*)c->dt_dev;
   p.result = c->result_dev;
+  p.cand_list = c->cand_list; p.cand_cnt = c->cand_cnt; p.cand_thr = (T*)c->cand_thr; p.cand_cap = c->cand_cap; p.cand_stats = c->cand_stats;
   {
     ProfScope ps(c, DH_K_CFL_REDUCE);
-    DH_CUDA(launch_cfl_reduce<T>(p, c->sm_count, c->stream), "dh_cfl_dt: reduction kernel launch");
-    c->launches += 1;
+    if (cand) {
+      DH_CUDA(launch_cfl_candidates<T>(p, c->sm_count, c->stream), "dh_advance: CFL candidate kernel launch");
+      c->launches += 2;
+    } else {
+      DH_CUDA(launch_cfl_reduce<T>(p, c->sm_count, c->stream), "dh_cfl_dt: reduction kernel launch");
+      c->launches += 1;
+    }
   }
   {
     ProfScope ps(c, DH_K_CFL_FINISH);
@@ -260,7 +270,8 @@ static int cfl_launch(dh_ctx* c, const void* U) {
 
 // ------------------------------------------------------------------------------------------ forward
 template <class T>
-static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool) {
+static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool,
+                        bool cand = false) {
   StageParams<T> p;
   p.U = (const T*)U; p.B = (const T*)B; p.out = (T*)out;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
@@ -271,6 +282,11 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
   p.frac = (T)frac;
   p.cool = cool ? 1 : 0;
   p.c = make_consts<T>(c);
+  p.cand_list = nullptr; p.cand_cnt = nullptr; p.cand_thr = nullptr; p.cand_cap = 0;
+  if (cand && c->kernel == 0 && c->cand_list && c->N < ((size_t)1 << 32)) {
+    p.cand_list = c->cand_list; p.cand_cnt = c->cand_cnt; p.cand_thr = (const T*)c->cand_thr; p.cand_cap = c->cand_cap;
+  }
+  c->cand_ok = 0;
   ProfScope ps(c, kind);
   bool done = false;
   if (c->kernel == 0) {
@@ -279,6 +295,7 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
     if (supported) {
       if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
       done = true;
+      c->cand_ok = p.cand_list != nullptr;      // only this kernel pushes candidates
     }
   }
   if (!done && c->kernel != 1) {
@@ -328,19 +345,19 @@ static int rk_prefix(dh_ctx* c, const void* U, double dt, bool devdt, const void
 }
 
 template <class T>
-static int step_impl(dh_ctx* c, void* U, double dt, bool devdt) {
+static int step_impl(dh_ctx* c, void* U, double dt, bool devdt, bool cand = false) {
   if (c->integrator != 0) {
     // Heun / SSPRK3 in Shu-Osher form: every stage is  out = B - w dt D(state)
     const void* last_in = nullptr;
     double w = 0.0;
     int rc = rk_prefix<T>(c, U, dt, devdt, &last_in, &w);
     if (rc) return rc;
-    return stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, c->cooling != 0);
+    return stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, c->cooling != 0, cand);
   }
   // predictor: U* = U^n - dt/2 D(U^n)   (Eq. A6);  corrector, in place: U^{n+1} = U^n - dt D(U*)   (Eq. A7)
   int rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 0.5, false);
   if (rc) return rc;
-  return stage_launch<T>(c, DH_K_STAGE2, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0);
+  return stage_launch<T>(c, DH_K_STAGE2, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0, cand);
 }
 
 // ------------------------------------------------------------------------------------------ reverse
@@ -544,13 +561,43 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
   if (!c || !U || nsteps < 0) return fail(DH_ERR_ARG, "dh_advance: bad argument%s");
   if (U == c->Us) return fail(DH_ERR_ARG, "dh_advance: U aliases library scratch%s");
   const bool f32 = c->dtype == DH_F32;
+  // From the second step on, the CFL pass runs on the candidates the previous last stage pushed (DH_OPT_FUSE_CFL)
+  const bool fuse = c->fuse_cfl && nsteps > 1 && c->kernel == 0;
+  if (fuse) {
+    if (!c->cand_list) {
+      c->cand_cap = 1u << 20;
+      int rc = lazy_alloc(c, (void**)&c->cand_list, (size_t)c->cand_cap * sizeof(unsigned), "the CFL candidate list");
+      if (rc) return rc;
+      rc = lazy_alloc(c, (void**)&c->cand_cnt, 2 * sizeof(unsigned), "the CFL candidate counters");
+      if (rc) return rc;
+      rc = lazy_alloc(c, &c->cand_thr, 16, "the CFL candidate thresholds");
+      if (rc) return rc;
+      rc = lazy_alloc(c, (void**)&c->cand_stats, 3 * sizeof(unsigned long long), "the CFL candidate counters");
+      if (rc) return rc;
+      DH_CUDA(cudaMemsetAsync(c->cand_stats, 0, 3 * sizeof(unsigned long long), c->stream), "dh_advance: reset of the candidate statistics");
+    }
+    DH_CUDA(cudaMemsetAsync(c->cand_cnt, 0, 2 * sizeof(unsigned), c->stream), "dh_advance: reset of the candidate counters");
+  }
+  c->cand_ok = 0;
   for (int s = 0; s < nsteps; ++s) {
-    int rc = f32 ? cfl_launch<float>(c, U) : cfl_launch<double>(c, U);
+    const bool use = fuse && s > 0 && c->cand_ok;
+    int rc = f32 ? cfl_launch<float>(c, U, use) : cfl_launch<double>(c, U, use);
     if (rc) return rc;
-    rc = f32 ? step_impl<float>(c, U, 0.0, true) : step_impl<double>(c, U, 0.0, true);
+    const bool push = fuse && s + 1 < nsteps;
+    rc = f32 ? step_impl<float>(c, U, 0.0, true, push) : step_impl<double>(c, U, 0.0, true, push);
     if (rc) return rc;
   }
+  c->cand_ok = 0;
   if (dt_last_out) return dh_poll_status(c, dt_last_out);
+  return DH_OK;
+}
+
+int dh_cfl_stats(dh_ctx* c, unsigned long long* out) {
+  if (!c || !out) return fail(DH_ERR_ARG, "dh_cfl_stats: NULL argument%s");
+  out[0] = out[1] = out[2] = 0ull;
+  if (!c->cand_stats) return DH_OK;
+  DH_CUDA(cudaMemcpyAsync(out, c->cand_stats, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream), "dh_cfl_stats: copy");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_cfl_stats: synchronize");
   return DH_OK;
 }
 

@@ -52,10 +52,11 @@ template <> struct Vec<float> { using type = float4; static constexpr int W = 4;
 template <> struct Vec<double> { using type = double2; static constexpr int W = 2; };
 
 template <class T>
-__global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p) {
+__global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, const bool guarded) {
   using V = typename Vec<T>::type;
   constexpr int W = Vec<T>::W;
   const size_t N = p.N;
+  if (guarded && p.cand_cnt[1] == 0u) return;      // the candidates already hold the maxima (cfl_cand_kernel)
   T sx = T(0), sy = T(0), sz = T(0);
   bool bad = false;
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
@@ -117,6 +118,63 @@ __global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p) {
   }
 }
 
+// Candidate path of dh_advance.  The last stage of the previous step appended every pack whose wave-speed ESTIMATE
+// (fast math, from the values it was about to store) reached 0.999 theta, theta = 0.97 min_a S_a of the previous dt.
+// This one-block kernel evaluates the exact dt recipe on those packs.  If the list did not overflow and the exact
+// maximum of every axis reaches theta, no other cell can exceed it (their speeds are below theta) and the maxima
+// are the global ones; otherwise the flag sends the guarded full reduction over the whole state.
+template <class T>
+__global__ void __launch_bounds__(1024) cfl_cand_kernel(const CflParams<T> p) {
+  const unsigned cnt = p.cand_cnt[0];
+  const unsigned n = cnt < p.cand_cap ? cnt : p.cand_cap;
+  const size_t N = p.N;
+  T sx = T(0), sy = T(0), sz = T(0);
+  bool bad = false;
+  for (unsigned i = threadIdx.x; i < n; i += blockDim.x) {
+    const size_t cidx = p.cand_list[i];
+#pragma unroll
+    for (int l = 0; l < 2; ++l)
+      cell_speeds<T>(p.U[cidx + l], p.U[N + cidx + l], p.U[2 * N + cidx + l], p.U[3 * N + cidx + l], p.U[4 * N + cidx + l], p, sx, sy, sz, bad);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    T ox = __shfl_xor_sync(0xffffffffu, sx, o), oy = __shfl_xor_sync(0xffffffffu, sy, o), oz = __shfl_xor_sync(0xffffffffu, sz, o);
+    sx = (ox > sx) ? ox : sx;
+    sy = (oy > sy) ? oy : sy;
+    sz = (oz > sz) ? oz : sz;
+  }
+  const unsigned anybad = __ballot_sync(0xffffffffu, bad);
+  __shared__ T sm[3][32];
+  __shared__ unsigned smbad[32];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  if (lane == 0) { sm[0][warp] = sx; sm[1][warp] = sy; sm[2][warp] = sz; smbad[warp] = anybad; }
+  __syncthreads();
+  if (warp == 0) {
+    sx = sm[0][lane]; sy = sm[1][lane]; sz = sm[2][lane];
+    unsigned b = smbad[lane];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      T ox = __shfl_xor_sync(0xffffffffu, sx, o), oy = __shfl_xor_sync(0xffffffffu, sy, o), oz = __shfl_xor_sync(0xffffffffu, sz, o);
+      sx = (ox > sx) ? ox : sx;
+      sy = (oy > sy) ? oy : sy;
+      sz = (oz > sz) ? oz : sz;
+      b |= __shfl_xor_sync(0xffffffffu, b, o);
+    }
+    if (lane == 0) {
+      atomicMax(p.acc + 0, bits_of(sx));
+      atomicMax(p.acc + 1, bits_of(sy));
+      atomicMax(p.acc + 2, bits_of(sz));
+      if (b) atomicOr(p.acc + 3, 1ull);
+      const T theta = p.cand_thr[1];
+      const bool need = cnt > p.cand_cap || !(sx >= theta && sy >= theta && sz >= theta);
+      p.cand_cnt[1] = need ? 1u : 0u;
+      p.cand_stats[0] += 1ull;                 // one block, one thread: plain updates
+      p.cand_stats[1] += need ? 1ull : 0ull;
+      p.cand_stats[2] += n;
+    }
+  }
+}
+
 template <class T>
 __global__ void cfl_finish_kernel(const CflParams<T> p) {
   T S[3];
@@ -130,6 +188,15 @@ __global__ void cfl_finish_kernel(const CflParams<T> p) {
   }
   const T dt = Ieee::mul(p.cfl, best);
   *p.dt_dev = dt;
+  if (p.cand_thr) {          // thresholds for the candidates the next last stage will push, and an empty list
+    T smin = S[0] < S[1] ? S[0] : S[1];
+    smin = smin < S[2] ? smin : S[2];
+    const T theta = T(0.97) * smin;
+    p.cand_thr[1] = theta;
+    p.cand_thr[0] = T(0.999) * theta;
+    p.cand_cnt[0] = 0u;
+    p.cand_cnt[1] = 0u;
+  }
   p.result->smax[0] = (double)S[0];
   p.result->smax[1] = (double)S[1];
   p.result->smax[2] = (double)S[2];
@@ -145,7 +212,22 @@ cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t 
   size_t cap = (size_t)sm_count * 8;     // 8 resident 256-thread blocks per SM
   int blocks = (int)(want < cap ? want : cap);
   if (blocks < 1) blocks = 1;
-  cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p);
+  cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p, false);
+  return cudaGetLastError();
+}
+
+template <class T>
+cudaError_t launch_cfl_candidates(const CflParams<T>& p, int sm_count, cudaStream_t s) {
+  cfl_cand_kernel<T><<<1, 1024, 0, s>>>(p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  constexpr int W = Vec<T>::W;
+  size_t work = (p.N % W == 0) ? p.N / W : p.N;
+  size_t want = (work + 255) / 256;
+  size_t cap = (size_t)sm_count * 8;
+  int blocks = (int)(want < cap ? want : cap);
+  if (blocks < 1) blocks = 1;
+  cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p, true);
   return cudaGetLastError();
 }
 
@@ -157,6 +239,8 @@ cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s) {
 
 template cudaError_t launch_cfl_reduce<float>(const CflParams<float>&, int, cudaStream_t);
 template cudaError_t launch_cfl_reduce<double>(const CflParams<double>&, int, cudaStream_t);
+template cudaError_t launch_cfl_candidates<float>(const CflParams<float>&, int, cudaStream_t);
+template cudaError_t launch_cfl_candidates<double>(const CflParams<double>&, int, cudaStream_t);
 template cudaError_t launch_cfl_finish<float>(const CflParams<float>&, cudaStream_t);
 template cudaError_t launch_cfl_finish<double>(const CflParams<double>&, cudaStream_t);
 

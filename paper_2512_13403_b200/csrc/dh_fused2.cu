@@ -77,7 +77,7 @@ DH_DI void recon_x2(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
 
 }  // namespace
 
-template <class T, int LIM, int NRW, bool V16>
+template <class T, int LIM, int NRW, bool V16, bool CAND>
 __global__ void __launch_bounds__((NRW + 1) * 32, 1)
 stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   using G = Geo2<NRW>;
@@ -104,6 +104,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   const P2<T> cz = bc2(tau * p.inv_dx[2]), ncz = bc2(-tau * p.inv_dx[2]);
   const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
   const Consts<T>& c = p.c;
+  const T cand_thr = CAND ? p.cand_thr[0] : T(0);   // CAND: push the CFL candidates of the result (dh_advance)
   int pz = wrapm2(z0 - 2, nz);
   size_t op = (size_t)pz * NP, opm1 = op, opm2 = op;   // element offsets of planes p, p-1, p-2
 
@@ -200,6 +201,10 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
         if (p.cool) cool2(Uo, dt, c);                                                               \
         if (st && ok_) {                                                                            \
           _Pragma("unroll") for (int f = 0; f < 5; ++f) stg2_(p.out + f * N + opm2 + o_, Uo[f]);    \
+          if (CAND && cfl_candidate2(Uo, c, cand_thr)) {                                           \
+            const unsigned slot = atomicAdd(p.cand_cnt, 1u);                                        \
+            if (slot < p.cand_cap) p.cand_list[slot] = (unsigned)(opm2 + o_);                       \
+          }                                                                                         \
         }                                                                                           \
         _Pragma("unroll") for (int f = 0; f < 5; ++f) acc_[f] = fma2(cz, Fz[f], lds2_(Bst + bq * G::STAGE + f * FS + st_)); \
       }
@@ -396,13 +401,13 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
 
 namespace {
 
-template <class T, int LIM, int NRW, bool V16>
-cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
+template <class T, int LIM, int NRW, bool V16, bool CAND>
+cudaError_t launch_one2c(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   using G = Geo2<NRW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
   static bool configured = false;     // per instantiation; the attribute is per function and sticks
   if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, NRW, V16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, NRW, V16, CAND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     configured = true;
   }
@@ -411,7 +416,7 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   // pick the chunk count that minimises waves x (planes per chunk + 4)
   int dev = 0, per_sm = 1;
   cudaGetDevice(&dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, NRW, V16>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, NRW, V16, CAND>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
   const long long slots = (long long)per_sm * sm_count, tiles = (long long)bx * by;
   int bz = 1;
   long long best = -1;
@@ -423,8 +428,13 @@ cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   }
   const int ZL = (p.nz + bz - 1) / bz;
   dim3 grid(bx, by, bz), block((NRW + 1) * 32);
-  stage_fused2_kernel<T, LIM, NRW, V16><<<grid, block, smem, s>>>(p, ZL);
+  stage_fused2_kernel<T, LIM, NRW, V16, CAND><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
+}
+
+template <class T, int LIM, int NRW, bool V16>
+cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
+  return p.cand_list ? launch_one2c<T, LIM, NRW, V16, true>(p, sm_count, s) : launch_one2c<T, LIM, NRW, V16, false>(p, sm_count, s);
 }
 
 }  // namespace

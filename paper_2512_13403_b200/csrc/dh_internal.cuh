@@ -21,6 +21,12 @@ struct StageParams {
   T frac;            // 1/2 for the predictor, 1 for the corrector
   int cool;          // apply the cooling source to the result (corrector only)
   Consts<T> c;
+  // CFL candidates of the NEXT step (last stage inside dh_advance only; nullptr = off): packs of the result whose
+  // wave-speed estimate reaches *cand_thr are appended to cand_list (dh_cfl.cu evaluates the exact recipe on them)
+  unsigned* cand_list;
+  unsigned* cand_cnt;     // [0] packs appended (may exceed cand_cap: overflow = fall back to the full reduction)
+  const T* cand_thr;      // [0] derated threshold for the estimate
+  unsigned cand_cap;
 };
 
 // Parameters of one reversed stage  out = b1 + b2 - frac*dt * J_D(U)^T g   (gather form).
@@ -84,6 +90,12 @@ struct CflParams {
   unsigned long long* acc;   // [0..2] running max (bit pattern of T, zero-extended), [3] non-finite flag
   T* dt_dev;                 // dt in T for the stage kernels
   CflResult* result;         // device copy of the result block
+  // candidate path (all nullptr = plain reduction): see StageParams
+  const unsigned* cand_list;
+  unsigned* cand_cnt;        // [0] packs appended by the last stage, [1] "the full reduction is needed" flag
+  T* cand_thr;               // [0] derated threshold for the estimate, [1] theta = 0.97 min_a S_a of the last dt
+  unsigned cand_cap;
+  unsigned long long* cand_stats;   // [0] candidate passes, [1] fallbacks to the full reduction, [2] packs evaluated
 };
 
 struct Ctx {
@@ -112,6 +124,13 @@ struct Ctx {
   double* adj_dts_dev;         // dh_adjoint: dt sequence (device, T widened by the CFL epilogue)
   double* adj_dts_host;        // pinned mirror
   int adj_dts_cap;
+  unsigned* cand_list;         // dh_advance: CFL candidates pushed by the last stage (packs), see StageParams
+  unsigned* cand_cnt;
+  void* cand_thr;
+  unsigned long long* cand_stats;
+  unsigned cand_cap;
+  int cand_ok;                 // the last stage launched did push candidates for the state it wrote
+  int fuse_cfl;                // DH_OPT_FUSE_CFL
   unsigned long long* acc;     // device accumulators of the CFL reduction
   void* dt_dev;                // device dt (T)
   CflResult* result_dev;
@@ -140,6 +159,7 @@ template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cu
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_lincomb(T* out, T a, const T* X, T b, const T* Y, size_t n, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
+template <class T> cudaError_t launch_cfl_candidates(const CflParams<T>& p, int sm_count, cudaStream_t s);   // candidates, then the guarded full pass
 template <class T> cudaError_t launch_cfl_finish(const CflParams<T>& p, cudaStream_t s);
 
 }  // namespace dh

@@ -19,7 +19,7 @@ DH_F32, DH_F64 = 0, 1
 DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, -4
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
-    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13,
+    "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
@@ -30,6 +30,7 @@ SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
+    "dh_cfl_stats",
 ]
 KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb"]
 
@@ -72,6 +73,8 @@ def load(rebuild: bool = False):
     lib.dh_launch_count.argtypes = [vp]
     lib.dh_profile_enable.argtypes = [vp, ci]
     lib.dh_profile_read.argtypes = [vp, pd, ctypes.POINTER(ctypes.c_ulonglong)]
+    lib.dh_cfl_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
+    lib.dh_cfl_stats.restype = ci
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
@@ -189,6 +192,13 @@ def dh_profile_enable(ctx, on: bool) -> None:
     _check(load().dh_profile_enable(ctx, 1 if on else 0))
 
 
+def dh_cfl_stats(ctx) -> dict:
+    """Counters of the CFL candidate path of dh_advance (include/dh.h)."""
+    out = (ctypes.c_ulonglong * 3)()
+    _check(load().dh_cfl_stats(ctx, out))
+    return {"candidate_passes": int(out[0]), "fallbacks": int(out[1]), "packs": int(out[2])}
+
+
 def dh_profile_read(ctx) -> dict:
     """{kernel kind: (milliseconds, launches)} recorded since the last read."""
     n = len(KERNEL_KINDS)
@@ -278,6 +288,9 @@ class Solver:
 
     def profile_read(self) -> dict:
         return dh_profile_read(self.ctx)
+
+    def cfl_stats(self) -> dict:
+        return dh_cfl_stats(self.ctx)
 
     @property
     def launch_count(self) -> int:

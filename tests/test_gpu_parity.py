@@ -675,3 +675,63 @@ def test_advance_and_adjoint_follow_the_integrator_option(integrator):
     assert torch.equal(Ud, Ua)
     err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
     assert err.max() <= 1e-11, float(err.max())
+
+
+# ------------------------------------------------------------------ CFL candidates inside dh_advance (DH_OPT_FUSE_CFL)
+def _advance_dts(s, U, n):
+    """dt of every step of one dh_advance-style run, by running 1..n steps from copies (dh_advance returns the last)."""
+    return [s.advance(U.clone(), k) for k in range(1, n + 1)]
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+@pytest.mark.parametrize("case", ["turbulence", "spike", "uniform_overflow", "heun"])
+def test_cfl_candidate_path_is_bitwise_the_full_reduction(case, dtype):
+    """From the second step of dh_advance the dt comes from the exact recipe on the packs the previous last stage
+    flagged (estimate >= 0.97 x the previous maximum); whenever that list cannot settle the maxima the full
+    reduction runs.  Either way every dt and the final state must equal, bit for bit, the run with the option off
+    and the host-driven loop: turbulence (the list settles it), a single fast cell whose speed falls by more than
+    3 % per step (threshold missed: fallback), a uniform state with > 2^20 flagged packs (list overflow: fallback),
+    and the candidates pushed by the last stage of another integrator."""
+    kw = {}
+    if case == "turbulence":
+        wl = workloads.turbulence(48, seed=5, mach=2.0, cooling=True, dtype=dtype)
+        U, gamma = wl.U[:, :40, :44, :].contiguous().cuda(), wl.gamma
+        kw = dict(cooling=1, lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor)
+    elif case == "spike":
+        gamma = 1.4
+        U = torch.zeros((5, 12, 14, 64), dtype=dtype)
+        U[0] = 1.0
+        U[4] = 1.0 / (gamma - 1)
+        U[1:4, 5, 6, 31] = 5.0                            # one fast cell: its speed decays by far more than 3 % per step
+        U[4, 5, 6, 31] += 0.5 * 75.0
+        U = U.cuda()
+    elif case == "uniform_overflow":
+        gamma = 1.4
+        U = torch.zeros((5, 132, 128, 132), dtype=dtype)
+        U[0] = 1.0
+        U[1], U[2], U[3] = 0.3, -0.2, 0.1
+        U[4] = 1.0 / (gamma - 1) + 0.5 * (0.09 + 0.04 + 0.01)
+        U = U.cuda()
+    else:
+        U, gamma = random_state((12, 20, 132), 97, 5 / 3, dtype, mach=1.5).cuda(), 5 / 3
+        kw = dict(integrator="heun")
+    n = 6
+    s_on = _solver(U, gamma, fuse_cfl=1, **kw)
+    s_off = _solver(U, gamma, fuse_cfl=0, **kw)
+    a, b, h = U.clone(), U.clone(), U.clone()
+    dt_on, dt_off = s_on.advance(a, n), s_off.advance(b, n)
+    dts = []
+    for _ in range(n):
+        dts.append(s_off.cfl_dt(h))
+        s_off.step(h, dts[-1])
+    assert dt_on == dt_off == dts[-1]
+    assert torch.equal(a, b) and torch.equal(a, h)
+    st = s_on.cfl_stats()
+    assert st["candidate_passes"] == n - 1 and s_off.cfl_stats()["candidate_passes"] == 0
+    if case in ("turbulence", "heun"):
+        assert st["fallbacks"] < n - 1 and 0 < st["packs"] < 0.2 * (n - 1) * U[0].numel() / 2, st
+    elif case == "uniform_overflow":
+        assert st["fallbacks"] == n - 1 and st["packs"] == (n - 1) * (1 << 20), st
+    else:
+        assert st["fallbacks"] >= 1, st                   # the peak speed drops by more than 3 % in a step
+    assert _advance_dts(s_on, U, n) == dts
