@@ -53,6 +53,8 @@ def parse_args():
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
     ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
+    ap.add_argument("--riemann", choices=["hllc", "hll", "rusanov"], default="hllc", help="DH_OPT_RIEMANN (PAPER.md:828, 835); default HLLC")
+    ap.add_argument("--limiter", choices=["minmod", "vanleer", "mc"], default="minmod", help="DH_OPT_LIMITER (PAPER.md:820)")
     ap.add_argument("--integrator", choices=["vl2", "heun", "ssprk3"], default="vl2",
                     help="vl2 = the predictor / corrector of Eqs. A6-A7 (BASELINE's metric); heun, ssprk3: SURVEY 8(f) item 2")
     ap.add_argument("--adjoint", type=int, default=0, help="also time dh_adjoint over this many steps (checkpointed multi-step adjoint)")
@@ -130,14 +132,19 @@ class ClockSampler:
 
 
 # --------------------------------------------------------------------------------------------- oracle legs
-def oracle_sample(U_block, gamma: float, cooling: bool, with_vjp: bool = False, seed: int = 2005) -> dict:
+def _scheme(a) -> dict:
+    return {"limiter": a.limiter, "riemann": a.riemann, "integrator": a.integrator}
+
+
+def oracle_sample(U_block, gamma: float, cooling: bool, with_vjp: bool = False, seed: int = 2005, scheme: dict | None = None) -> dict:
     """Time the CPU oracle, as it stands, for one CFL dt + one full step on `U_block` ([5, m, m, m] numpy,
     treated as its own periodic box).  Returns cell-updates/s and what was timed."""
     import numpy as np
 
     import oracle
 
-    p = oracle.params(gamma=gamma, shape=tuple(U_block.shape), cooling=cooling)
+    scheme = scheme or {}          # limiter / riemann / integrator of the timed arm
+    p = oracle.params(gamma=gamma, shape=tuple(U_block.shape), cooling=cooling, **scheme)
     cells = int(np.prod(U_block.shape[1:]))
     t0 = time.perf_counter()
     dt, _ = oracle.cfl_dt(U_block, p)
@@ -150,7 +157,7 @@ def oracle_sample(U_block, gamma: float, cooling: bool, with_vjp: bool = False, 
         m = min(96, U_block.shape[1])
         sub = np.ascontiguousarray(U_block[:, :m, :m, :m])
         g = np.random.default_rng(seed).normal(size=sub.shape)
-        ps = oracle.params(gamma=gamma, shape=tuple(sub.shape), cooling=cooling)
+        ps = oracle.params(gamma=gamma, shape=tuple(sub.shape), cooling=cooling, **scheme)
         t0 = time.perf_counter()
         oracle.step_vjp(sub, dt, g, ps)
         t_v = time.perf_counter() - t0
@@ -181,11 +188,11 @@ def run_reference(a):
 
     oracle.build()
     for _ in range(min(a.warmup, 1)):
-        oracle_sample(U, gamma, bool(a.cooling))
+        oracle_sample(U, gamma, bool(a.cooling), scheme=_scheme(a))
     times, last = [], None
     for _ in range(a.steps):
         t0 = time.perf_counter()
-        last = oracle_sample(U, gamma, bool(a.cooling))
+        last = oracle_sample(U, gamma, bool(a.cooling), scheme=_scheme(a))
         times.append(time.perf_counter() - t0)
     cells = m ** 3
     total = sum(times)
@@ -247,7 +254,7 @@ def run_dh(a):
     U_cpu_block = U[:, :m, :m, :m].contiguous().cpu().numpy() if (rank == 0 and world == 1 and not a.no_cpu) else None
 
     s = dh.Solver(n, n, n, gamma=wl.gamma, dtype=torch.float32, kernel=a.kernel, cooling=int(a.cooling),
-                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator)
+                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator, riemann=a.riemann, limiter=a.limiter)
     # algorithmic words per cell of one step: CFL 5 + per stage (5 in [+ 5 base] + 5 out) + per combination 15
     fwd_words = {"vl2": FWD_WORDS, "heun": 5 + 10 + 15 + 15, "ssprk3": 5 + 10 + 15 + 15 + 15 + 15}[a.integrator]
 
@@ -351,7 +358,7 @@ def run_dh(a):
             "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
-                       "cfl": 0.4, "limiter": "minmod", "riemann": "hllc", "integrator": {"vl2": "rk2 predictor/corrector", "heun": "heun rk2", "ssprk3": "ssprk3"}[a.integrator],
+                       "cfl": 0.4, "limiter": a.limiter, "riemann": a.riemann, "integrator": {"vl2": "rk2 predictor/corrector", "heun": "heun rk2", "ssprk3": "ssprk3"}[a.integrator],
                        "cooling": bool(a.cooling), "kernel": a.kernel,
                        "call": "dh_cfl_dt_async + dh_step_devdt per step" if a.no_chain else "dh_advance(U, K): K x (CFL reduce, dt epilogue, predictor, corrector)", "parallelism": f"replicas x{world}",
                        "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
@@ -450,7 +457,7 @@ def run_dh(a):
         import oracle
 
         oracle.build()
-        line["cpu_baseline"] = oracle_sample(U_cpu_block, wl.gamma, bool(a.cooling), with_vjp=not a.no_vjp)
+        line["cpu_baseline"] = oracle_sample(U_cpu_block, wl.gamma, bool(a.cooling), with_vjp=not a.no_vjp, scheme=_scheme(a))
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -79,6 +79,9 @@ enum {
                             packs of its result whose estimated wave speed reaches 0.97 x the previous maximum to a list,
                             and the next dt comes from the exact recipe on that list (the full reduction runs only
                             when the list cannot settle the maxima).  dt and the states are bit-identical either way */
+  DH_OPT_RIEMANN = 15,   /* Riemann flux at the faces, all with the wave speeds of Eq. A3: 0 HLLC (default),
+                            1 two-wave HLL, 2 Rusanov / local Lax-Friedrichs.  Forward: the fused stage kernel;
+                            dh_step_vjp / dh_adjoint with 1 or 2: the one-thread-per-cell gather kernels */
   DH_OPT_COUNT_
 };
 

@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import concurrent.futures
 import glob
 import os
 import shutil
@@ -15,11 +16,13 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdh.so")
 ROOT = os.path.dirname(HERE)
 
-NVCC_FLAGS = [
+COMPILE_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-std=c++17", "-lineinfo",
-    "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-Xcompiler", "-fPIC",
 ]
+LINK_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "static"]
+NVCC_FLAGS = COMPILE_FLAGS + LINK_FLAGS[2:]   # the flags of the whole build, for callers that print them
 
 
 def nvcc_path() -> str | None:
@@ -52,12 +55,35 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if nvcc is None:
         raise RuntimeError("nvcc not found: cannot build libdh.so (there is no CPU fallback)")
     tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + sources() + ["-o", tmp]
-    res = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
-    if verbose or res.returncode != 0:
-        sys.stderr.write(res.stdout + res.stderr)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed building libdh.so")
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    extra = ["-Xptxas", "-v"] if verbose else []
+
+    def compile_one(src: str):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + f".{os.getpid()}.o")
+        cmd = [nvcc] + COMPILE_FLAGS + extra + ["-c", src, "-o", obj]
+        return obj, subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+
+    # one nvcc per translation unit, side by side (the stage kernels dominate: the build takes as long as the slowest file)
+    with concurrent.futures.ThreadPoolExecutor(max_workers=max(1, min(len(sources()), os.cpu_count() or 1))) as pool:
+        results = list(pool.map(compile_one, sources()))
+    failed = False
+    for _, res in results:
+        if verbose or res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+        failed |= res.returncode != 0
+    objs = [o for o, _ in results]
+    try:
+        if failed:
+            raise RuntimeError("nvcc failed building libdh.so")
+        res = subprocess.run([nvcc] + LINK_FLAGS + objs + ["-o", tmp], cwd=CSRC, capture_output=True, text=True)
+        if res.returncode != 0:
+            sys.stderr.write(res.stdout + res.stderr)
+            raise RuntimeError("nvcc failed linking libdh.so")
+    finally:
+        for o in objs:
+            if os.path.exists(o):
+                os.remove(o)
     os.replace(tmp, LIB)
     return LIB
 

@@ -115,7 +115,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->gamma = gamma;
   c->cfl = 0.4;
   c->L[0] = c->L[1] = c->L[2] = 1.0;
-  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->integrator = 0; c->fuse_cfl = 1;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->fuse_cfl = 1;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
@@ -176,6 +176,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
     case DH_OPT_FUSE_CFL: c->fuse_cfl = (v != 0.0); break;
+    case DH_OPT_RIEMANN: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: riemann must be 0, 1 or 2%s"); c->riemann = (int)v; break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
   return DH_OK;
@@ -197,6 +198,7 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_REV_SLAB: *out = c->rev_slab_opt; break;
     case DH_OPT_INTEGRATOR: *out = c->integrator; break;
     case DH_OPT_FUSE_CFL: *out = c->fuse_cfl; break;
+    case DH_OPT_RIEMANN: *out = c->riemann; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
   return DH_OK;
@@ -291,14 +293,14 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
   bool done = false;
   if (c->kernel == 0) {
     bool supported = false;
-    cudaError_t e = launch_stage_fused2<T>(p, c->limiter, c->sm_count, c->stream, &supported);
+    cudaError_t e = launch_stage_fused2<T>(p, c->limiter, c->riemann, c->sm_count, c->stream, &supported);
     if (supported) {
       if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
       done = true;
       c->cand_ok = p.cand_list != nullptr;      // only this kernel pushes candidates
     }
   }
-  if (!done && c->kernel != 1) {
+  if (!done && c->kernel != 1 && c->riemann == 0) {      // the first fused kernel has the HLLC flux only
     bool supported = false;
     cudaError_t e = launch_stage_fused<T>(p, c->limiter, c->sm_count, c->stream, &supported);
     if (supported) {
@@ -306,7 +308,7 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
       done = true;
     }
   }
-  if (!done) DH_CUDA(launch_stage_naive<T>(p, c->limiter, c->stream), "dh_step: stage kernel launch");
+  if (!done) DH_CUDA(launch_stage_naive<T>(p, c->limiter, c->riemann, c->stream), "dh_step: stage kernel launch");
   c->launches += 1;
   return DH_OK;
 }
@@ -372,7 +374,7 @@ static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const v
   p.frac = (T)frac;
   p.c = make_consts<T>(c);
   ProfScope ps(c, kind);
-  DH_CUDA(launch_rev_naive<T>(p, c->limiter, c->stream), "dh_step_vjp: reverse stage kernel launch");
+  DH_CUDA(launch_rev_naive<T>(p, c->limiter, c->riemann, c->stream), "dh_step_vjp: reverse stage kernel launch");
   c->launches += 1;
   return DH_OK;
 }
@@ -432,7 +434,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
 template <class T>
 static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
   // the fused pair handles minmod on even nx; everything else takes the one-thread-per-cell gather kernel
-  if (c->kernel == 0 && c->limiter == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
+  if (c->kernel == 0 && c->limiter == 0 && c->riemann == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
   return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
 }
 

@@ -102,7 +102,7 @@ struct Ctx {
   int nx, ny, nz, dtype;
   size_t N;
   double gamma, cfl, L[3];
-  int cooling, kernel, limiter, integrator;
+  int cooling, kernel, limiter, riemann, integrator;
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
   int sm_count;
@@ -150,10 +150,11 @@ struct ProfRec {
 size_t elem_size(const Ctx* c);
 
 // launchers (each returns the cudaError_t of the launch)
-template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, cudaStream_t s);
+template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, int riemann, cudaStream_t s);
 template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
-template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
-template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s);
+template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s, bool* supported);
+template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
+template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);
 template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);

@@ -1,7 +1,7 @@
 // dh_math.cuh — pointwise device arithmetic of the Euler finite-volume step (sm_100a).
 //
 // Primitive conversion (Eq. 2), limited slopes (Eq. A1), the HLLC flux with
-// the wave-speed estimates of Eq. A3, the cooling update (Eq. 23) and the
+// the wave-speed estimates of Eq. A3, the HLL and Rusanov alternatives, the cooling update (Eq. 23) and the
 // hand-written reverse-mode counterparts of each.  The formulas are arranged for instruction count
 // (one reciprocal per density, star state evaluated on the upwind side only, transverse momentum flux
 // as v_t * F_mass, the supersonic branches folded into S_eff = min(S_L,0) / max(S_R,0)); they are
@@ -261,6 +261,126 @@ __device__ __forceinline__ void hllc_vjp(const T L[5], const T R[5], const Const
   rhoRb -= rRb * rR * rR;
   Lb[0] += rhoLb; Lb[n] += uLb; Lb[4] += PLb;
   Rb[0] += rhoRb; Rb[n] += uRb; Rb[4] += PRb;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Two-wave HLL and Rusanov / local Lax-Friedrichs fluxes (PAPER.md:835 lists them beside HLLC; same wave-speed
+// estimates, Eq. A3).  Both are F = wL F_L + wR F_R + wU (U_R - U_L):
+//   HLL      b- = min(S_L, 0), b+ = max(S_R, 0):  wL = b+/(b+ - b-), wR = -b-/(b+ - b-), wU = b+ b-/(b+ - b-)
+//            (b- = 0 gives F_L, b+ = 0 gives F_R: the supersonic branches without a select);
+//   Rusanov  a = max(|S_L|, |S_R|):               wL = wR = 1/2, wU = -a/2.
+// RS: 1 HLL, 2 Rusanov.
+// ------------------------------------------------------------------------------------------------
+template <class T, int AX>
+__device__ __forceinline__ void phys_flux(const T W[5], const Consts<T>& c, T U[5], T F[5]) {
+  constexpr int n = 1 + AX;
+  const T rho = W[0], u = W[n];
+  const T q = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  const T E = W[4] * c.inv_gm1 + T(0.5) * rho * q;
+  const T fm = rho * u;
+  U[0] = rho; U[1] = rho * W[1]; U[2] = rho * W[2]; U[3] = rho * W[3]; U[4] = E;
+  F[0] = fm; F[1] = fm * W[1]; F[2] = fm * W[2]; F[3] = fm * W[3]; F[4] = u * (E + W[4]);
+  F[n] += W[4];
+}
+
+// Wb += (dU/dW)^T Ub + (dF/dW)^T Fb
+template <class T, int AX>
+__device__ __forceinline__ void phys_flux_vjp(const T W[5], const Consts<T>& c, const T Ub[5], const T Fb[5], T Wb[5]) {
+  constexpr int n = 1 + AX;
+  const T rho = W[0], u = W[n];
+  const T q = W[1] * W[1] + W[2] * W[2] + W[3] * W[3];
+  const T E = W[4] * c.inv_gm1 + T(0.5) * rho * q;
+  const T fm = rho * u;
+  const T Eb = Ub[4] + Fb[4] * u;
+  const T fmb = Fb[0] + Fb[1] * W[1] + Fb[2] * W[2] + Fb[3] * W[3];
+  const T er = Eb * rho;
+  Wb[4] += Fb[4] * u + Fb[n] + Eb * c.inv_gm1;
+  Wb[0] += Ub[0] + Ub[1] * W[1] + Ub[2] * W[2] + Ub[3] * W[3] + fmb * u + T(0.5) * Eb * q;
+  Wb[1] += Fb[1] * fm + Ub[1] * rho + er * W[1];
+  Wb[2] += Fb[2] * fm + Ub[2] * rho + er * W[2];
+  Wb[3] += Fb[3] * fm + Ub[3] * rho + er * W[3];
+  Wb[n] += Fb[4] * (E + W[4]) + fmb * rho;
+}
+
+template <class T, int AX, int RS>
+__device__ __forceinline__ void hll_flux(const T L[5], const T R[5], const Consts<T>& c, T F[5]) {
+  constexpr int n = 1 + AX;
+  const T cL = sqrt_(c.gamma * L[4] * rcp_(L[0])), cR = sqrt_(c.gamma * R[4] * rcp_(R[0]));
+  const T SL = min_(L[n] - cL, R[n] - cR);          // Eq. A3
+  const T SR = max_(L[n] + cL, R[n] + cR);
+  T UL[5], UR[5], FL[5], FR[5];
+  phys_flux<T, AX>(L, c, UL, FL);
+  phys_flux<T, AX>(R, c, UR, FR);
+  T wL, wR, wU;
+  if (RS == 1) {
+    const T bm = min_(SL, T(0)), bp = max_(SR, T(0));
+    const T inv = rcp_(bp - bm);
+    wL = bp * inv; wR = -bm * inv; wU = bp * bm * inv;
+  } else {
+    wL = wR = T(0.5);
+    wU = T(-0.5) * max_(abs_(SL), abs_(SR));
+  }
+#pragma unroll
+  for (int f = 0; f < 5; ++f) F[f] = wL * FL[f] + wR * FR[f] + wU * (UR[f] - UL[f]);
+}
+
+// (Lb, Rb) += (dF/dL, dF/dR)^T Fb on the branches taken (ties as in the flux: S_L >= 0 -> b- inactive, S_R <= 0 -> b+
+// inactive, min / max ties -> first argument, |S_L| >= |S_R| -> S_L carries the Rusanov speed)
+template <class T, int AX, int RS>
+__device__ __forceinline__ void hll_flux_vjp(const T L[5], const T R[5], const Consts<T>& c, const T Fb[5], T Lb[5], T Rb[5]) {
+  constexpr int n = 1 + AX;
+  const T cL = sqrt_(c.gamma * L[4] * rcp_(L[0])), cR = sqrt_(c.gamma * R[4] * rcp_(R[0]));
+  const T sLa = L[n] - cL, sLb = R[n] - cR, sRa = L[n] + cL, sRb = R[n] + cR;
+  const bool pickLa = (sLa <= sLb), pickRa = (sRa >= sRb);
+  const T SL = pickLa ? sLa : sLb, SR = pickRa ? sRa : sRb;
+  T UL[5], UR[5], FL[5], FR[5];
+  phys_flux<T, AX>(L, c, UL, FL);
+  phys_flux<T, AX>(R, c, UR, FR);
+  T wLb = T(0), wRb = T(0), wUb = T(0);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { wLb += Fb[f] * FL[f]; wRb += Fb[f] * FR[f]; wUb += Fb[f] * (UR[f] - UL[f]); }
+  T wL, wR, wU, SLb = T(0), SRb = T(0);
+  if (RS == 1) {
+    const bool onm = (SL < T(0)), onp = (SR > T(0));
+    const T bm = onm ? SL : T(0), bp = onp ? SR : T(0);
+    const T inv = rcp_(bp - bm);
+    wL = bp * inv; wR = -bm * inv; wU = bp * bm * inv;
+    const T invb = wLb * bp - wRb * bm + wUb * bp * bm;
+    const T db = -invb * inv * inv;
+    const T bpb = (wLb + wUb * bm) * inv + db;
+    const T bmb = (wUb * bp - wRb) * inv - db;
+    if (onp) SRb = bpb;
+    if (onm) SLb = bmb;
+  } else {
+    wL = wR = T(0.5);
+    const T aL = abs_(SL), aR = abs_(SR);
+    const T a = (aL >= aR) ? aL : aR;
+    wU = T(-0.5) * a;
+    const T ab = T(-0.5) * wUb;
+    if (aL >= aR) SLb = (SL >= T(0)) ? ab : -ab; else SRb = (SR >= T(0)) ? ab : -ab;
+  }
+  T ULb[5], URb[5], FLb[5], FRb[5];
+#pragma unroll
+  for (int f = 0; f < 5; ++f) { FLb[f] = wL * Fb[f]; FRb[f] = wR * Fb[f]; URb[f] = wU * Fb[f]; ULb[f] = -URb[f]; }
+  phys_flux_vjp<T, AX>(L, c, ULb, FLb, Lb);
+  phys_flux_vjp<T, AX>(R, c, URb, FRb, Rb);
+  // S_R = max(uL + cL, uR + cR), S_L = min(uL - cL, uR - cR); c_K = sqrt(gamma P_K / rho_K)
+  T cLb = T(0), cRb = T(0);
+  if (pickRa) { Lb[n] += SRb; cLb += SRb; } else { Rb[n] += SRb; cRb += SRb; }
+  if (pickLa) { Lb[n] += SLb; cLb -= SLb; } else { Rb[n] += SLb; cRb -= SLb; }
+  const T hL = T(0.5) * cLb * cL, hR = T(0.5) * cRb * cR;
+  Lb[4] += hL * rcp_(L[4]); Lb[0] -= hL * rcp_(L[0]);
+  Rb[4] += hR * rcp_(R[4]); Rb[0] -= hR * rcp_(R[0]);
+}
+
+// RS: 0 HLLC, 1 HLL, 2 Rusanov (DH_OPT_RIEMANN)
+template <class T, int AX, int RS>
+__device__ __forceinline__ void riemann_flux(const T L[5], const T R[5], const Consts<T>& c, T F[5]) {
+  if (RS == 0) hllc<T, AX>(L, R, c, F); else hll_flux<T, AX, (RS == 0 ? 1 : RS)>(L, R, c, F);
+}
+template <class T, int AX, int RS>
+__device__ __forceinline__ void riemann_flux_vjp(const T L[5], const T R[5], const Consts<T>& c, const T Fb[5], T Lb[5], T Rb[5]) {
+  if (RS == 0) hllc_vjp<T, AX>(L, R, c, Fb, Lb, Rb); else hll_flux_vjp<T, AX, (RS == 0 ? 1 : RS)>(L, R, c, Fb, Lb, Rb);
 }
 
 // ------------------------------------------------------------------------------------------------

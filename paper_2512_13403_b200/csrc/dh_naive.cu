@@ -1,8 +1,9 @@
 // dh_naive.cu — one-thread-per-cell gather kernels (DH_OPT_KERNEL = 1).
 //
 // Same arithmetic as the fused z-sweep kernels, but every thread recomputes everything its cell needs
-// straight from global memory with periodic index arithmetic: 13 primitive conversions, 9 slopes and 6 HLLC
-// fluxes per cell-stage forward; 19 conversions, 15 slopes and 12 HLLC adjoints per cell-stage in reverse.
+// straight from global memory with periodic index arithmetic: 13 primitive conversions, 9 slopes and 6 Riemann
+// fluxes per cell-stage forward; 19 conversions, 15 slopes and 12 flux adjoints per cell-stage in reverse.
+// Template parameters: the limiter (DH_OPT_LIMITER) and the Riemann flux (DH_OPT_RIEMANN: HLLC, HLL, Rusanov).
 // They exist (a) as the in-library cross-check of the fused kernels, (b) as the path for grids the fused
 // kernels do not cover, and (c) as the first correct reverse-mode path (gather form: no atomics,
 // deterministic).  Steps a2-a7 of SURVEY.md §8(a).
@@ -27,7 +28,7 @@ __device__ __forceinline__ void slope(const T Wm[5], const T W0[5], const T Wp[5
 }
 
 // acc -= coef * (F_{+1/2} - F_{-1/2}) along AX, from the five cells W[-2..2]
-template <class T, int LIM, int AX>
+template <class T, int LIM, int RS, int AX>
 __device__ __forceinline__ void axis_divergence(const T Wm2[5], const T Wm1[5], const T W0[5], const T Wp1[5],
                                                 const T Wp2[5], const Consts<T>& c, T coef, T acc[5]) {
   T sm[5], s0[5], sp[5], L[5], R[5], Fm[5], Fp[5];
@@ -36,15 +37,15 @@ __device__ __forceinline__ void axis_divergence(const T Wm2[5], const T Wm1[5], 
   slope<T, LIM>(W0, Wp1, Wp2, sp);
 #pragma unroll
   for (int q = 0; q < 5; ++q) { L[q] = Wm1[q] + T(0.5) * sm[q]; R[q] = W0[q] - T(0.5) * s0[q]; }
-  hllc<T, AX>(L, R, c, Fm);
+  riemann_flux<T, AX, RS>(L, R, c, Fm);
 #pragma unroll
   for (int q = 0; q < 5; ++q) { L[q] = W0[q] + T(0.5) * s0[q]; R[q] = Wp1[q] - T(0.5) * sp[q]; }
-  hllc<T, AX>(L, R, c, Fp);
+  riemann_flux<T, AX, RS>(L, R, c, Fp);
 #pragma unroll
   for (int q = 0; q < 5; ++q) acc[q] -= coef * (Fp[q] - Fm[q]);
 }
 
-template <class T, int LIM>
+template <class T, int LIM, int RS>
 __global__ void __launch_bounds__(128) stage_naive_kernel(const StageParams<T> p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y, k = blockIdx.z;
@@ -63,17 +64,17 @@ __global__ void __launch_bounds__(128) stage_naive_kernel(const StageParams<T> p
   load_prim(p.U, N, at(wrapi(i - 1, nx), j, k), p.c, B);
   load_prim(p.U, N, at(wrapi(i + 1, nx), j, k), p.c, C);
   load_prim(p.U, N, at(wrapi(i + 2, nx), j, k), p.c, D);
-  axis_divergence<T, LIM, 0>(A, B, W0, C, D, p.c, tau * p.inv_dx[0], acc);
+  axis_divergence<T, LIM, RS, 0>(A, B, W0, C, D, p.c, tau * p.inv_dx[0], acc);
   load_prim(p.U, N, at(i, wrapi(j - 2, ny), k), p.c, A);
   load_prim(p.U, N, at(i, wrapi(j - 1, ny), k), p.c, B);
   load_prim(p.U, N, at(i, wrapi(j + 1, ny), k), p.c, C);
   load_prim(p.U, N, at(i, wrapi(j + 2, ny), k), p.c, D);
-  axis_divergence<T, LIM, 1>(A, B, W0, C, D, p.c, tau * p.inv_dx[1], acc);
+  axis_divergence<T, LIM, RS, 1>(A, B, W0, C, D, p.c, tau * p.inv_dx[1], acc);
   load_prim(p.U, N, at(i, j, wrapi(k - 2, nz)), p.c, A);
   load_prim(p.U, N, at(i, j, wrapi(k - 1, nz)), p.c, B);
   load_prim(p.U, N, at(i, j, wrapi(k + 1, nz)), p.c, C);
   load_prim(p.U, N, at(i, j, wrapi(k + 2, nz)), p.c, D);
-  axis_divergence<T, LIM, 2>(A, B, W0, C, D, p.c, tau * p.inv_dx[2], acc);
+  axis_divergence<T, LIM, RS, 2>(A, B, W0, C, D, p.c, tau * p.inv_dx[2], acc);
   if (p.cool) acc[4] = cool_energy(acc, dt, p.c);
 #pragma unroll
   for (int f = 0; f < 5; ++f) p.out[f * N + c0] = acc[f];
@@ -81,7 +82,7 @@ __global__ void __launch_bounds__(128) stage_naive_kernel(const StageParams<T> p
 
 // Wb += contribution of axis AX to the cotangent of W at the centre cell.
 // W[0..6] = cells i-3..i+3 along the axis, g[0..4] = cotangent at cells i-2..i+2, coef = tau/dx.
-template <class T, int LIM, int AX>
+template <class T, int LIM, int RS, int AX>
 __device__ __forceinline__ void axis_vjp(const T (&W)[7][5], const T (&g)[5][5], const Consts<T>& c, T coef, T Wb[5]) {
   T s[5][5];          // slopes of cells i-2..i+2
 #pragma unroll
@@ -98,7 +99,7 @@ __device__ __forceinline__ void axis_vjp(const T (&W)[7][5], const T (&g)[5][5],
       WLb[j][q] = T(0);
       WRb[j][q] = T(0);
     }
-    hllc_vjp<T, AX>(L, R, c, lam, WLb[j], WRb[j]);
+    riemann_flux_vjp<T, AX, RS>(L, R, c, lam, WLb[j], WRb[j]);
   }
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
@@ -115,7 +116,7 @@ __device__ __forceinline__ void axis_vjp(const T (&W)[7][5], const T (&g)[5][5],
   }
 }
 
-template <class T, int LIM>
+template <class T, int LIM, int RS>
 __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   const int j = blockIdx.y, k = blockIdx.z;
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
 #pragma unroll
   for (int m = 0; m < 5; ++m)
     for (int f = 0; f < 5; ++f) g[m][f] = (m == 2) ? gc[f] : p.g[f * N + at(wrapi(i + m - 2, nx), j, k)];
-  axis_vjp<T, LIM, 0>(W, g, p.c, tau * p.inv_dx[0], Wb);
+  axis_vjp<T, LIM, RS, 0>(W, g, p.c, tau * p.inv_dx[0], Wb);
 
 #pragma unroll
   for (int m = 0; m < 7; ++m)
@@ -147,7 +148,7 @@ __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
 #pragma unroll
   for (int m = 0; m < 5; ++m)
     for (int f = 0; f < 5; ++f) g[m][f] = (m == 2) ? gc[f] : p.g[f * N + at(i, wrapi(j + m - 2, ny), k)];
-  axis_vjp<T, LIM, 1>(W, g, p.c, tau * p.inv_dx[1], Wb);
+  axis_vjp<T, LIM, RS, 1>(W, g, p.c, tau * p.inv_dx[1], Wb);
 
 #pragma unroll
   for (int m = 0; m < 7; ++m)
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
 #pragma unroll
   for (int m = 0; m < 5; ++m)
     for (int f = 0; f < 5; ++f) g[m][f] = (m == 2) ? gc[f] : p.g[f * N + at(i, j, wrapi(k + m - 2, nz))];
-  axis_vjp<T, LIM, 2>(W, g, p.c, tau * p.inv_dx[2], Wb);
+  axis_vjp<T, LIM, RS, 2>(W, g, p.c, tau * p.inv_dx[2], Wb);
 
   T u[5], Ub[5];
 #pragma unroll
@@ -183,25 +184,31 @@ __global__ void __launch_bounds__(256) cool_vjp_kernel(const T* __restrict__ U1,
   }
 }
 
-template <class T>
-cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, cudaStream_t s) {
-  dim3 block(128), grid((p.nx + 127) / 128, p.ny, p.nz);
-  switch (limiter) {
-    case 1: stage_naive_kernel<T, 1><<<grid, block, 0, s>>>(p); break;
-    case 2: stage_naive_kernel<T, 2><<<grid, block, 0, s>>>(p); break;
-    default: stage_naive_kernel<T, 0><<<grid, block, 0, s>>>(p); break;
+// limiter in {0, 1, 2} x riemann in {0, 1, 2} -> one instantiation each
+#define DH_NAIVE_DISPATCH(KERNEL, ...)                                        \
+  switch (limiter * 3 + riemann) {                                            \
+    case 1: KERNEL<T, 0, 1><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 2: KERNEL<T, 0, 2><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 3: KERNEL<T, 1, 0><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 4: KERNEL<T, 1, 1><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 5: KERNEL<T, 1, 2><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 6: KERNEL<T, 2, 0><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 7: KERNEL<T, 2, 1><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    case 8: KERNEL<T, 2, 2><<<grid, block, 0, s>>>(__VA_ARGS__); break;       \
+    default: KERNEL<T, 0, 0><<<grid, block, 0, s>>>(__VA_ARGS__); break;      \
   }
+
+template <class T>
+cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, int riemann, cudaStream_t s) {
+  dim3 block(128), grid((p.nx + 127) / 128, p.ny, p.nz);
+  DH_NAIVE_DISPATCH(stage_naive_kernel, p)
   return cudaGetLastError();
 }
 
 template <class T>
-cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, cudaStream_t s) {
+cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s) {
   dim3 block(64), grid((p.nx + 63) / 64, p.ny, p.nz);
-  switch (limiter) {
-    case 1: rev_naive_kernel<T, 1><<<grid, block, 0, s>>>(p); break;
-    case 2: rev_naive_kernel<T, 2><<<grid, block, 0, s>>>(p); break;
-    default: rev_naive_kernel<T, 0><<<grid, block, 0, s>>>(p); break;
-  }
+  DH_NAIVE_DISPATCH(rev_naive_kernel, p)
   return cudaGetLastError();
 }
 
@@ -213,10 +220,10 @@ cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, co
   return cudaGetLastError();
 }
 
-template cudaError_t launch_stage_naive<float>(const StageParams<float>&, int, cudaStream_t);
-template cudaError_t launch_stage_naive<double>(const StageParams<double>&, int, cudaStream_t);
-template cudaError_t launch_rev_naive<float>(const RevParams<float>&, int, cudaStream_t);
-template cudaError_t launch_rev_naive<double>(const RevParams<double>&, int, cudaStream_t);
+template cudaError_t launch_stage_naive<float>(const StageParams<float>&, int, int, cudaStream_t);
+template cudaError_t launch_stage_naive<double>(const StageParams<double>&, int, int, cudaStream_t);
+template cudaError_t launch_rev_naive<float>(const RevParams<float>&, int, int, cudaStream_t);
+template cudaError_t launch_rev_naive<double>(const RevParams<double>&, int, int, cudaStream_t);
 template cudaError_t launch_cool_vjp<float>(const float*, const float*, float*, size_t, float, const Consts<float>&, cudaStream_t);
 template cudaError_t launch_cool_vjp<double>(const double*, const double*, double*, size_t, double, const Consts<double>&, cudaStream_t);
 

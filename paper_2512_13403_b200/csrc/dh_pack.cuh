@@ -152,6 +152,55 @@ DH_DI void hllc2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F
   F[4] = fma2(mul2(Seff, w), ZE, mul2(uK, add2(EK, PK)));
 }
 
+// HLL (RS = 1) and Rusanov (RS = 2) fluxes of two faces (wave speeds of Eq. A3), the arrangement of
+// hll_flux() in dh_math.cuh: F = wL F_L + wR F_R + wU (U_R - U_L) with
+//   HLL      b- = min(S_L, 0), b+ = max(S_R, 0):  wL = b+/(b+ - b-), wR = -b-/(b+ - b-), wU = b- wL
+//   Rusanov  wL = wR = 1/2, wU = -max(|S_L|, |S_R|)/2.
+template <class T, int AX>
+DH_DI void phys2(const P2<T> W[5], const Consts<T>& c, P2<T> U[5], P2<T> F[5]) {
+  constexpr int n = 1 + AX, t1 = 1 + (AX + 1) % 3, t2 = 1 + (AX + 2) % 3;
+  const P2<T> q = fma2(W[3], W[3], fma2(W[2], W[2], mul2(W[1], W[1])));
+  const P2<T> E = fma2(mul2(bc2(T(0.5)), W[0]), q, mul2(bc2(c.inv_gm1), W[4]));
+  U[0] = W[0]; U[1] = mul2(W[0], W[1]); U[2] = mul2(W[0], W[2]); U[3] = mul2(W[0], W[3]); U[4] = E;
+  const P2<T> fm = U[n];
+  F[0] = fm;
+  F[n] = fma2(fm, W[n], W[4]);
+  F[t1] = mul2(fm, W[t1]);
+  F[t2] = mul2(fm, W[t2]);
+  F[4] = mul2(W[n], add2(E, W[4]));
+}
+
+template <class T, int AX, int RS>
+DH_DI void hll2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F[5]) {
+  constexpr int n = 1 + AX;
+  const P2<T> g = bc2(c.gamma);
+  const P2<T> gPL = mul2(g, L[4]), gPR = mul2(g, R[4]);
+  const P2<T> cL = mul2(gPL, rsqrt2(mul2(gPL, L[0]))), cR = mul2(gPR, rsqrt2(mul2(gPR, R[0])));
+  const P2<T> SL = min2(sub2(L[n], cL), sub2(R[n], cR));          // Eq. A3
+  const P2<T> SR = max2(add2(L[n], cL), add2(R[n], cR));
+  P2<T> wL, wR, wU;
+  if (RS == 1) {
+    const P2<T> bm = min2(SL, T(0)), bp = max2(SR, T(0));
+    const P2<T> nbm = {max_(-SL.x, T(0)), max_(-SL.y, T(0))};
+    const P2<T> inv = rcp2(add2(bp, nbm));
+    wL = mul2(bp, inv); wR = mul2(nbm, inv); wU = mul2(bm, wL);
+  } else {
+    wL = wR = bc2(T(0.5));
+    wU = mul2(bc2(T(-0.5)), P2<T>{max_(abs_(SL.x), abs_(SR.x)), max_(abs_(SL.y), abs_(SR.y))});
+  }
+  P2<T> UL[5], UR[5], FL[5], FR[5];
+  phys2<T, AX>(L, c, UL, FL);
+  phys2<T, AX>(R, c, UR, FR);
+#pragma unroll
+  for (int f = 0; f < 5; ++f) F[f] = fma2(wU, sub2(UR[f], UL[f]), fma2(wL, FL[f], mul2(wR, FR[f])));
+}
+
+// RS: 0 HLLC, 1 HLL, 2 Rusanov (DH_OPT_RIEMANN)
+template <class T, int AX, int RS>
+DH_DI void riemann2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F[5]) {
+  if (RS == 0) hllc2<T, AX>(L, R, c, F); else hll2<T, AX, (RS == 0 ? 1 : RS)>(L, R, c, F);
+}
+
 // cooling of two finished cells (Eqs. 23-24); per lane
 // CFL candidate test (dh_advance): an estimate of max_a |v_a| + c_s for the two cells of a pack of CONSERVED values in
 // fast math (Eq. A8; dh_cfl.cu evaluates the exact recipe on the packs that pass).  No selects: the pressure floor

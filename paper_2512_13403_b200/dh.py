@@ -20,8 +20,10 @@ DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, 
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
+    "riemann": 15,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
+RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
 KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 
@@ -229,6 +231,8 @@ class Solver:
         for k, v in options.items():
             if k == "limiter" and isinstance(v, str):
                 v = LIMITERS[v]
+            if k == "riemann" and isinstance(v, str):
+                v = RIEMANN[v]
             if k == "integrator" and isinstance(v, str):
                 v = INTEGRATORS[v]
             if k == "kernel" and isinstance(v, str):

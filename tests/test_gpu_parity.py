@@ -735,3 +735,94 @@ def test_cfl_candidate_path_is_bitwise_the_full_reduction(case, dtype):
     else:
         assert st["fallbacks"] >= 1, st                   # the peak speed drops by more than 3 % in a step
     assert _advance_dts(s_on, U, n) == dts
+
+
+# ------------------------------------------------------ HLL / Rusanov fluxes (DH_OPT_RIEMANN)
+RIEMANNS = ["hll", "rusanov"]
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("limiter", ["minmod", "vanleer"])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("riemann", RIEMANNS)
+def test_step_parity_other_riemann(riemann, dtype, limiter, kernel):
+    """HLL / Rusanov in the fused stage kernel and in the gather kernel: ragged tiles, rms Mach 1.5 so that
+    the supersonic branches of HLL (b- = 0 / b+ = 0) are taken on a fair share of the faces."""
+    gamma = 1.4
+    for shape, seed in (((12, 20, 36), 501), ((7, 9, 13), 502), ((5, 16, 128), 503)):
+        U = random_state(shape, seed, gamma, dtype, mach=1.5)
+        p = oracle_params(U, gamma, riemann=riemann, limiter=limiter)
+        s = _solver(U, gamma, riemann=riemann, limiter=limiter, kernel=kernel)
+        assert s.get_option("riemann") == {"hll": 1, "rusanov": 2}[riemann]
+        Ud = U.cuda()
+        dt = s.cfl_dt(Ud)
+        assert dt == oracle.cfl_dt(U.numpy(), p)[0]
+        s.step(Ud, dt)
+        err = max_rel_err(Ud.cpu().numpy(), oracle.step(U.numpy(), dt, p))
+        assert err <= TOL[dtype], (shape, err)
+
+
+@pytest.mark.parametrize("riemann", RIEMANNS)
+def test_other_riemann_differs_from_hllc_and_keeps_the_invariants(riemann):
+    """The option is really honoured (the result differs from HLLC's by far more than rounding), a uniform moving state
+    is preserved bitwise, the step is translation-equivariant bitwise and conservative (fp64, 1e-13)."""
+    gamma = 5 / 3
+    U = random_state((12, 20, 40), 511, gamma, torch.float64, mach=1.0).cuda()
+    s, s0 = _solver(U, gamma, riemann=riemann), _solver(U, gamma)
+    dt = s.cfl_dt(U)
+    a, b = U.clone(), U.clone()
+    s.step(a, dt)
+    s0.step(b, dt)
+    assert max_rel_err(a.cpu().numpy(), b.cpu().numpy()) > 1e-4
+    for f in range(5):
+        tot0, tot1 = math.fsum(U[f].cpu().numpy().ravel()), math.fsum(a[f].cpu().numpy().ravel())
+        assert abs(tot1 - tot0) <= 1e-13 * math.fsum(U[f].abs().cpu().numpy().ravel())
+    for shift in ((1, 0, 0), (0, 3, 0), (5, 7, 33)):
+        V = torch.roll(U, shift, dims=(1, 2, 3)).contiguous()
+        s.step(V, dt)
+        assert torch.equal(V, torch.roll(a, shift, dims=(1, 2, 3)))
+    for dtype in (torch.float64, torch.float32):
+        one = torch.ones((8, 12, 36), dtype=torch.float64)
+        rho, v, P = 1.3, (0.3, -1.7, 2.2), 0.7
+        Uu = torch.stack([rho * one, rho * v[0] * one, rho * v[1] * one, rho * v[2] * one,
+                          (P / (gamma - 1) + 0.5 * rho * sum(x * x for x in v)) * one]).to(dtype).cuda()
+        su = _solver(Uu, gamma, riemann=riemann)
+        ref = Uu.clone()
+        su.step(Uu, 0.5 * su.cfl_dt(Uu))
+        assert torch.equal(Uu, ref)
+
+
+@pytest.mark.parametrize("cooling", [0, 1])
+@pytest.mark.parametrize("limiter", ["minmod", "mc"])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("riemann", RIEMANNS)
+def test_vjp_parity_other_riemann(riemann, dtype, limiter, cooling):
+    """dh_step_vjp with the HLL / Rusanov adjoints (hll_flux_vjp in dh_math.cuh, gather kernels) against the oracle's
+    scatter-form reverse mode: fp64 pointwise 1e-12, fp32 1e-4 of the gradient's rms."""
+    U = random_state((8, 10, 14), 521, 1.4, dtype, mach=1.5)
+    okw = dict(riemann=riemann, limiter=limiter)
+    skw = dict(riemann=riemann, limiter=limiter)
+    if cooling:
+        okw.update(cooling=True, lambda0=0.5, alpha=0.5, t_floor=0.01)
+        skw.update(cooling=1, lambda0=0.5)
+    _vjp_case(U, 1.4, 522, dtype, okw, skw, 1e-12 if dtype == torch.float64 else 1e-4)
+
+
+@pytest.mark.parametrize("riemann", RIEMANNS)
+def test_advance_and_adjoint_follow_the_riemann_option(riemann):
+    """dh_advance (candidate CFL path included) / dh_adjoint with HLL / Rusanov: 4 steps fp64 against the oracle's loop
+    and its composed adjoint."""
+    U = random_state((9, 10, 70), 531, 5 / 3, torch.float64)
+    p = oracle_params(U, 5 / 3, riemann=riemann)
+    g = np.random.default_rng(532).normal(size=tuple(U.shape))
+    Un_ref, g0_ref, dts_ref = oracle.adjoint(U.numpy(), 4, g, p)
+    s = _solver(U, 5 / 3, riemann=riemann)
+    Ua = U.cuda()
+    s.advance(Ua, 4)
+    assert max_rel_err(Ua.cpu().numpy(), Un_ref) <= 5e-12
+    Ud, gd = U.cuda(), torch.from_numpy(g).cuda()
+    dts = s.adjoint(Ud, gd, 4, 3)
+    assert dts[0] == dts_ref[0] and np.allclose(dts, dts_ref, rtol=1e-13, atol=0)
+    assert torch.equal(Ud, Ua)
+    err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
+    assert err.max() <= 1e-11, float(err.max())
