@@ -34,10 +34,12 @@ struct Params {
   int limiter;        // 0 minmod (A4), 1 van Leer, 2 MC, 3 piecewise-constant
   int riemann;        // 0 HLLC, 1 HLL, 2 Rusanov/LF
   int integrator;     // 0 predictor/corrector A6-A7, 1 Heun, 2 SSPRK3
-  int cooling;        // 0 off, 1 on: Eq. 23 with N_sub=1, reading A9
+  int cooling;        // 0 off, 1 on; which update: cool_mode / cool_nsub below
   double lambda0;     // Lambda(T) = lambda0 * T^alpha (reading A10)
   double alpha;
   double t_floor;     // temperature floor, Eq. 24 with R=1
+  int cool_mode;      // 0: Euler + floor of Eq. 23, sub-cycled; 1: trapezoid of Eq. 22, reading A20
+  int cool_nsub;      // N_sub >= 1 substeps of size dt / N_sub in mode 0
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -214,22 +216,42 @@ inline void face_flux(const S Wm1[5], const S W0[5], const S Wp1[5], const S Wp2
 }
 
 // ------------------------------------------------------------------------------------------------
-// Step 6 — pointwise cooling, Eq. 23 with N_sub = 1 and the floor of Eq. 24,
-// applied once after the hydro update and changing only E.  Code units n = rho,
-// T = P/rho, Gamma = 0, Lambda = lambda0 T^alpha (reading A10).
+// Step 6 — pointwise cooling, applied once after the hydro update and changing only E.
+// Code units n = rho, T = P/rho, Gamma = 0, Lambda = lambda0 T^alpha (reading A10), so
+//   Edot(E_th) = -rho^2 lambda0 max(T, 0)^alpha,   T = (gamma-1) E_th / rho.
+// cool_mode 0: the sub-cycled update of Eq. 23: N_sub substeps delta t = dt / N_sub,
+//   E_th^{k+1} = max(E_floor, E_th^k + Edot(T^k) delta t), T^k re-evaluated every substep; N_sub = 1 is reading A9.
+//   (The "maximum fractional change" limiter the paper mentions without a formula is not applied, reading A9.)
+// cool_mode 1: the trapezoid of Eq. 22: E_th^{n+1} = E_th^n + dt/2 [Edot(T^n) + Edot(T^pred)]; the
+//   paper does not define T^pred: reading A20 takes the temperature of the Euler-predicted, floored energy
+//   E_pred = max(E_floor, E_th^n + Edot(T^n) dt), and floors the result by Eq. 24 as well.
+// Floor: Eq. 24 with R = 1.
 // ------------------------------------------------------------------------------------------------
+template <class S>
+inline S cool_rate(const S& Eth, const S& rho, const Params& p) {
+  S T = (p.gamma - 1.0) * Eth / rho;
+  S Tpos = smax(T, S(0.0));
+  return -1.0 * rho * rho * p.lambda0 * spow(Tpos, p.alpha);
+}
+
 template <class S>
 inline void cool(const S U[5], double dt, const Params& p, S out[5]) {
   S rho = U[0];
   S Ek = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
   S Eth = U[4] - Ek;
-  S T = (p.gamma - 1.0) * Eth / rho;
-  S Tpos = smax(T, S(0.0));
-  S Edot = -1.0 * rho * rho * p.lambda0 * spow(Tpos, p.alpha);
   S Efloor = rho * p.t_floor / (p.gamma - 1.0);
-  S Eth1 = smax(Efloor, S(Eth + Edot * dt));
+  if (p.cool_mode == 1) {                       // Eq. 22
+    S Edot_n = cool_rate(Eth, rho, p);
+    S Epred = smax(Efloor, S(Eth + Edot_n * dt));
+    S Edot_p = cool_rate(Epred, rho, p);
+    Eth = smax(Efloor, S(Eth + (0.5 * dt) * (Edot_n + Edot_p)));
+  } else {                                      // Eq. 23
+    const int nsub = p.cool_nsub > 1 ? p.cool_nsub : 1;
+    const double ddt = dt / nsub;
+    for (int k = 0; k < nsub; ++k) Eth = smax(Efloor, S(Eth + cool_rate(Eth, rho, p) * ddt));
+  }
   out[0] = U[0]; out[1] = U[1]; out[2] = U[2]; out[3] = U[3];
-  out[4] = Ek + Eth1;
+  out[4] = Ek + Eth;
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -27,6 +27,7 @@ _lib = None
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2, "constant": 3}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}
+COOL_MODES = {"euler": 0, "trapezoid": 1}
 
 
 class _Params(ctypes.Structure):
@@ -42,6 +43,8 @@ class _Params(ctypes.Structure):
         ("lambda0", ctypes.c_double),
         ("alpha", ctypes.c_double),
         ("t_floor", ctypes.c_double),
+        ("cool_mode", ctypes.c_int),
+        ("cool_nsub", ctypes.c_int),
     ]
 
 
@@ -81,7 +84,8 @@ def set_num_threads(n: int) -> None:
 
 
 def params(gamma=5.0 / 3.0, dx=None, shape=None, rho_floor=1e-10, p_floor=1e-10, limiter="minmod",
-           riemann="hllc", integrator="vl2", cooling=False, lambda0=1e-3, alpha=0.5, t_floor=0.01):
+           riemann="hllc", integrator="vl2", cooling=False, lambda0=1e-3, alpha=0.5, t_floor=0.01,
+           cool_mode="euler", cool_nsub=1):
     """Scheme parameters.  ``dx`` defaults to the unit box, dx_a = 1/n_a (reading A13)."""
     p = _Params()
     p.gamma = float(gamma)
@@ -95,6 +99,10 @@ def params(gamma=5.0 / 3.0, dx=None, shape=None, rho_floor=1e-10, p_floor=1e-10,
     p.limiter, p.riemann, p.integrator = LIMITERS[limiter], RIEMANN[riemann], INTEGRATORS[integrator]
     p.cooling = int(bool(cooling))
     p.lambda0, p.alpha, p.t_floor = float(lambda0), float(alpha), float(t_floor)
+    # Eq. 23 sub-cycled ("euler", N_sub = cool_nsub) or the trapezoid of Eq. 22 (reading A20)
+    p.cool_mode, p.cool_nsub = COOL_MODES[cool_mode], int(cool_nsub)
+    if p.cool_nsub < 1:
+        raise ValueError("cool_nsub must be >= 1")
     return p
 
 

@@ -247,6 +247,79 @@ def test_cooling_floor_engages_exactly():
     assert np.allclose(out[4], rho * 0.01 / (g - 1), rtol=1e-15)
 
 
+def _T_of(U, g):
+    return (g - 1) * (U[4] - 0.5 * (U[1] ** 2 + U[2] ** 2 + U[3] ** 2) / U[0]) / U[0]
+
+
+@pytest.mark.parametrize("nsub", [1, 3, 8])
+def test_cooling_subcycled_is_the_numpy_recurrence(nsub):
+    """Eq. 23 retyped in numpy for moving gas and a general alpha: N_sub Euler substeps of
+    dt / N_sub with T re-evaluated each substep and the floor of Eq. 24 applied each substep; a dropped
+    re-evaluation (rate frozen at T^n) or a floor applied only at the end changes the result."""
+    g, lam, al, tf, dt = 1.4, 0.8, 0.7, 0.4, 0.9
+    rng = np.random.default_rng(12)
+    rho, T0 = rng.uniform(0.5, 2.0, 16), rng.uniform(0.3, 3.0, 16)   # some cells reach the floor mid-way
+    v = rng.normal(0, 0.5, (3, 16))
+    U = np.stack([rho, rho * v[0], rho * v[1], rho * v[2], rho * T0 / (g - 1) + 0.5 * rho * (v ** 2).sum(0)]).reshape(5, 1, 1, 16)
+    p = oracle.params(gamma=g, dx=(1, 1, 1), cooling=True, lambda0=lam, alpha=al, t_floor=tf, cool_nsub=nsub)
+    out = oracle.cooling(U, dt, p)
+    assert np.array_equal(out[:4], U[:4])
+    Eth = rho * T0 / (g - 1)
+    hit_midway = False
+    for k in range(nsub):
+        T = (g - 1) * Eth / rho
+        new = Eth - rho * rho * lam * np.maximum(T, 0.0) ** al * (dt / nsub)
+        hit_midway |= bool(np.any(new < rho * tf / (g - 1))) and k < nsub - 1
+        Eth = np.maximum(rho * tf / (g - 1), new)
+    assert np.allclose(_T_of(out, g).ravel(), (g - 1) * Eth / rho, rtol=1e-13)
+    if nsub > 1:
+        assert hit_midway
+        frozen = np.maximum(rho * tf / (g - 1), rho * T0 / (g - 1) - rho * rho * lam * T0 ** al * dt)
+        assert not np.allclose((g - 1) * frozen / rho, (g - 1) * Eth / rho, rtol=1e-3)
+
+
+def test_cooling_subcycling_error_falls_as_one_over_nsub():
+    """One step of size t against the ODE solution sqrt(T(t)) = sqrt(T0) - (gamma-1) lambda0 rho t / 2 (alpha = 1/2):
+    the sub-cycled Euler update is first order in dt / N_sub."""
+    g, rho, T0, lam, t = 5.0 / 3.0, 2.0, 1.0, 0.05, 4.0
+    exact = (np.sqrt(T0) - 0.5 * (g - 1) * lam * rho * t) ** 2
+    errs = []
+    for n in (16, 32, 64):
+        p = oracle.params(gamma=g, dx=(1, 1, 1), cooling=True, lambda0=lam, alpha=0.5, t_floor=1e-6, cool_nsub=n)
+        out = oracle.cooling(_uniform(rho, (0.2, 0, -0.1), rho * T0), t, p)
+        errs.append(abs(_T_of(out, g)[0, 0, 0] - exact))
+    assert 1.8 < errs[0] / errs[1] < 2.2 and 1.8 < errs[1] / errs[2] < 2.2
+
+
+def test_cooling_trapezoid_closed_form_and_second_order():
+    """Eq. 22 with reading A20 (T^pred = temperature of the Euler-predicted energy): one step retyped in
+    numpy; repeated steps converge to the ODE solution at second order (error ratio 4 per halving of dt), which a
+    missing factor 1/2 or a predictor evaluated at T^n would not."""
+    g, rho, T0, lam = 5.0 / 3.0, 1.7, 2.3, 0.05
+    p = oracle.params(gamma=g, dx=(1, 1, 1), cooling=True, lambda0=lam, alpha=0.5, t_floor=1e-6, cool_mode="trapezoid")
+    dt = 0.37
+    out = oracle.cooling(_uniform(rho, (0.3, -0.2, 0.1), rho * T0), dt, p)
+    k = (g - 1) * rho * lam
+    Tp = T0 - k * np.sqrt(T0) * dt
+    assert np.allclose(_T_of(out, g), T0 - 0.5 * dt * k * (np.sqrt(T0) + np.sqrt(Tp)), rtol=1e-14)
+    t = 4.0
+    exact = (np.sqrt(T0) - 0.5 * k * t) ** 2
+    errs = []
+    for n in (10, 20, 40):
+        U = _uniform(rho, (0, 0, 0), rho * T0)
+        for _ in range(n):
+            U = oracle.cooling(U, t / n, p)
+        errs.append(abs(_T_of(U, g)[0, 0, 0] - exact))
+    assert 3.6 < errs[0] / errs[1] < 4.4 and 3.6 < errs[1] / errs[2] < 4.4
+
+
+def test_cooling_trapezoid_floor():
+    g, rho = 5.0 / 3.0, 1.5
+    p = oracle.params(gamma=g, dx=(1, 1, 1), cooling=True, lambda0=10.0, alpha=0.5, t_floor=0.01, cool_mode="trapezoid")
+    out = oracle.cooling(_uniform(rho, (0, 0, 0), rho * 0.5), 100.0, p)
+    assert np.array_equal(out[4], np.full_like(out[4], rho * 0.01 / (g - 1)))
+
+
 # ----------------------------------------------------------------------------------------------- CFL
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
 def test_cfl_closed_form_uniform_state(dtype):

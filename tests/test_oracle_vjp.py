@@ -26,6 +26,8 @@ CASES = [
     dict(integrator="heun", cooling=True, lambda0=0.5),
     dict(integrator="ssprk3"),
     dict(integrator="ssprk3", cooling=True, lambda0=0.5),
+    dict(cooling=True, lambda0=0.5, cool_nsub=4),
+    dict(cooling=True, lambda0=0.5, cool_mode="trapezoid"),
 ]
 
 
@@ -47,8 +49,9 @@ def test_vjp_equals_transposed_dual_number_jvp(kw):
         assert abs(lhs - rhs) <= 1e-13 * (np.abs(g * Jv).sum() + np.abs(gin * v).sum())
 
 
-@pytest.mark.parametrize("kw", [dict(), dict(cooling=True, lambda0=0.5), dict(integrator="heun"), dict(integrator="ssprk3")],
-                         ids=["hydro", "cooling", "heun", "ssprk3"])
+@pytest.mark.parametrize("kw", [dict(), dict(cooling=True, lambda0=0.5), dict(integrator="heun"), dict(integrator="ssprk3"),
+                                dict(cooling=True, lambda0=0.5, cool_nsub=4), dict(cooling=True, lambda0=0.5, cool_mode="trapezoid")],
+                         ids=["hydro", "cooling", "heun", "ssprk3", "cooling-nsub4", "cooling-trapezoid"])
 def test_vjp_against_central_finite_differences(kw):
     """BASELINE requirement: 8^3 fp64, <g, (H(U+eps v) - H(U-eps v)) / 2 eps> vs <J^T g, v>.
     The scheme is piecewise smooth (limiter / HLLC / floor switches); eps is small enough that for these
