@@ -38,7 +38,7 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/s per RK2 step (forward: CFL dt + predictor + corrector)"
 UNIT = "cell-updates/s"
 FWD_WORDS, VJP_WORDS = 25, 45          # algorithmic words per cell: SURVEY.md §8(d), DESIGN.md §"Kernels"
-STAGE_WORDS = {"stage1": 10, "stage2": 15, "rev2": 15, "rev1": 20, "cfl_reduce": 5, "lincomb": 15}
+STAGE_WORDS = {"stage1": 10, "stage2": 15, "rev2": 15, "rev1": 20, "cfl_reduce": 5, "lincomb": 15, "cool": 6}
 FALLBACK_HBM_GBS = 6650.0              # /opt/skills/guides/B200_PROFILING.md, used only without MEASURED_PEAKS.json
 
 
@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--impl", default="dh", choices=["dh", "reference"])
     ap.add_argument("--n", "--grid", dest="n", type=int, default=1024, help="grid size per axis (default 1024: BASELINE configs[4])")
     ap.add_argument("--cooling", type=int, default=0, help="1: configs[3]'s cooling source in the corrector epilogue")
+    ap.add_argument("--cool-mode", choices=["euler", "trapezoid"], default="euler", help="DH_OPT_COOL_MODE (PAPER.md:318-325), with --cooling 1")
+    ap.add_argument("--cool-nsub", type=int, default=1, help="DH_OPT_COOL_NSUB: substeps of Eq. 23, with --cooling 1")
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
     ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
@@ -133,7 +135,7 @@ class ClockSampler:
 
 # --------------------------------------------------------------------------------------------- oracle legs
 def _scheme(a) -> dict:
-    return {"limiter": a.limiter, "riemann": a.riemann, "integrator": a.integrator}
+    return {"limiter": a.limiter, "riemann": a.riemann, "integrator": a.integrator, "cool_mode": a.cool_mode, "cool_nsub": a.cool_nsub}
 
 
 def oracle_sample(U_block, gamma: float, cooling: bool, with_vjp: bool = False, seed: int = 2005, scheme: dict | None = None) -> dict:
@@ -254,7 +256,8 @@ def run_dh(a):
     U_cpu_block = U[:, :m, :m, :m].contiguous().cpu().numpy() if (rank == 0 and world == 1 and not a.no_cpu) else None
 
     s = dh.Solver(n, n, n, gamma=wl.gamma, dtype=torch.float32, kernel=a.kernel, cooling=int(a.cooling),
-                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator, riemann=a.riemann, limiter=a.limiter)
+                  lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator, riemann=a.riemann, limiter=a.limiter,
+                  cool_mode=a.cool_mode, cool_nsub=a.cool_nsub)
     # algorithmic words per cell of one step: CFL 5 + per stage (5 in [+ 5 base] + 5 out) + per combination 15
     fwd_words = {"vl2": FWD_WORDS, "heun": 5 + 10 + 15 + 15, "ssprk3": 5 + 10 + 15 + 15 + 15 + 15}[a.integrator]
 
@@ -359,7 +362,7 @@ def run_dh(a):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
                        "cfl": 0.4, "limiter": a.limiter, "riemann": a.riemann, "integrator": {"vl2": "rk2 predictor/corrector", "heun": "heun rk2", "ssprk3": "ssprk3"}[a.integrator],
-                       "cooling": bool(a.cooling), "kernel": a.kernel,
+                       "cooling": bool(a.cooling), "cool_mode": a.cool_mode, "cool_nsub": a.cool_nsub, "kernel": a.kernel,
                        "call": "dh_cfl_dt_async + dh_step_devdt per step" if a.no_chain else "dh_advance(U, K): K x (CFL reduce, dt epilogue, predictor, corrector)", "parallelism": f"replicas x{world}",
                        "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
                        if fits_l2 else f"inputs larger than L2 ({5 * 4 * N / 1e6:.0f} MB per state vs 126 MB), no flush",

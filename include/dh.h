@@ -58,7 +58,8 @@ enum {
   DH_OPT_LX = 1,         /* box lengths, default 1; dx_a = L_a / n_a */
   DH_OPT_LY = 2,
   DH_OPT_LZ = 3,
-  DH_OPT_COOLING = 4,    /* 0 (default) / 1: E_th <- max(E_floor(rho), E_th - rho^2 Lambda0 T^alpha dt) after stage 2 */
+  DH_OPT_COOLING = 4,    /* 0 (default) / 1: E_th <- max(E_floor(rho), E_th - rho^2 Lambda0 T^alpha dt) after stage 2
+                            (other integrators of the source: DH_OPT_COOL_MODE, DH_OPT_COOL_NSUB) */
   DH_OPT_LAMBDA0 = 5,    /* default 1e-3 */
   DH_OPT_ALPHA = 6,      /* default 0.5 */
   DH_OPT_T_FLOOR = 7,    /* default 0.01; E_floor = rho T_floor / (gamma-1) (Eq. 24 with R = 1) */
@@ -82,6 +83,11 @@ enum {
   DH_OPT_RIEMANN = 15,   /* Riemann flux at the faces, all with the wave speeds of Eq. A3: 0 HLLC (default),
                             1 two-wave HLL, 2 Rusanov / local Lax-Friedrichs.  Forward: the fused stage kernel;
                             dh_step_vjp / dh_adjoint with 1 or 2: the one-thread-per-cell gather kernels */
+  DH_OPT_COOL_MODE = 16, /* integrator of the cooling source: 0 (default) the Euler update with floor of Eq. 23,
+                            sub-cycled DH_OPT_COOL_NSUB times; 1 the trapezoid of Eq. 22 with T^pred from the Euler-predicted,
+                            floored energy (reading A20).  (0, N_sub = 1) runs in the last stage's epilogue; the others
+                            as one streaming pass over the finished state (DH_K_COOL) */
+  DH_OPT_COOL_NSUB = 17, /* N_sub of Eq. 23: integer in 1 .. 64, default 1; substeps dt / N_sub, rate and floor every substep */
   DH_OPT_COUNT_
 };
 
@@ -173,7 +179,8 @@ enum {
   DH_K_REV1 = 5,         /* reverse predictor */
   DH_K_COOL_VJP = 6,     /* pointwise cooling adjoint */
   DH_K_LINCOMB = 7,      /* out = a X + b Y: base states / scaled cotangents of Heun and SSPRK3 */
-  DH_K_COUNT_ = 8
+  DH_K_COOL = 8,         /* in-place cooling pass of DH_OPT_COOL_MODE = 1 / DH_OPT_COOL_NSUB > 1 */
+  DH_K_COUNT_ = 9
 };
 int dh_profile_enable(dh_ctx* ctx, int on);
 int dh_profile_read(dh_ctx* ctx, double* ms_out, unsigned long long* launches_out);

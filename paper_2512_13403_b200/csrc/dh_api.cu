@@ -48,6 +48,8 @@ static Consts<T> make_consts(const dh_ctx* c) {
   k.alpha = (T)c->alpha;
   k.t_floor = (T)c->t_floor;
   k.alpha_is_half = (c->alpha == 0.5);
+  k.cool_mode = c->cool_mode;
+  k.cool_nsub = c->cool_nsub;
   return k;
 }
 
@@ -115,7 +117,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->gamma = gamma;
   c->cfl = 0.4;
   c->L[0] = c->L[1] = c->L[2] = 1.0;
-  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->fuse_cfl = 1;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->cool_mode = 0; c->cool_nsub = 1; c->fuse_cfl = 1;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
@@ -177,6 +179,10 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
     case DH_OPT_FUSE_CFL: c->fuse_cfl = (v != 0.0); break;
     case DH_OPT_RIEMANN: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: riemann must be 0, 1 or 2%s"); c->riemann = (int)v; break;
+    case DH_OPT_COOL_MODE: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: cool_mode must be 0 or 1%s"); c->cool_mode = (int)v; break;
+    case DH_OPT_COOL_NSUB:
+      if (v < 1 || v > DH_COOL_NSUB_MAX || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: cool_nsub must be an integer in 1 .. 64%s");
+      c->cool_nsub = (int)v; break;
     default: return fail(DH_ERR_ARG, "dh_set_option: unknown key%s");
   }
   return DH_OK;
@@ -199,6 +205,8 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_INTEGRATOR: *out = c->integrator; break;
     case DH_OPT_FUSE_CFL: *out = c->fuse_cfl; break;
     case DH_OPT_RIEMANN: *out = c->riemann; break;
+    case DH_OPT_COOL_MODE: *out = c->cool_mode; break;
+    case DH_OPT_COOL_NSUB: *out = c->cool_nsub; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
   return DH_OK;
@@ -346,20 +354,39 @@ static int rk_prefix(dh_ctx* c, const void* U, double dt, bool devdt, const void
   return rc;
 }
 
+// The cooling integrators the stage kernels do not fuse (sub-cycled Eq. 23 with N_sub > 1, trapezoid Eq. 22): one
+// streaming pass over the finished state (reads 5 words per cell, rewrites E).
+template <class T>
+static int cool_launch(dh_ctx* c, void* U, double dt, bool devdt) {
+  ProfScope ps(c, DH_K_COOL);
+  DH_CUDA(launch_cool_fwd<T>((T*)U, c->N, (T)dt, devdt ? (const T*)c->dt_dev : nullptr, make_consts<T>(c), c->stream),
+          "dh_step: cooling kernel launch");
+  c->launches += 1;
+  return DH_OK;
+}
+
 template <class T>
 static int step_impl(dh_ctx* c, void* U, double dt, bool devdt, bool cand = false) {
+  // default cooling update (Eq. 23, N_sub = 1): epilogue of the last stage; the others: a pass of their own, and the
+  // CFL candidates (pushed by the last stage from the pre-cooling values) are not used
+  const bool split_cool = c->cooling != 0 && (c->cool_mode != 0 || c->cool_nsub > 1);
+  const bool fused_cool = c->cooling != 0 && !split_cool;
   if (c->integrator != 0) {
     // Heun / SSPRK3 in Shu-Osher form: every stage is  out = B - w dt D(state)
     const void* last_in = nullptr;
     double w = 0.0;
     int rc = rk_prefix<T>(c, U, dt, devdt, &last_in, &w);
     if (rc) return rc;
-    return stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, c->cooling != 0, cand);
+    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, fused_cool, cand && !split_cool);
+    if (rc || !split_cool) return rc;
+    return cool_launch<T>(c, U, dt, devdt);
   }
   // predictor: U* = U^n - dt/2 D(U^n)   (Eq. A6);  corrector, in place: U^{n+1} = U^n - dt D(U*)   (Eq. A7)
   int rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 0.5, false);
   if (rc) return rc;
-  return stage_launch<T>(c, DH_K_STAGE2, c->Us, U, U, dt, devdt, 1.0, c->cooling != 0, cand);
+  rc = stage_launch<T>(c, DH_K_STAGE2, c->Us, U, U, dt, devdt, 1.0, fused_cool, cand && !split_cool);
+  if (rc || !split_cool) return rc;
+  return cool_launch<T>(c, U, dt, devdt);
 }
 
 // ------------------------------------------------------------------------------------------ reverse

@@ -103,6 +103,7 @@ struct Ctx {
   size_t N;
   double gamma, cfl, L[3];
   int cooling, kernel, limiter, riemann, integrator;
+  int cool_mode, cool_nsub;    // DH_OPT_COOL_MODE (0 Euler sub-cycled, 1 trapezoid), DH_OPT_COOL_NSUB
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
   int sm_count;
@@ -157,6 +158,7 @@ template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);
 template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
+template <class T> cudaError_t launch_cool_fwd(T* U, size_t N, T dt, const T* dt_dev, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_lincomb(T* out, T a, const T* X, T b, const T* Y, size_t n, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);

@@ -38,6 +38,7 @@ struct Consts {
   // cooling
   T lambda0, alpha, t_floor;
   int alpha_is_half;
+  int cool_mode, cool_nsub;   // DH_OPT_COOL_MODE / DH_OPT_COOL_NSUB; (0, 1) is the update fused into the stage kernels
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -429,6 +430,115 @@ __device__ __forceinline__ void cool_vjp(const T U[5], T dt, const Consts<T>& c,
   }
   // Eth = E - Ek;  Ek = m2 / (2 rho)
   Ekb -= Ethb;
+  gb[4] = Ethb;
+  gb[1] = g[1] + Ekb * U[1] * r;
+  gb[2] = g[2] + Ekb * U[2] * r;
+  gb[3] = g[3] + Ekb * U[3] * r;
+  gb[0] = g[0] + rhob - Ekb * Ek * r;
+}
+
+// ------------------------------------------------------------------------------------------------
+// The other cooling integrators of PAPER.md:318-325 (reading A20), used by the streaming kernels
+// cool_fwd_kernel / cool_vjp_kernel:  cool_mode 0, N_sub > 1: Eq. 23 sub-cycled (rate re-evaluated and the floor of
+// Eq. 24 applied every substep);  cool_mode 1: the trapezoid of Eq. 22 with T^pred from the Euler-predicted, floored
+// energy.  Edot(E_th) = -rho^2 lambda0 max(T, 0)^alpha,  T = (gamma-1) E_th / rho.
+// ------------------------------------------------------------------------------------------------
+constexpr int DH_COOL_NSUB_MAX = 64;
+
+template <class T>
+__device__ __forceinline__ T cool_rate(T Eth, T rho, T r, const Consts<T>& c) {
+  const T Tg = max_(c.gm1 * Eth * r, T(0));
+  const T Ta = c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0));
+  return -(rho * rho * c.lambda0) * Ta;
+}
+
+// (Ethb, rhob) += (dEdot/dE_th, dEdot/drho) * rateb
+template <class T>
+__device__ __forceinline__ void cool_rate_vjp(T Eth, T rho, T r, const Consts<T>& c, T rateb, T& Ethb, T& rhob) {
+  const T Traw = c.gm1 * Eth * r;
+  const bool Tpos = (Traw >= T(0));
+  const T Tg = Tpos ? Traw : T(0);
+  const T Ta = c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0));
+  const T dTa = (Tpos && Tg > T(0)) ? c.alpha * Ta * rcp_(Tg) : T(0);
+  const T Tb = -rateb * rho * rho * c.lambda0 * dTa;
+  rhob += -rateb * T(2) * rho * c.lambda0 * Ta;
+  Ethb += Tb * c.gm1 * r;
+  rhob += -Tb * Traw * r;
+}
+
+template <class T>
+__device__ __forceinline__ T cool_energy_general(const T U[5], T dt, const Consts<T>& c) {
+  const T rho = U[0];
+  const T r = rcp_(rho);
+  const T Ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * r;
+  T Eth = U[4] - Ek;
+  const T Efl = rho * c.t_floor * c.inv_gm1;
+  if (c.cool_mode == 1) {
+    const T rn = cool_rate(Eth, rho, r, c);
+    const T Ep = max_(Efl, Eth + rn * dt);
+    const T rp = cool_rate(Ep, rho, r, c);
+    Eth = max_(Efl, Eth + (T(0.5) * dt) * (rn + rp));
+  } else {
+    const int nsub = c.cool_nsub;
+    const T ddt = dt / T(nsub);
+    for (int k = 0; k < nsub; ++k) Eth = max_(Efl, Eth + cool_rate(Eth, rho, r, c) * ddt);
+  }
+  return Ek + Eth;
+}
+
+// gbar = J_cool(U1)^T g for the integrators above (U1: pre-cooling state); max(E_floor, x) ties -> the floor
+template <class T>
+__device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Consts<T>& c, const T g[5], T gb[5]) {
+  const T rho = U[0];
+  const T r = rcp_(rho);
+  const T Ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * r;
+  const T Eth0 = U[4] - Ek;
+  const T Efl = rho * c.t_floor * c.inv_gm1;
+  const T dfl = c.t_floor * c.inv_gm1;          // dE_floor / drho
+  const T gE = g[4];
+  T Ethb = T(0), rhob = T(0);                   // cotangents of E_th^0 and rho
+  if (c.cool_mode == 1) {
+    const T rn = cool_rate(Eth0, rho, r, c);
+    const T candp = Eth0 + rn * dt;
+    const bool flp = !(Efl < candp);
+    const T Ep = flp ? Efl : candp;
+    const T rp = cool_rate(Ep, rho, r, c);
+    const T cand = Eth0 + (T(0.5) * dt) * (rn + rp);
+    if (!(Efl < cand)) {
+      rhob += gE * dfl;
+    } else {
+      Ethb += gE;
+      T rnb = T(0.5) * dt * gE;
+      const T rpb = rnb;
+      T Epb = T(0);
+      cool_rate_vjp(Ep, rho, r, c, rpb, Epb, rhob);
+      if (flp) rhob += Epb * dfl; else { Ethb += Epb; rnb += Epb * dt; }
+      cool_rate_vjp(Eth0, rho, r, c, rnb, Ethb, rhob);
+    }
+  } else {
+    const int nsub = c.cool_nsub;
+    const T ddt = dt / T(nsub);
+    T Es[DH_COOL_NSUB_MAX];                     // E_th^k, k = 0 .. nsub-1
+    bool fl_last = false;
+    T Eth = Eth0;
+    for (int k = 0; k < nsub; ++k) {
+      Es[k] = Eth;
+      const T cand = Eth + cool_rate(Eth, rho, r, c) * ddt;
+      fl_last = !(Efl < cand);
+      Eth = fl_last ? Efl : cand;
+    }
+    T eb = gE;                                  // cotangent of E_th^{k+1}
+    for (int k = nsub - 1; k >= 0; --k) {
+      const T cand = Es[k] + cool_rate(Es[k], rho, r, c) * ddt;
+      if (!(Efl < cand)) { rhob += eb * dfl; eb = T(0); break; }   // floored: nothing earlier matters
+      T ekb = eb;
+      cool_rate_vjp(Es[k], rho, r, c, eb * ddt, ekb, rhob);
+      eb = ekb;
+    }
+    Ethb = eb;
+  }
+  // E_out = Ek + E_th^N;  E_th^0 = E - Ek;  Ek = |m|^2 / (2 rho)
+  const T Ekb = gE - Ethb;
   gb[4] = Ethb;
   gb[1] = g[1] + Ekb * U[1] * r;
   gb[2] = g[2] + Ekb * U[2] * r;

@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(256) cool_vjp_kernel(const T* __restrict__ U1,
     T u[5], gi[5], gb[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) { u[f] = U1[f * N + i]; gi[f] = g[f * N + i]; }
-    cool_vjp(u, dt, c, gi, gb);
+    if (c.cool_mode != 0 || c.cool_nsub > 1) cool_vjp_general(u, dt, c, gi, gb); else cool_vjp(u, dt, c, gi, gb);
 #pragma unroll
     for (int f = 0; f < 5; ++f) gout[f * N + i] = gb[f];
   }
@@ -212,6 +212,27 @@ cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cu
   return cudaGetLastError();
 }
 
+// In-place cooling of a finished state for the integrators the stage kernels do not fuse (sub-cycled Eq. 23, trapezoid
+// Eq. 22; DH_OPT_COOL_MODE / DH_OPT_COOL_NSUB): reads the 5 fields, rewrites E.  dt from the device when dt_dev != NULL.
+template <class T>
+__global__ void __launch_bounds__(256) cool_fwd_kernel(T* __restrict__ U, size_t N, T dt_host, const T* __restrict__ dt_dev, Consts<T> c) {
+  const T dt = dt_dev ? *dt_dev : dt_host;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+    T u[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) u[f] = U[f * N + i];
+    U[4 * N + i] = cool_energy_general(u, dt, c);
+  }
+}
+
+template <class T>
+cudaError_t launch_cool_fwd(T* U, size_t N, T dt, const T* dt_dev, const Consts<T>& c, cudaStream_t s) {
+  int blocks = (int)((N + 255) / 256);
+  if (blocks > 148 * 16) blocks = 148 * 16;
+  cool_fwd_kernel<T><<<blocks, 256, 0, s>>>(U, N, dt, dt_dev, c);
+  return cudaGetLastError();
+}
+
 template <class T>
 cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s) {
   int blocks = (int)((N + 255) / 256);
@@ -224,6 +245,8 @@ template cudaError_t launch_stage_naive<float>(const StageParams<float>&, int, i
 template cudaError_t launch_stage_naive<double>(const StageParams<double>&, int, int, cudaStream_t);
 template cudaError_t launch_rev_naive<float>(const RevParams<float>&, int, int, cudaStream_t);
 template cudaError_t launch_rev_naive<double>(const RevParams<double>&, int, int, cudaStream_t);
+template cudaError_t launch_cool_fwd<float>(float*, size_t, float, const float*, const Consts<float>&, cudaStream_t);
+template cudaError_t launch_cool_fwd<double>(double*, size_t, double, const double*, const Consts<double>&, cudaStream_t);
 template cudaError_t launch_cool_vjp<float>(const float*, const float*, float*, size_t, float, const Consts<float>&, cudaStream_t);
 template cudaError_t launch_cool_vjp<double>(const double*, const double*, double*, size_t, double, const Consts<double>&, cudaStream_t);
 

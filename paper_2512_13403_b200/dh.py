@@ -20,10 +20,11 @@ DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, 
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
-    "riemann": 15,
+    "riemann": 15, "cool_mode": 16, "cool_nsub": 17,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
+COOL_MODES = {"euler": 0, "trapezoid": 1}           # DH_OPT_COOL_MODE
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
 KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
 
@@ -34,7 +35,7 @@ SYMBOLS = [
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
     "dh_cfl_stats",
 ]
-KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb"]
+KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb", "cool"]
 
 _lib = None
 
@@ -231,6 +232,8 @@ class Solver:
         for k, v in options.items():
             if k == "limiter" and isinstance(v, str):
                 v = LIMITERS[v]
+            if k == "cool_mode" and isinstance(v, str):
+                v = COOL_MODES[v]
             if k == "riemann" and isinstance(v, str):
                 v = RIEMANN[v]
             if k == "integrator" and isinstance(v, str):

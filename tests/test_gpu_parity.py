@@ -826,3 +826,86 @@ def test_advance_and_adjoint_follow_the_riemann_option(riemann):
     assert torch.equal(Ud, Ua)
     err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
     assert err.max() <= 1e-11, float(err.max())
+
+
+# ------------------------------ sub-cycled and trapezoid cooling (DH_OPT_COOL_MODE / DH_OPT_COOL_NSUB)
+COOL_VARIANTS = [dict(cool_nsub=4), dict(cool_nsub=64), dict(cool_mode="trapezoid")]
+_cool_id = lambda v: "-".join(f"{a}={b}" for a, b in v.items())
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("variant", COOL_VARIANTS, ids=_cool_id)
+def test_step_parity_cooling_integrators(variant, dtype, kernel):
+    """Eq. 23 with N_sub substeps and the trapezoid of Eq. 22 after the hydro step: strong cooling
+    (lambda0 = 200: a share of the cells reaches the floor, some of them mid-way through the substeps), general alpha in
+    one case, ragged shape."""
+    gamma = 5 / 3
+    for alpha in (0.5, 0.7):
+        U = random_state((9, 12, 34), 601, gamma, dtype)
+        kw = dict(cooling=True, lambda0=200.0, alpha=alpha, t_floor=0.3, **variant)
+        p = oracle_params(U, gamma, **kw)
+        s = _solver(U, gamma, kernel=kernel, cooling=1, lambda0=200.0, alpha=alpha, t_floor=0.3, **variant)
+        Ud = U.cuda()
+        dt = s.cfl_dt(Ud)
+        s.step(Ud, dt)
+        ref = oracle.step(U.numpy(), dt, p)
+        assert max_rel_err(Ud.cpu().numpy(), ref) <= TOL[dtype]
+        floor_E = ref[0] * 0.3 / (gamma - 1)
+        eth = ref[4] - 0.5 * (ref[1] ** 2 + ref[2] ** 2 + ref[3] ** 2) / ref[0]
+        frac = float(np.mean(np.abs(eth - floor_E) <= 1e-9 * floor_E))
+        assert 0.02 < frac < 0.98, frac               # both branches of the floor are exercised
+        base = oracle.step(U.numpy(), dt, oracle_params(U, gamma, cooling=True, lambda0=200.0, alpha=alpha, t_floor=0.3))
+        assert np.abs(ref[4] - base[4]).max() > 1e-3  # and the variant is not the default update
+
+
+@pytest.mark.parametrize("integrator", ["vl2", "ssprk3"])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("variant", COOL_VARIANTS, ids=_cool_id)
+def test_vjp_parity_cooling_integrators(variant, dtype, integrator):
+    """cool_vjp_general (reverse sweep over the substeps / through the trapezoid's predictor, floor branches included)
+    against the oracle's dual-number transpose."""
+    U = random_state((8, 10, 14), 611, 5 / 3, dtype)
+    okw = dict(cooling=True, lambda0=100.0, alpha=0.5, t_floor=0.3, integrator=integrator, **variant)
+    skw = dict(cooling=1, lambda0=100.0, t_floor=0.3, integrator=integrator, **variant)
+    _vjp_case(U, 5 / 3, 612, dtype, okw, skw, 1e-12 if dtype == torch.float64 else 1e-4)
+
+
+@pytest.mark.parametrize("variant", COOL_VARIANTS[::2], ids=_cool_id)
+def test_advance_and_adjoint_follow_the_cooling_integrator(variant):
+    """dh_advance (device-resident dt, full CFL reduction each step: the candidate list is not used with a split
+    cooling pass) and dh_adjoint over 4 steps against the oracle's loop; fp32 dh_advance bitwise equal to the host-driven
+    loop."""
+    gamma = 5 / 3
+    U = random_state((9, 10, 70), 621, gamma, torch.float64)
+    kw = dict(cooling=True, lambda0=3.0, alpha=0.5, t_floor=0.3, **variant)
+    p = oracle_params(U, gamma, **kw)
+    g = np.random.default_rng(622).normal(size=tuple(U.shape))
+    Un_ref, g0_ref, dts_ref = oracle.adjoint(U.numpy(), 4, g, p)
+    s = _solver(U, gamma, cooling=1, lambda0=3.0, t_floor=0.3, **variant)
+    Ua = U.cuda()
+    s.advance(Ua, 4)
+    assert max_rel_err(Ua.cpu().numpy(), Un_ref) <= 5e-12
+    Ud, gd = U.cuda(), torch.from_numpy(g).cuda()
+    dts = s.adjoint(Ud, gd, 4, 3)
+    assert dts[0] == dts_ref[0] and np.allclose(dts, dts_ref, rtol=1e-13, atol=0)
+    assert torch.equal(Ud, Ua)
+    err = np.abs(gd.cpu().numpy() - g0_ref) / np.sqrt(np.mean(g0_ref ** 2))
+    assert err.max() <= 1e-11, float(err.max())
+    U32 = random_state((12, 16, 32), 623, gamma, torch.float32).cuda()
+    s32 = _solver(U32, gamma, cooling=1, lambda0=3.0, t_floor=0.3, **variant)
+    a, b = U32.clone(), U32.clone()
+    s32.advance(a, 3)
+    for _ in range(3):
+        s32.step(b, s32.cfl_dt(b))
+    assert torch.equal(a, b)
+
+
+def test_cooling_integrator_option_errors():
+    from paper_2512_13403_b200 import dh
+    U = random_state((4, 4, 4), 631, 1.4, torch.float32)
+    s = _solver(U, 1.4)
+    for key, bad in (("cool_nsub", 0), ("cool_nsub", 65), ("cool_nsub", 2.5), ("cool_mode", 2), ("riemann", 3)):
+        with pytest.raises(dh.DhError):
+            s.set_options(**{key: bad})
+    assert s.get_option("cool_nsub") == 1 and s.get_option("cool_mode") == 0
