@@ -1,7 +1,7 @@
 """CPU oracle of the periodic multigrid Poisson solver of arxiv/paper_2512_13403 §6.2 and Appendix C — TEST
 INFRASTRUCTURE ONLY (plain numpy, fp64, one array operation per printed formula; no blocking, no fusion).  Only
 tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference legs may import it; it shares no code with
-the CUDA path (paper_2512_13403_b200/csrc/dh_poisson.cu).
+the CUDA path.
 
 Arrays are [nz, ny, nx] (x fastest), cubic cells of size h, periodic in every direction.
 
@@ -19,8 +19,8 @@ Readings (A21-A23):
   A21  Eq. 40 as printed has (1-omega)/6 in front of phi, which contradicts Eq. 39; Eq. 39 is followed:
        phi_new = (1-omega) phi + (omega/6) (sum of the six neighbours - h^2 F).
   A22  "direct solver on the coarse grid" (Fig. 9): A is singular on the torus.  Levels coarsen by 2 while every
-       extent is even and > 2; the coarsest level is solved by `nu_coarse` Jacobi sweeps from zero (default 64), which
-       (4^3 for power-of-two grids, where the slowest mode contracts by 0.78 per sweep).
+       extent is even and > 2; the coarsest level is solved by `nu_coarse` Jacobi sweeps from zero (default 64;
+       4^3 for power-of-two grids, where the slowest mode contracts by 0.78 per sweep).
   A23  F must have zero mean for A phi = F to be solvable: solve() removes the mean of F and returns the zero-mean phi.
 """
 from __future__ import annotations
