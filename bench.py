@@ -60,6 +60,9 @@ def parse_args():
     ap.add_argument("--integrator", choices=["vl2", "heun", "ssprk3"], default="vl2",
                     help="vl2 = the predictor / corrector of Eqs. A6-A7 (BASELINE's metric); heun, ssprk3: SURVEY 8(f) item 2")
     ap.add_argument("--adjoint", type=int, default=0, help="also time dh_adjoint over this many steps (checkpointed multi-step adjoint)")
+    ap.add_argument("--poisson", type=int, default=0, metavar="N",
+                    help="instead of the hydro step: time multigrid cycles of the periodic Poisson solver on an N^3 grid (SURVEY 8(f) item 3)")
+    ap.add_argument("--mg-cycle", choices=["V", "W"], default="V")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -467,9 +470,99 @@ def run_dh(a):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------- multigrid Poisson (--poisson N)
+MG_WORDS_PER_CELL_CYCLE = (4 * 3 + 2.125 + 2.125) * 8.0 / 7.0   # nu1 = nu2 = 2 sweeps x (in, F, out) + fused
+#   residual/restriction (phi, F, 1/8 out) + prolongation/correction (phi in, phi out, 1/8 in), all levels: x 8/7
+
+
+def run_poisson(a):
+    """K cycles of dh_mg_cycle on an N^3 fp32 grid (one JSON line; single GPU; the oracle's cycle timed on a 64^3 grid)."""
+    import numpy as np
+    import torch
+
+    from paper_2512_13403_b200 import dh
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --poisson needs a CUDA device: the path has no CPU fallback")
+    n, K, W = a.poisson, a.steps, max(a.warmup, 3)
+    torch.cuda.set_device(0)
+    gen = torch.Generator(device="cuda").manual_seed(1006)
+    F = torch.randn((n, n, n), generator=gen, device="cuda", dtype=torch.float32)
+    F -= F.mean()
+    phi = torch.zeros_like(F)
+    s = dh.Multigrid(n, n, n, 1.0 / n, dtype=torch.float32, cycle=a.mg_cycle)
+    for _ in range(W):
+        s.cycle(phi, F)
+    phi.zero_()
+    torch.cuda.synchronize()
+    l0 = s.launches
+    sampler = ClockSampler(0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.time()
+    e0.record()
+    for _ in range(K):
+        s.cycle(phi, F)
+    e1.record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(t0, t1)
+    launches = s.launches - l0
+    N = n ** 3
+    peak, peak_src = measured_peak()
+    gbs = MG_WORDS_PER_CELL_CYCLE * 4.0 * N * K / (ms * 1e-3) / 1e9
+    line = {"metric": f"cell-cycles/s (multigrid {a.mg_cycle}-cycle of the periodic Poisson solver, nu1 = nu2 = 2)", "value": N * K / (ms * 1e-3),
+            "unit": "cell-cycles/s", "n_gpus": 1, "steps": K, "warmup": W, "ms_per_step": ms / K, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"poisson_multigrid_{n}^3_fp32 (white-noise zero-mean source, seed 1006)", "grid": [n, n, n], "cycle": a.mg_cycle,
+                       "levels": s.levels, "nu1": 2, "nu2": 2, "nu_coarse": 64, "omega": 2.0 / 3.0, "call": "dh_mg_cycle(phi, F) x K (CUDA graph replay)",
+                       "l2": f"inputs larger than L2 ({2 * 4 * N / 1e6:.0f} MB vs 126 MB), no flush" if 8 * N > 126e6 else "working set fits L2: not an HBM number"},
+            "roofline": {"bound": "hbm", "kernel": "whole cycle (Jacobi sweeps dominate: 12 of 16.25 words per fine cell)", "achieved": gbs, "peak": peak,
+                         "unit": "GB/s", "frac": gbs / peak, "peak_source": peak_src, "traffic": None,
+                         "words_per_cell_cycle": MG_WORDS_PER_CELL_CYCLE},
+            "clocks": clocks, "gpu_launches": launches}
+    # convergence actually reached by the timed cycles (a property check, not a timing)
+    r = F - (sum(torch.roll(phi, sh, d) for d in range(3) for sh in (1, -1)) - 6 * phi) * float(n * n)
+    line["config"]["rel_residual_after_K_cycles"] = float(r.norm() / F.norm())
+    if not a.no_e2e:
+        hF = F.cpu().pin_memory()
+        hphi = torch.empty_like(hF).pin_memory()
+        dF, dphi = torch.empty_like(F), torch.empty_like(F)
+        ncyc = 8
+        t_best = None
+        for _ in range(3):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            dF.copy_(hF, non_blocking=True)
+            dh.dh_mg_solve(s.ctx, dF.data_ptr(), dphi.data_ptr(), ncyc, False)
+            hphi.copy_(dphi, non_blocking=True)
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
+            t_best = dt if t_best is None else min(t_best, dt)
+        line["e2e"] = {"value": N * ncyc / t_best, "unit": "cell-cycles/s", "h2d_bytes_per_step": 4 * N, "d2h_bytes_per_step": 4 * N,
+                       "ms_per_step": t_best * 1e3, "call": f"pinned host F -> device, dh_mg_solve({ncyc} cycles), phi -> pinned host"}
+    if not a.no_cpu:
+        from oracle import poisson as omg
+        m = min(64, n)
+        Fc = np.random.default_rng(1006).normal(size=(m, m, m))
+        Fc -= Fc.mean()
+        t0 = time.perf_counter()
+        reps = 0
+        x = np.zeros_like(Fc)
+        while time.perf_counter() - t0 < 10.0:
+            x = omg.cycle(x, Fc, 1.0 / m, gamma={"V": 1, "W": 2}[a.mg_cycle])
+            reps += 1
+        tc = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": m ** 3 * reps / tc, "unit": "cell-cycles/s", "cores": 1, "kind": "oracle",
+                                "sample": f"{reps} cycles of oracle.poisson.cycle on a {m}^3 grid ({tc:.1f} s, numpy fp64)"}
+    print(json.dumps(line))
+
+
 def main():
     a = parse_args()
-    if a.impl == "reference":
+    if a.poisson:
+        run_poisson(a)
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_dh(a)

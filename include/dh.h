@@ -197,6 +197,50 @@ const char* dh_last_error(void);
 /* Library version string, e.g. "dh 0.1 sm_100a". */
 const char* dh_version(void);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * Periodic multigrid Poisson solver (§6.2 Eqs. 37-48, Appendix C Eqs. C10-C12).
+ *
+ * Solves A phi = F on the nx x ny x nz torus with cubic cells of size h, A the seven-point Laplacian of Eq. 38
+ * (PAPER.md:475).  One cycle = nu1 weighted-Jacobi sweeps (Eq. 39; omega = 2/3), residual (Eq. 41) and
+ * 8-cell full-weighting restriction (Eq. 42), gamma recursive visits of the coarse level (1: V-cycle, 2: W-cycle, Eq. C12),
+ * trilinear prolongation and correction (Eqs. 44-45), nu2 sweeps.  Levels coarsen by 2 while every extent is even and > 2;
+ * the coarsest level gets nu_coarse sweeps (readings A21-A23).
+ *
+ * Arrays: DEVICE pointers, contiguous [nz][ny][nx] of the context's dtype, 32-byte aligned, owned by the caller, not
+ * retained past the call (stream ordered).  The library owns the level hierarchy (about 1.6 extra arrays), allocated in
+ * dh_mg_create.  Errors: return code + dh_last_error(); no CPU fallback.  One context per stream, not re-entrant.
+ * ------------------------------------------------------------------------------------------------------------------ */
+typedef struct dh_mg dh_mg;
+
+enum {
+  DH_MG_NU1 = 0,        /* pre-smoothing sweeps, default 2 */
+  DH_MG_NU2 = 1,        /* post-smoothing sweeps, default 2 */
+  DH_MG_GAMMA = 2,      /* 1 V-cycle (default), 2 W-cycle (the paper's default for gravity) */
+  DH_MG_NU_COARSE = 3,  /* Jacobi sweeps on the coarsest level, default 64 */
+  DH_MG_OMEGA = 4,      /* Jacobi weight, default 2/3 */
+  DH_MG_GRAPH = 5       /* 1 (default) / 0: replay each cycle as a CUDA graph captured once per (phi, F, options) */
+};
+
+dh_mg* dh_mg_create(int nx, int ny, int nz, double h, int dtype);   /* NULL on failure (dh_last_error) */
+void dh_mg_destroy(dh_mg* ctx);
+int dh_mg_set_stream(dh_mg* ctx, void* cuda_stream);                /* default: legacy stream 0 */
+int dh_mg_set_option(dh_mg* ctx, int key, double value);
+int dh_mg_levels(const dh_mg* ctx);                                 /* number of grid levels incl. the finest */
+long long dh_mg_launches(const dh_mg* ctx);                         /* kernels launched so far (graph nodes counted) */
+
+/* One cycle for A phi = F, in place on phi (in: current iterate, out: next iterate).  F is used as given (it should have
+ * zero mean).  Asynchronous on the context's stream. */
+int dh_mg_cycle(dh_mg* ctx, void* phi, const void* F);
+
+/* phi = result of `ncycles` cycles from phi = 0 for the zero-mean part of F, mean of phi removed (reading A23).  phi is
+ * overwritten, F untouched.  If rel_residual (HOST pointer) is not NULL the call synchronises the stream and stores
+ * |F0 - A phi| / |F0| there; otherwise it is asynchronous. */
+int dh_mg_solve(dh_mg* ctx, const void* F, void* phi, int ncycles, double* rel_residual);
+
+/* VJP of the converged solve with respect to F (Eqs. 46-48): g_F = A^-1 g_phi, another solve; nothing of
+ * the forward solve is stored. */
+int dh_mg_solve_vjp(dh_mg* ctx, const void* g_phi, void* g_F, int ncycles, double* rel_residual);
+
 #ifdef __cplusplus
 }
 #endif

@@ -20,7 +20,7 @@ Readings (A21-A23):
        phi_new = (1-omega) phi + (omega/6) (sum of the six neighbours - h^2 F).
   A22  "direct solver on the coarse grid" (Fig. 9): A is singular on the torus.  Levels coarsen by 2 while every
        extent is even and > 2; the coarsest level is solved by `nu_coarse` Jacobi sweeps from zero (default 64;
-       4^3 for power-of-two grids, where the slowest mode contracts by 0.78 per sweep).
+       2^3 for power-of-two grids, where the slowest mode contracts by 0.56 per sweep).
   A23  F must have zero mean for A phi = F to be solvable: solve() removes the mean of F and returns the zero-mean phi.
 """
 from __future__ import annotations

@@ -32,6 +32,10 @@ static int cuda_fail(cudaError_t e, const char* where) {
 
 namespace dh {
 size_t elem_size(const Ctx* c) { return c->dtype == DH_F32 ? 4 : 8; }
+void set_error(const char* where, const char* detail) {   // for the other translation units of the library
+  if (detail && detail[0]) snprintf(g_err, sizeof(g_err), "%s: %s", where, detail);
+  else snprintf(g_err, sizeof(g_err), "%s", where);
+}
 }  // namespace dh
 
 static size_t state_bytes(const dh_ctx* c) { return 5 * c->N * elem_size(c); }

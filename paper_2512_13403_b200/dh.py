@@ -34,7 +34,11 @@ SYMBOLS = [
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
     "dh_cfl_stats",
+    "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
+    "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
+MG_OPTIONS = {"nu1": 0, "nu2": 1, "gamma": 2, "nu_coarse": 3, "omega": 4, "graph": 5}
+MG_CYCLES = {"V": 1, "W": 2}
 KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb", "cool"]
 
 _lib = None
@@ -83,6 +87,20 @@ def load(rebuild: bool = False):
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
                "dh_step", "dh_step_devdt", "dh_step_vjp", "dh_run_host", "dh_advance", "dh_adjoint", "dh_step_vjp_host", "dh_profile_enable",
                "dh_profile_read"):
+        getattr(lib, fn).restype = ci
+    lib.dh_mg_create.restype = vp
+    lib.dh_mg_create.argtypes = [ci, ci, ci, cd, ci]
+    lib.dh_mg_destroy.restype = None
+    lib.dh_mg_destroy.argtypes = [vp]
+    lib.dh_mg_set_stream.argtypes = [vp, vp]
+    lib.dh_mg_set_option.argtypes = [vp, ci, cd]
+    lib.dh_mg_levels.argtypes = [vp]
+    lib.dh_mg_launches.argtypes = [vp]
+    lib.dh_mg_launches.restype = ctypes.c_longlong
+    lib.dh_mg_cycle.argtypes = [vp, vp, vp]
+    lib.dh_mg_solve.argtypes = [vp, vp, vp, ci, pd]
+    lib.dh_mg_solve_vjp.argtypes = [vp, vp, vp, ci, pd]
+    for fn in ("dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp"):
         getattr(lib, fn).restype = ci
     _lib = lib
     return lib
@@ -313,3 +331,114 @@ class Solver:
             self.close()
         except Exception:
             pass
+
+
+# ------------------------------------------------------------------ multigrid Poisson solver (§6.2)
+def dh_mg_create(nx: int, ny: int, nz: int, h: float, dtype: int):
+    p = load().dh_mg_create(int(nx), int(ny), int(nz), float(h), int(dtype))
+    if not p:
+        raise DhError(DH_ERR_ARG, dh_last_error())
+    return p
+
+
+def dh_mg_destroy(ctx) -> None:
+    load().dh_mg_destroy(ctx)
+
+
+def dh_mg_set_stream(ctx, cuda_stream: int) -> None:
+    _check(load().dh_mg_set_stream(ctx, ctypes.c_void_p(cuda_stream)))
+
+
+def dh_mg_set_option(ctx, key: int, value: float) -> None:
+    _check(load().dh_mg_set_option(ctx, int(key), float(value)))
+
+
+def dh_mg_levels(ctx) -> int:
+    return int(load().dh_mg_levels(ctx))
+
+
+def dh_mg_launches(ctx) -> int:
+    return int(load().dh_mg_launches(ctx))
+
+
+def dh_mg_cycle(ctx, phi_ptr: int, F_ptr: int) -> None:
+    _check(load().dh_mg_cycle(ctx, ctypes.c_void_p(phi_ptr), ctypes.c_void_p(F_ptr)))
+
+
+def dh_mg_solve(ctx, F_ptr: int, phi_ptr: int, ncycles: int, want_residual: bool = True):
+    r = ctypes.c_double(0.0)
+    _check(load().dh_mg_solve(ctx, ctypes.c_void_p(F_ptr), ctypes.c_void_p(phi_ptr), int(ncycles), ctypes.byref(r) if want_residual else None))
+    return r.value if want_residual else None
+
+
+def dh_mg_solve_vjp(ctx, g_phi_ptr: int, g_F_ptr: int, ncycles: int, want_residual: bool = True):
+    r = ctypes.c_double(0.0)
+    _check(load().dh_mg_solve_vjp(ctx, ctypes.c_void_p(g_phi_ptr), ctypes.c_void_p(g_F_ptr), int(ncycles), ctypes.byref(r) if want_residual else None))
+    return r.value if want_residual else None
+
+
+class Multigrid:
+    """Thin owner of a dh_mg context for [nz, ny, nx] torch CUDA tensors (argument marshalling only)."""
+
+    def __init__(self, nx: int, ny: int, nz: int, h: float, dtype=None, stream=None, **options):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("dh.Multigrid needs a CUDA device: the path has no CPU fallback")
+        dtype = dtype or torch.float32
+        self.shape, self.dtype, self.h = (nz, ny, nx), dtype, float(h)
+        self.ctx = dh_mg_create(nx, ny, nz, h, DH_F32 if dtype == torch.float32 else DH_F64)
+        stream = stream if stream is not None else torch.cuda.current_stream()
+        dh_mg_set_stream(self.ctx, stream.cuda_stream)
+        self.set_options(**options)
+
+    def set_options(self, **options):
+        for k, v in options.items():
+            if k == "cycle":
+                k, v = "gamma", MG_CYCLES[v]
+            dh_mg_set_option(self.ctx, MG_OPTIONS[k], float(v))
+
+    def _chk(self, *ts):
+        for t in ts:
+            if not (t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape):
+                raise ValueError(f"expected a contiguous CUDA {self.dtype} tensor of shape {self.shape}")
+
+    @property
+    def levels(self) -> int:
+        return dh_mg_levels(self.ctx)
+
+    @property
+    def launches(self) -> int:
+        return dh_mg_launches(self.ctx)
+
+    def cycle(self, phi, F) -> None:
+        self._chk(phi, F)
+        dh_mg_cycle(self.ctx, phi.data_ptr(), F.data_ptr())
+
+    def solve(self, F, ncycles: int = 10, want_residual: bool = True):
+        import torch
+
+        self._chk(F)
+        phi = torch.empty_like(F)
+        rel = dh_mg_solve(self.ctx, F.data_ptr(), phi.data_ptr(), ncycles, want_residual)
+        return phi, rel
+
+    def solve_vjp(self, g_phi, ncycles: int = 10, want_residual: bool = True):
+        import torch
+
+        self._chk(g_phi)
+        g_F = torch.empty_like(g_phi)
+        rel = dh_mg_solve_vjp(self.ctx, g_phi.data_ptr(), g_F.data_ptr(), ncycles, want_residual)
+        return g_F, rel
+
+    def close(self):
+        if getattr(self, "ctx", None):
+            dh_mg_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
