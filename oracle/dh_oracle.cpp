@@ -120,4 +120,15 @@ int dho_reconstruct(int n, const Params* p, const double* W, double* WL, double*
 
 double dho_limiter(double a, double b, int kind) { return limiter<double>(a, b, kind); }
 
+// Eqs. 20-21: min_x t_cool(x) in double, and the limited dt compared in the array's type
+int dho_cool_dt(int nx, int ny, int nz, const Params* p, int dtype, const void* U, double dt_hydro, double c_cool,
+                double dt_max, double* tmin_out, double* dt_out) {
+  Grid g = mkgrid(nx, ny, nz);
+  double tmin = dtype == 0 ? t_cool_min<float>(g, *p, (const float*)U) : t_cool_min<double>(g, *p, (const double*)U);
+  *tmin_out = tmin;
+  *dt_out = dtype == 0 ? limited_dt<float>(dt_hydro, tmin, c_cool, dt_max) : limited_dt<double>(dt_hydro, tmin, c_cool, dt_max);
+  return 0;
+}
+
 }  // extern "C"
+

@@ -18,6 +18,7 @@
 // PAPER.md:96-104), i (x) fastest, periodic in all three directions.
 #pragma once
 #include <cmath>
+#include <limits>
 #include <cstddef>
 #include <vector>
 
@@ -541,6 +542,48 @@ int cfl_dt(const Grid& g, const Params& p, double cfl, const T* U, double* dt_ou
   T dt = (T)cfl * best;
   *dt_out = (double)dt;
   return 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Cooling-time limit on the time step, Eqs. 20-21.
+//   t_cool(x) = |E_th| / |n_H Gamma - n_H^2 Lambda|                                          (Eq. 20)
+//   dt <= min(dt_hydro, c_cool min_x t_cool(x), dt_max)                                       (Eq. 21)
+// Code units of this file (reading A10): n_H = rho, Gamma = 0, Lambda = lambda0 T^alpha, T = (gamma-1) E_th / rho,
+// so the denominator is |Edot| of cool_rate().  Reading A24: E_th is taken from the conserved variables exactly as
+// cool() does (no floors); the per-cell quotient is formed in double whatever the array type (the power function has
+// no bit-exact definition to share, unlike the recipe of Eq. A8); a cell with zero rate (T <= 0) has t_cool = +inf
+// and never decides the minimum; cells already on the temperature floor are NOT exempted (the paper exempts none).
+// The three candidates of Eq. 21 are compared in T: dt = min(dt_hydro, T(c_cool * tmin), T(dt_max)); c_cool <= 0
+// or dt_max <= 0 switches that candidate off.
+// ------------------------------------------------------------------------------------------------
+inline double t_cool_cell(const double U[5], const Params& p) {
+  double rho = U[0];
+  double Ek = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
+  double Eth = U[4] - Ek;
+  double Edot = cool_rate<double>(Eth, rho, p);
+  if (Edot == 0.0) return std::numeric_limits<double>::infinity();
+  return std::fabs(Eth) / std::fabs(Edot);
+}
+
+template <class T>
+double t_cool_min(const Grid& g, const Params& p, const T* U) {
+  const size_t N = g.N();
+  double best = std::numeric_limits<double>::infinity();
+  for (size_t c = 0; c < N; ++c) {
+    double u[5];
+    for (int f = 0; f < 5; ++f) u[f] = (double)U[f * N + c];
+    double t = t_cool_cell(u, p);
+    if (t < best) best = t;
+  }
+  return best;
+}
+
+template <class T>
+double limited_dt(double dt_hydro, double tmin, double c_cool, double dt_max) {
+  T dt = (T)dt_hydro;
+  if (c_cool > 0.0) { T dc = (T)(c_cool * tmin); if (dc < dt) dt = dc; }
+  if (dt_max > 0.0) { T dm = (T)dt_max; if (dm < dt) dt = dm; }
+  return (double)dt;
 }
 
 }  // namespace dho

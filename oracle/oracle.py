@@ -134,6 +134,20 @@ def cfl_dt(U, p, cfl=0.4):
     return dt.value, np.array(list(smax))
 
 
+def cool_dt(U, p, dt_hydro, c_cool=0.0, dt_max=0.0):
+    """Eqs. 20-21: (min_x t_cool(x), min(dt_hydro, c_cool * that, dt_max)); t_cool in double,
+    the three candidates compared in the array's dtype (reading A24); c_cool <= 0 / dt_max <= 0 switch a candidate off."""
+    lib = _load()
+    U = np.ascontiguousarray(U)
+    assert U.dtype in (np.float32, np.float64)
+    tmin = ctypes.c_double(0.0)
+    dt = ctypes.c_double(0.0)
+    lib.dho_cool_dt(*_dims(U), ctypes.byref(p), ctypes.c_int(0 if U.dtype == np.float32 else 1), _ptr(U),
+                    ctypes.c_double(dt_hydro), ctypes.c_double(c_cool), ctypes.c_double(dt_max),
+                    ctypes.byref(tmin), ctypes.byref(dt))
+    return tmin.value, dt.value
+
+
 def prims(U, p):
     lib = _load()
     U = _f64(U)
