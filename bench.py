@@ -52,6 +52,7 @@ def parse_args():
     ap.add_argument("--cooling", type=int, default=0, help="1: configs[3]'s cooling source in the corrector epilogue")
     ap.add_argument("--cool-mode", choices=["euler", "trapezoid"], default="euler", help="DH_OPT_COOL_MODE (PAPER.md:318-325), with --cooling 1")
     ap.add_argument("--cool-nsub", type=int, default=1, help="DH_OPT_COOL_NSUB: substeps of Eq. 23, with --cooling 1")
+    ap.add_argument("--c-cool", type=float, default=0.0, help="DH_OPT_C_COOL: c_cool of Eq. 21 (PAPER.md:314), with --cooling 1; 0 = no cooling-time limit")
     ap.add_argument("--mach", type=float, default=2.0)
     ap.add_argument("--kernel", default="fused", choices=["fused", "gather"])
     ap.add_argument("--no-chain", action="store_true", help="one dh_cfl_dt_async + dh_step_devdt pair per step instead of one dh_advance call")
@@ -260,7 +261,7 @@ def run_dh(a):
 
     s = dh.Solver(n, n, n, gamma=wl.gamma, dtype=torch.float32, kernel=a.kernel, cooling=int(a.cooling),
                   lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator, riemann=a.riemann, limiter=a.limiter,
-                  cool_mode=a.cool_mode, cool_nsub=a.cool_nsub)
+                  cool_mode=a.cool_mode, cool_nsub=a.cool_nsub, c_cool=a.c_cool)
     # algorithmic words per cell of one step: CFL 5 + per stage (5 in [+ 5 base] + 5 out) + per combination 15
     fwd_words = {"vl2": FWD_WORDS, "heun": 5 + 10 + 15 + 15, "ssprk3": 5 + 10 + 15 + 15 + 15 + 15}[a.integrator]
 
@@ -365,7 +366,7 @@ def run_dh(a):
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_name(a), "grid": [n, n, n], "cells_per_gpu": N, "gamma": wl.gamma,
                        "cfl": 0.4, "limiter": a.limiter, "riemann": a.riemann, "integrator": {"vl2": "rk2 predictor/corrector", "heun": "heun rk2", "ssprk3": "ssprk3"}[a.integrator],
-                       "cooling": bool(a.cooling), "cool_mode": a.cool_mode, "cool_nsub": a.cool_nsub, "kernel": a.kernel,
+                       "cooling": bool(a.cooling), "cool_mode": a.cool_mode, "cool_nsub": a.cool_nsub, "c_cool": a.c_cool, "kernel": a.kernel,
                        "call": "dh_cfl_dt_async + dh_step_devdt per step" if a.no_chain else "dh_advance(U, K): K x (CFL reduce, dt epilogue, predictor, corrector)", "parallelism": f"replicas x{world}",
                        "l2": "state fits in L2: a 512 MB buffer is written between iterations (outside the event pairs)"
                        if fits_l2 else f"inputs larger than L2 ({5 * 4 * N / 1e6:.0f} MB per state vs 126 MB), no flush",

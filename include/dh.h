@@ -88,6 +88,14 @@ enum {
                             floored energy (reading A20).  (0, N_sub = 1) runs in the last stage's epilogue; the others
                             as one streaming pass over the finished state (DH_K_COOL) */
   DH_OPT_COOL_NSUB = 17, /* N_sub of Eq. 23: integer in 1 .. 64, default 1; substeps dt / N_sub, rate and floor every substep */
+  DH_OPT_C_COOL = 18,    /* c_cool of Eq. 21, finite >= 0, default 0 = no cooling-time limit.  With DH_OPT_COOLING = 1 and
+                            c_cool > 0 every CFL pass (dh_cfl_dt, dh_cfl_dt_async, dh_advance, dh_adjoint, dh_run_host) also reduces
+                            min_x t_cool(x) of Eq. 20 in the same sweep over the five fields (no extra HBM traffic) and returns
+                            dt = min(dt_hydro, c_cool min_x t_cool, dt_max).  Code units of DH_OPT_COOLING: n_H = rho, Gamma = 0,
+                            t_cool = |E_th| / (rho^2 Lambda0 max(T,0)^alpha), formed in fp64 whatever the dtype; cells with zero
+                            rate do not count; the candidates are compared in the dtype (reading A24).  dt is
+                            bit-identical to Eq. A8 whenever the hydro candidate is the smallest */
+  DH_OPT_DT_MAX = 19,    /* Delta t_max of Eq. 21, finite >= 0, default 0 = none; applies with or without cooling */
   DH_OPT_COUNT_
 };
 
@@ -110,6 +118,12 @@ int dh_get_option(const dh_ctx* ctx, int key, double* value_out);
  * dt_out: HOST; receives the T value widened exactly.  Synchronises the stream (the only host sync of
  * the path).  Returns DH_ERR_NONFINITE (and leaves *dt_out untouched) if any input or speed is NaN/Inf. */
 int dh_cfl_dt(dh_ctx* ctx, const void* U, double* dt_out);
+
+/* min_x t_cool(x), Eq. 20, for the cooling parameters of the context (DH_OPT_LAMBDA0 / DH_OPT_ALPHA; DH_OPT_COOLING
+ * need not be on): one pass of the CFL reduction kernel with the cooling-time branch.  U: DEVICE, read only.
+ * tcool_min_out: HOST (+inf if no cell cools).  dt_hydro_out: HOST or NULL, the Eq. A8 value of the same pass.  Like dh_cfl_dt
+ * it synchronises the stream, leaves the dt of Eq. 21 in the context's device slot, and returns DH_ERR_NONFINITE on NaN/Inf. */
+int dh_cool_tmin(dh_ctx* ctx, const void* U, double* tcool_min_out, double* dt_hydro_out);
 
 /* One step in place, U^n -> U^{n+1} (stage 1 into the library's U* scratch, stage 2 back into U, cooling
  * in the stage-2 epilogue if enabled).  U: DEVICE, read and overwritten.  dt > 0 finite.  Asynchronous on

@@ -121,18 +121,22 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->gamma = gamma;
   c->cfl = 0.4;
   c->L[0] = c->L[1] = c->L[2] = 1.0;
-  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->cool_mode = 0; c->cool_nsub = 1; c->fuse_cfl = 1;
+  c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->cool_mode = 0; c->cool_nsub = 1; c->fuse_cfl = 1; c->c_cool = 0.0; c->dt_max = 0.0;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
   if (c->sm_count <= 0) c->sm_count = 148;
   bool ok = cudaMalloc(&c->Us, state_bytes(c)) == cudaSuccess;
-  ok = ok && cudaMalloc((void**)&c->acc, 4 * sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && cudaMalloc((void**)&c->acc, 8 * sizeof(unsigned long long)) == cudaSuccess;
   ok = ok && cudaMalloc(&c->dt_dev, 8) == cudaSuccess;
   ok = ok && cudaMalloc((void**)&c->result_dev, sizeof(CflResult)) == cudaSuccess;
   ok = ok && cudaMallocHost((void**)&c->result_host, sizeof(CflResult)) == cudaSuccess;
-  ok = ok && cudaMemset(c->acc, 0, 4 * sizeof(unsigned long long)) == cudaSuccess;
+  ok = ok && cudaMemset(c->acc, 0, 8 * sizeof(unsigned long long)) == cudaSuccess;
+  {
+    const unsigned long long inf_bits = 0x7ff0000000000000ull;   // slot [4]: running min of t_cool (Eq. 20), armed with +inf
+    ok = ok && cudaMemcpy(c->acc + 4, &inf_bits, sizeof(inf_bits), cudaMemcpyHostToDevice) == cudaSuccess;
+  }
   ok = ok && cudaMemset(c->dt_dev, 0, 8) == cudaSuccess;
   ok = ok && cudaMemset(c->result_dev, 0, sizeof(CflResult)) == cudaSuccess;
   if (!ok) {
@@ -182,6 +186,8 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
     case DH_OPT_FUSE_CFL: c->fuse_cfl = (v != 0.0); break;
+    case DH_OPT_C_COOL: if (!(v >= 0.0) || !isfinite(v)) return fail(DH_ERR_ARG, "dh_set_option: c_cool must be finite and >= 0%s"); c->c_cool = v; break;
+    case DH_OPT_DT_MAX: if (!(v >= 0.0) || !isfinite(v)) return fail(DH_ERR_ARG, "dh_set_option: dt_max must be finite and >= 0%s"); c->dt_max = v; break;
     case DH_OPT_RIEMANN: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: riemann must be 0, 1 or 2%s"); c->riemann = (int)v; break;
     case DH_OPT_COOL_MODE: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: cool_mode must be 0 or 1%s"); c->cool_mode = (int)v; break;
     case DH_OPT_COOL_NSUB:
@@ -208,6 +214,8 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_REV_SLAB: *out = c->rev_slab_opt; break;
     case DH_OPT_INTEGRATOR: *out = c->integrator; break;
     case DH_OPT_FUSE_CFL: *out = c->fuse_cfl; break;
+    case DH_OPT_C_COOL: *out = c->c_cool; break;
+    case DH_OPT_DT_MAX: *out = c->dt_max; break;
     case DH_OPT_RIEMANN: *out = c->riemann; break;
     case DH_OPT_COOL_MODE: *out = c->cool_mode; break;
     case DH_OPT_COOL_NSUB: *out = c->cool_nsub; break;
@@ -249,8 +257,12 @@ int dh_profile_read(dh_ctx* c, double* ms_out, unsigned long long* launches_out)
 // cand: the state was written by a last stage that pushed its CFL candidates (dh_advance): exact recipe on those
 // packs, then the full reduction only if they do not settle the maxima
 template <class T>
-static int cfl_launch(dh_ctx* c, const void* U, bool cand = false) {
+static int cfl_launch(dh_ctx* c, const void* U, bool cand = false, bool force_tcool = false) {
   CflParams<T> p;
+  // Eq. 21: the reduction also evaluates Eq. 20 when cooling is on and c_cool > 0 (or for dh_cool_tmin)
+  p.cool_lim = (force_tcool || (c->cooling != 0 && c->c_cool > 0.0)) ? 1 : 0;
+  p.gm1d = c->gamma - 1.0; p.lambda0 = c->lambda0; p.alpha = c->alpha; p.c_cool = c->cooling != 0 ? c->c_cool : 0.0; p.dt_max = c->dt_max;
+  if (p.cool_lim) cand = false;
   p.U = (const T*)U;
   p.N = c->N;
   p.gamma = (T)c->gamma;
@@ -595,7 +607,8 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
   if (U == c->Us) return fail(DH_ERR_ARG, "dh_advance: U aliases library scratch%s");
   const bool f32 = c->dtype == DH_F32;
   // From the second step on, the CFL pass runs on the candidates the previous last stage pushed (DH_OPT_FUSE_CFL)
-  const bool fuse = c->fuse_cfl && nsteps > 1 && c->kernel == 0;
+  // (not with the cooling-time limit of Eq. 21: t_cool needs every cell, so the full pass runs anyway)
+  const bool fuse = c->fuse_cfl && nsteps > 1 && c->kernel == 0 && !(c->cooling != 0 && c->c_cool > 0.0);
   if (fuse) {
     if (!c->cand_list) {
       c->cand_cap = 1u << 20;
@@ -622,6 +635,17 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
   }
   c->cand_ok = 0;
   if (dt_last_out) return dh_poll_status(c, dt_last_out);
+  return DH_OK;
+}
+
+int dh_cool_tmin(dh_ctx* c, const void* U, double* tcool_min_out, double* dt_hydro_out) {
+  if (!c || !U || !tcool_min_out) return fail(DH_ERR_ARG, "dh_cool_tmin: NULL argument%s");
+  int rc = c->dtype == DH_F32 ? cfl_launch<float>(c, U, false, true) : cfl_launch<double>(c, U, false, true);
+  if (rc) return rc;
+  rc = dh_poll_status(c, nullptr);
+  if (rc) return rc;
+  *tcool_min_out = c->result_host->tcool_min;
+  if (dt_hydro_out) *dt_hydro_out = c->result_host->dt_hydro;
   return DH_OK;
 }
 

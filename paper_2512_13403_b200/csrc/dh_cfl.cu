@@ -47,20 +47,111 @@ __device__ __forceinline__ void cell_speeds(T rho, T mx, T my, T mz, T E, const 
   sz = (az > sz) ? az : sz;
 }
 
+// Eq. 20 for one cell in the code units of reading A10, in double whatever T (reading A24); the
+// operations and their order are those of cool() / cool_rate() of the cooling update, never contracted.
+template <class T>
+__device__ __forceinline__ void cell_tcool(T rho_, T mx_, T my_, T mz_, T E_, const CflParams<T>& p, double& tmin) {
+  const double rho = (double)rho_, mx = (double)mx_, my = (double)my_, mz = (double)mz_, E = (double)E_;
+  const double q = Ieee::add(Ieee::add(Ieee::mul(mx, mx), Ieee::mul(my, my)), Ieee::mul(mz, mz));
+  const double Ek = Ieee::div(Ieee::mul(0.5, q), rho);
+  const double Eth = Ieee::sub(E, Ek);
+  const double Tc = Ieee::div(Ieee::mul(p.gm1d, Eth), rho);
+  const double Tpos = (Tc > 0.0) ? Tc : 0.0;
+  const double rate = Ieee::mul(Ieee::mul(Ieee::mul(rho, rho), p.lambda0), pow(Tpos, p.alpha));
+  const double t = Ieee::div(fabs(Eth), fabs(rate));
+  if (rate != 0.0 && t < tmin) tmin = t;
+}
+
+// fp32 screen in front of cell_tcool (whose fp64 power function would make the pass ALU bound: 1.92 ms instead of the 0.41 ms
+// the 20 B/cell take at 512^3).  Any exact t_cool already evaluated is an upper bound of the global minimum, so a cell whose
+// exact value provably exceeds the warp's running minimum need not be evaluated.  The estimate t_f repeats Eq. 20 in fast
+// fp32; when E_th is well conditioned (|E_th| >= 2^-8 (|E| + E_kin): relative error of E_th below 6e-5, of t_f below
+// (1 + |1 - alpha|) 1e-4) and every intermediate is a normal number, t_f > thr = tmin (1 + 1e-3 (1 + |1 - alpha|)) proves
+// t > tmin, and E_th <= 0 proves a zero rate.  Everything else (ill conditioned, out of range, NaN) returns true = "evaluate".
+template <class T>
+__device__ __forceinline__ bool tcool_may_decide(T rho_, T mx_, T my_, T mz_, T E_, float gm1f, float lambda0f, float alphaf, float thr) {
+  const float rho = (float)rho_, mx = (float)mx_, my = (float)my_, mz = (float)mz_, E = (float)E_;
+  const float q = mx * mx + my * my + mz * mz;
+  const float Ek = __fdividef(0.5f * q, rho);
+  const float Eth = E - Ek;
+  const float S = fabsf(E) + Ek;
+  const float Tc = __fdividef(gm1f * Eth, rho);
+  const float rate = rho * rho * lambda0f * __powf(fmaxf(Tc, 0.0f), alphaf);
+  const float t = __fdividef(Eth, rate);
+  const bool sure = fabsf(Eth) >= 0.00390625f * S && S > 1e-30f && S < 1e30f && rho > 1e-15f && rho < 1e15f;
+  const bool skip = sure && (Eth <= 0.0f || (rate > 1e-30f && rate < 1e30f && t > thr));
+  return !skip;
+}
+
 template <class T> struct Vec;
 template <> struct Vec<float> { using type = float4; static constexpr int W = 4; };
 template <> struct Vec<double> { using type = double2; static constexpr int W = 2; };
 
-template <class T>
+template <class T, bool COOL>
 __global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, const bool guarded) {
   using V = typename Vec<T>::type;
   constexpr int W = Vec<T>::W;
   const size_t N = p.N;
   if (guarded && p.cand_cnt[1] == 0u) return;      // the candidates already hold the maxima (cfl_cand_kernel)
   T sx = T(0), sy = T(0), sz = T(0);
+  double tmin = __longlong_as_double(0x7ff0000000000000ll);
   bool bad = false;
   const size_t tid = (size_t)blockIdx.x * blockDim.x + threadIdx.x, nth = (size_t)gridDim.x * blockDim.x;
-  if (N % W == 0) {
+  if constexpr (COOL) {
+    // warp-uniform trip counts (the screen's threshold is shared by the warp through shuffles)
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const size_t w0 = tid - lane;
+    const float gm1f = (float)p.gm1d, lambda0f = (float)p.lambda0, alphaf = (float)p.alpha;
+    const double margin = 1.0 + 1e-3 * (1.0 + fabs(1.0 - p.alpha));
+    float thr = __int_as_float(0x7f800000);
+    const bool vec = (N % W == 0);
+    const size_t cnt = vec ? N / W : N;
+    const V* r0 = reinterpret_cast<const V*>(p.U);
+    const V* r1 = reinterpret_cast<const V*>(p.U + N);
+    const V* r2 = reinterpret_cast<const V*>(p.U + 2 * N);
+    const V* r3 = reinterpret_cast<const V*>(p.U + 3 * N);
+    const V* r4 = reinterpret_cast<const V*>(p.U + 4 * N);
+    for (size_t b0 = w0; b0 < cnt; b0 += nth) {
+      const size_t v = b0 + lane;
+      T ca[W], cb[W], cc[W], cd[W], ce[W];
+      int n = 0;
+      if (v < cnt) {
+        if (vec) {
+          const V a = __ldg(r0 + v), b = __ldg(r1 + v), c = __ldg(r2 + v), d = __ldg(r3 + v), e = __ldg(r4 + v);
+#pragma unroll
+          for (int l = 0; l < W; ++l) {
+            ca[l] = reinterpret_cast<const T*>(&a)[l]; cb[l] = reinterpret_cast<const T*>(&b)[l]; cc[l] = reinterpret_cast<const T*>(&c)[l];
+            cd[l] = reinterpret_cast<const T*>(&d)[l]; ce[l] = reinterpret_cast<const T*>(&e)[l];
+          }
+          n = W;
+        } else {
+          ca[0] = p.U[v]; cb[0] = p.U[N + v]; cc[0] = p.U[2 * N + v]; cd[0] = p.U[3 * N + v]; ce[0] = p.U[4 * N + v];
+          n = 1;
+        }
+      }
+      bool need = false;
+#pragma unroll
+      for (int l = 0; l < W; ++l)
+        if (l < n) {
+          cell_speeds<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, sx, sy, sz, bad);
+          need = need || tcool_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], gm1f, lambda0f, alphaf, thr);
+        }
+      if (__any_sync(full, need)) {
+        if (need) {
+#pragma unroll
+          for (int l = 0; l < W; ++l)
+            if (l < n) cell_tcool<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, tmin);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const double ot = __shfl_xor_sync(full, tmin, o);
+          tmin = (ot < tmin) ? ot : tmin;
+        }
+        thr = __double2float_ru(tmin * margin);
+      }
+    }
+  } else if (N % W == 0) {
     const size_t nv = N / W;
     const V* r0 = reinterpret_cast<const V*>(p.U);
     const V* r1 = reinterpret_cast<const V*>(p.U + N);
@@ -80,6 +171,21 @@ __global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, c
   } else {
     for (size_t i = tid; i < N; i += nth)
       cell_speeds<T>(p.U[i], p.U[N + i], p.U[2 * N + i], p.U[3 * N + i], p.U[4 * N + i], p, sx, sy, sz, bad);
+  }
+  if constexpr (COOL) {      // min over the block: shuffles, then one slot per warp (min is exact and order independent)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const double ot = __shfl_xor_sync(0xffffffffu, tmin, o);
+      tmin = (ot < tmin) ? ot : tmin;
+    }
+    __shared__ double smt[8];
+    if ((threadIdx.x & 31) == 0) smt[threadIdx.x >> 5] = tmin;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const int nw = blockDim.x >> 5;
+      for (int w = 1; w < nw; ++w) tmin = (smt[w] < tmin) ? smt[w] : tmin;
+      atomicMin(p.acc + 4, (unsigned long long)__double_as_longlong(tmin));   // non-negative doubles order like their bits
+    }
   }
   // warp reduce (values are >= 0 or NaN; NaN handled through `bad`)
 #pragma unroll
@@ -186,7 +292,19 @@ __global__ void cfl_finish_kernel(const CflParams<T> p) {
     const T r = Ieee::div(p.dx[a], S[a]);
     if (r < best) best = r;
   }
-  const T dt = Ieee::mul(p.cfl, best);
+  T dt = Ieee::mul(p.cfl, best);
+  const T dt_hydro = dt;
+  // Eq. 21: dt <= min(dt_hydro, c_cool min_x t_cool, dt_max), the candidates compared in T (reading A24)
+  const double tcool = __longlong_as_double((long long)p.acc[4]);
+  p.acc[4] = 0x7ff0000000000000ull;
+  if (p.cool_lim && p.c_cool > 0.0) {
+    const T dc = (T)Ieee::mul(p.c_cool, tcool);
+    if (dc < dt) dt = dc;
+  }
+  if (p.dt_max > 0.0) {
+    const T dm = (T)p.dt_max;
+    if (dm < dt) dt = dm;
+  }
   *p.dt_dev = dt;
   if (p.cand_thr) {          // thresholds for the candidates the next last stage will push, and an empty list
     T smin = S[0] < S[1] ? S[0] : S[1];
@@ -202,6 +320,8 @@ __global__ void cfl_finish_kernel(const CflParams<T> p) {
   p.result->smax[2] = (double)S[2];
   p.result->dt = (double)dt;
   p.result->nonfinite = bad;
+  p.result->tcool_min = tcool;
+  p.result->dt_hydro = (double)dt_hydro;
 }
 
 template <class T>
@@ -212,7 +332,8 @@ cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t 
   size_t cap = (size_t)sm_count * 8;     // 8 resident 256-thread blocks per SM
   int blocks = (int)(want < cap ? want : cap);
   if (blocks < 1) blocks = 1;
-  cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p, false);
+  if (p.cool_lim) cfl_reduce_kernel<T, true><<<blocks, 256, 0, s>>>(p, false);
+  else cfl_reduce_kernel<T, false><<<blocks, 256, 0, s>>>(p, false);
   return cudaGetLastError();
 }
 
@@ -227,7 +348,7 @@ cudaError_t launch_cfl_candidates(const CflParams<T>& p, int sm_count, cudaStrea
   size_t cap = (size_t)sm_count * 8;
   int blocks = (int)(want < cap ? want : cap);
   if (blocks < 1) blocks = 1;
-  cfl_reduce_kernel<T><<<blocks, 256, 0, s>>>(p, true);
+  cfl_reduce_kernel<T, false><<<blocks, 256, 0, s>>>(p, true);    // the candidate path is never taken with the limit of Eq. 21
   return cudaGetLastError();
 }
 

@@ -78,6 +78,8 @@ struct CflResult {
   double smax[3];    // T values widened
   double dt;         // T value widened
   unsigned long long nonfinite;
+  double tcool_min;  // min_x t_cool(x) of Eq. 20 (+inf if the limit of Eq. 21 was not evaluated)
+  double dt_hydro;   // the Eq. A8 value before the other candidates of Eq. 21 (T value widened)
 };
 
 template <class T>
@@ -87,7 +89,11 @@ struct CflParams {
   T gamma, gm1, rho_floor, p_floor;
   T dx[3];
   T cfl;
-  unsigned long long* acc;   // [0..2] running max (bit pattern of T, zero-extended), [3] non-finite flag
+  unsigned long long* acc;   // [0..2] running max (bit pattern of T, zero-extended), [3] non-finite flag,
+                             // [4] running min of t_cool (bit pattern of a non-negative double; armed with +inf)
+  // Eq. 21: cool_lim != 0 makes the reduction evaluate Eq. 20 per cell (in double, reading A24)
+  int cool_lim;
+  double gm1d, lambda0, alpha, c_cool, dt_max;
   T* dt_dev;                 // dt in T for the stage kernels
   CflResult* result;         // device copy of the result block
   // candidate path (all nullptr = plain reduction): see StageParams
@@ -104,6 +110,7 @@ struct Ctx {
   double gamma, cfl, L[3];
   int cooling, kernel, limiter, riemann, integrator;
   int cool_mode, cool_nsub;    // DH_OPT_COOL_MODE (0 Euler sub-cycled, 1 trapezoid), DH_OPT_COOL_NSUB
+  double c_cool, dt_max;       // DH_OPT_C_COOL, DH_OPT_DT_MAX (Eq. 21; 0 = candidate off)
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
   int sm_count;

@@ -20,7 +20,7 @@ DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, 
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
-    "riemann": 15, "cool_mode": 16, "cool_nsub": 17,
+    "riemann": 15, "cool_mode": 16, "cool_nsub": 17, "c_cool": 18, "dt_max": 19,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
@@ -33,7 +33,7 @@ SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
-    "dh_cfl_stats",
+    "dh_cfl_stats", "dh_cool_tmin",
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
     "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
@@ -82,6 +82,8 @@ def load(rebuild: bool = False):
     lib.dh_profile_read.argtypes = [vp, pd, ctypes.POINTER(ctypes.c_ulonglong)]
     lib.dh_cfl_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_ulonglong)]
     lib.dh_cfl_stats.restype = ci
+    lib.dh_cool_tmin.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
+    lib.dh_cool_tmin.restype = ci
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
@@ -213,6 +215,13 @@ def dh_profile_enable(ctx, on: bool) -> None:
     _check(load().dh_profile_enable(ctx, 1 if on else 0))
 
 
+def dh_cool_tmin(ctx, U_ptr: int):
+    """(min_x t_cool(x) of Eq. 20, dt_hydro of Eq. A8) from one pass of the CFL reduction (include/dh.h)."""
+    t, d = ctypes.c_double(), ctypes.c_double()
+    _check(load().dh_cool_tmin(ctx, ctypes.c_void_p(U_ptr), ctypes.byref(t), ctypes.byref(d)))
+    return t.value, d.value
+
+
 def dh_cfl_stats(ctx) -> dict:
     """Counters of the CFL candidate path of dh_advance (include/dh.h)."""
     out = (ctypes.c_ulonglong * 3)()
@@ -316,6 +325,9 @@ class Solver:
 
     def cfl_stats(self) -> dict:
         return dh_cfl_stats(self.ctx)
+
+    def cool_tmin(self, U):
+        return dh_cool_tmin(self.ctx, self._dev(U, "U"))
 
     @property
     def launch_count(self) -> int:
