@@ -31,12 +31,16 @@ __device__ __forceinline__ void from_bits(unsigned long long b, double& x) { x =
 __device__ __forceinline__ bool finite_(float x) { return isfinite(x); }
 __device__ __forceinline__ bool finite_(double x) { return isfinite(x); }
 
+// ek / eth: the kinetic and thermal energy densities the recipe forms on its way (in T, with the floored density)
 template <class T>
-__device__ __forceinline__ void cell_speeds(T rho, T mx, T my, T mz, T E, const CflParams<T>& p, T& sx, T& sy, T& sz, bool& bad) {
+__device__ __forceinline__ void cell_speeds(T rho, T mx, T my, T mz, T E, const CflParams<T>& p, T& sx, T& sy, T& sz, bool& bad,
+                                            T& ek, T& eth) {
   const T rt = (rho >= p.rho_floor) ? rho : p.rho_floor;
   const T vx = Ieee::div(mx, rt), vy = Ieee::div(my, rt), vz = Ieee::div(mz, rt);
   const T q = Ieee::add(Ieee::add(Ieee::mul(mx, mx), Ieee::mul(my, my)), Ieee::mul(mz, mz));
-  T P = Ieee::mul(p.gm1, Ieee::sub(E, Ieee::mul(T(0.5), Ieee::div(q, rt))));
+  ek = Ieee::mul(T(0.5), Ieee::div(q, rt));
+  eth = Ieee::sub(E, ek);
+  T P = Ieee::mul(p.gm1, eth);
   P = (P >= p.p_floor) ? P : p.p_floor;
   const T cs = Ieee::sqrt(Ieee::div(Ieee::mul(p.gamma, P), rt));
   const T ax = Ieee::add(abs_(vx), cs), ay = Ieee::add(abs_(vy), cs), az = Ieee::add(abs_(vz), cs);
@@ -47,39 +51,43 @@ __device__ __forceinline__ void cell_speeds(T rho, T mx, T my, T mz, T E, const 
   sz = (az > sz) ? az : sz;
 }
 
+template <class T>
+__device__ __forceinline__ void cell_speeds(T rho, T mx, T my, T mz, T E, const CflParams<T>& p, T& sx, T& sy, T& sz, bool& bad) {
+  T ek, eth;
+  cell_speeds<T>(rho, mx, my, mz, E, p, sx, sy, sz, bad, ek, eth);
+}
+
 // Eq. 20 for one cell in the code units of reading A10, in double whatever T (reading A24); the
 // operations and their order are those of cool() / cool_rate() of the cooling update, never contracted.
-template <class T>
-__device__ __forceinline__ void cell_tcool(T rho_, T mx_, T my_, T mz_, T E_, const CflParams<T>& p, double& tmin) {
-  const double rho = (double)rho_, mx = (double)mx_, my = (double)my_, mz = (double)mz_, E = (double)E_;
+// (not inlined: the rare exact path is a call, so that the fp64 power function does not weigh on the registers of the sweep)
+__device__ __noinline__ double cell_tcool(double rho, double mx, double my, double mz, double E, double gm1d, double lambda0, double alpha,
+                                          double tmin) {
   const double q = Ieee::add(Ieee::add(Ieee::mul(mx, mx), Ieee::mul(my, my)), Ieee::mul(mz, mz));
   const double Ek = Ieee::div(Ieee::mul(0.5, q), rho);
   const double Eth = Ieee::sub(E, Ek);
-  const double Tc = Ieee::div(Ieee::mul(p.gm1d, Eth), rho);
+  const double Tc = Ieee::div(Ieee::mul(gm1d, Eth), rho);
   const double Tpos = (Tc > 0.0) ? Tc : 0.0;
-  const double rate = Ieee::mul(Ieee::mul(Ieee::mul(rho, rho), p.lambda0), pow(Tpos, p.alpha));
+  const double rate = Ieee::mul(Ieee::mul(Ieee::mul(rho, rho), lambda0), pow(Tpos, alpha));
   const double t = Ieee::div(fabs(Eth), fabs(rate));
-  if (rate != 0.0 && t < tmin) tmin = t;
+  return (rate != 0.0 && t < tmin) ? t : tmin;
 }
 
 // fp32 screen in front of cell_tcool (whose fp64 power function would make the pass ALU bound: 1.92 ms instead of the 0.41 ms
 // the 20 B/cell take at 512^3).  Any exact t_cool already evaluated is an upper bound of the global minimum, so a cell whose
-// exact value provably exceeds the warp's running minimum need not be evaluated.  The estimate t_f repeats Eq. 20 in fast
-// fp32; when E_th is well conditioned (|E_th| >= 2^-8 (|E| + E_kin): relative error of E_th below 6e-5, of t_f below
-// (1 + |1 - alpha|) 1e-4) and every intermediate is a normal number, t_f > thr = tmin (1 + 1e-3 (1 + |1 - alpha|)) proves
-// t > tmin, and E_th <= 0 proves a zero rate.  Everything else (ill conditioned, out of range, NaN) returns true = "evaluate".
+// exact value provably exceeds the warp's running minimum need not be evaluated.  The screen works in log2 on the E_kin / E_th
+// the wave-speed recipe has just formed:  log2 t_cool = (1 - alpha) log2 E_th + (alpha - 2) log2 rho - log2 lambda0
+// - alpha log2(gamma - 1), two MUFU.LG2 and two FMAs.  When E_th is well conditioned (|E_th| >= 2^-8 (|E| + E_kin): relative
+// error of the fp32 E_th below 6e-5) and rho, E are normal fp32 numbers above the density floor, the left-hand side is within
+// (1 + |1 - alpha|) 1e-4 + 1e-4 of the exact value, and lhs > lthr = log2(tmin) + log2(1 + 1e-3 (1 + |1 - alpha|)) + the constants
+// proves t > tmin; a well-conditioned E_th <= 0 proves a zero rate.  Everything else (ill conditioned, out of range, NaN)
+// returns true = "evaluate exactly".
 template <class T>
-__device__ __forceinline__ bool tcool_may_decide(T rho_, T mx_, T my_, T mz_, T E_, float gm1f, float lambda0f, float alphaf, float thr) {
-  const float rho = (float)rho_, mx = (float)mx_, my = (float)my_, mz = (float)mz_, E = (float)E_;
-  const float q = mx * mx + my * my + mz * mz;
-  const float Ek = __fdividef(0.5f * q, rho);
-  const float Eth = E - Ek;
+__device__ __forceinline__ bool tcool_may_decide(T rho_, T E_, T ek_, T eth_, T rho_floor, float c_eth, float c_rho, float lthr) {
+  const float rho = (float)rho_, E = (float)E_, Ek = (float)ek_, Eth = (float)eth_;
   const float S = fabsf(E) + Ek;
-  const float Tc = __fdividef(gm1f * Eth, rho);
-  const float rate = rho * rho * lambda0f * __powf(fmaxf(Tc, 0.0f), alphaf);
-  const float t = __fdividef(Eth, rate);
-  const bool sure = fabsf(Eth) >= 0.00390625f * S && S > 1e-30f && S < 1e30f && rho > 1e-15f && rho < 1e15f;
-  const bool skip = sure && (Eth <= 0.0f || (rate > 1e-30f && rate < 1e30f && t > thr));
+  const bool sure = rho_ >= rho_floor && fabsf(Eth) >= 0.00390625f * S && S > 1e-30f && S < 1e30f && rho > 1e-15f && rho < 1e15f;
+  const float lhs = fmaf(c_eth, __log2f(Eth), c_rho * __log2f(rho));
+  const bool skip = sure && (Eth <= 0.0f || lhs > lthr);
   return !skip;
 }
 
@@ -88,7 +96,7 @@ template <> struct Vec<float> { using type = float4; static constexpr int W = 4;
 template <> struct Vec<double> { using type = double2; static constexpr int W = 2; };
 
 template <class T, bool COOL>
-__global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, const bool guarded) {
+__global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const CflParams<T> p, const bool guarded) {
   using V = typename Vec<T>::type;
   constexpr int W = Vec<T>::W;
   const size_t N = p.N;
@@ -102,9 +110,10 @@ __global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, c
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const size_t w0 = tid - lane;
-    const float gm1f = (float)p.gm1d, lambda0f = (float)p.lambda0, alphaf = (float)p.alpha;
-    const double margin = 1.0 + 1e-3 * (1.0 + fabs(1.0 - p.alpha));
-    float thr = __int_as_float(0x7f800000);
+    const float c_eth = (float)(1.0 - p.alpha), c_rho = (float)(p.alpha - 2.0);
+    // log2 of the safety factor, and the constant terms of log2 t_cool moved to the threshold's side
+    const double lconst = log2(1.0 + 1e-3 * (1.0 + fabs(1.0 - p.alpha))) + log2(p.lambda0) + p.alpha * log2(p.gm1d);
+    float lthr = __int_as_float(0x7f800000);     // +inf: nothing is skipped before the first exact value
     const bool vec = (N % W == 0);
     const size_t cnt = vec ? N / W : N;
     const V* r0 = reinterpret_cast<const V*>(p.U);
@@ -134,21 +143,22 @@ __global__ void __launch_bounds__(256) cfl_reduce_kernel(const CflParams<T> p, c
 #pragma unroll
       for (int l = 0; l < W; ++l)
         if (l < n) {
-          cell_speeds<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, sx, sy, sz, bad);
-          need = need || tcool_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], gm1f, lambda0f, alphaf, thr);
+          T ek, eth;
+          cell_speeds<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, sx, sy, sz, bad, ek, eth);
+          need = need || tcool_may_decide<T>(ca[l], ce[l], ek, eth, p.rho_floor, c_eth, c_rho, lthr);
         }
       if (__any_sync(full, need)) {
         if (need) {
 #pragma unroll
           for (int l = 0; l < W; ++l)
-            if (l < n) cell_tcool<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, tmin);
+            if (l < n) tmin = cell_tcool((double)ca[l], (double)cb[l], (double)cc[l], (double)cd[l], (double)ce[l], p.gm1d, p.lambda0, p.alpha, tmin);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
           const double ot = __shfl_xor_sync(full, tmin, o);
           tmin = (ot < tmin) ? ot : tmin;
         }
-        thr = __double2float_ru(tmin * margin);
+        lthr = __double2float_ru(log2(tmin) + lconst);     // tmin = +inf stays +inf; a NaN (lambda0 = 0) never skips
       }
     }
   } else if (N % W == 0) {
@@ -329,7 +339,11 @@ cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t 
   constexpr int W = Vec<T>::W;
   size_t work = (p.N % W == 0) ? p.N / W : p.N;
   size_t want = (work + 255) / 256;
-  size_t cap = (size_t)sm_count * 8;     // 8 resident 256-thread blocks per SM
+  int per_sm = 8;                        // 8 resident 256-thread blocks per SM
+  if (p.cool_lim) {                      // the variant with the t_cool branch holds more registers: one wave of resident blocks
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, cfl_reduce_kernel<T, true>, 256, 0) != cudaSuccess || per_sm < 1) per_sm = 2;
+  }
+  size_t cap = (size_t)sm_count * per_sm;
   int blocks = (int)(want < cap ? want : cap);
   if (blocks < 1) blocks = 1;
   if (p.cool_lim) cfl_reduce_kernel<T, true><<<blocks, 256, 0, s>>>(p, false);
