@@ -163,6 +163,35 @@ def test_fp32_screen_never_drops_the_minimum(dtype, alpha):
         assert np.isfinite(t_ora) and t_gpu == pytest.approx(t_ora, rel=1e-14), (k, t_gpu, t_ora)
 
 
+def test_adjoint_holds_the_limited_dt_constant():
+    """dh_adjoint with c_cool > 0: the forward sweep's dt sequence is the limited one (Eq. 21), and the reverse sweep is the
+    chain of step VJPs at those dt held constant, checked against the oracle's step VJP chained over the
+    oracle's own limited-dt loop."""
+    gamma = 5 / 3
+    U = _lognormal_state((9, 10, 36), 761, gamma, torch.float64)
+    kw = dict(cooling=True, lambda0=20.0, alpha=0.5, t_floor=0.01)
+    p = oracle_params(U, gamma, **kw)
+    s = _solver(U, gamma, cooling=1, lambda0=20.0, t_floor=0.01, c_cool=0.1)
+    g = np.random.default_rng(762).normal(size=tuple(U.shape))
+    Ud, gd = U.cuda(), torch.from_numpy(g).cuda()
+    dts = s.adjoint(Ud, gd, 3, 2)
+    states, dts_ref, cur = [], [], U.numpy().copy()
+    for _ in range(3):
+        dth, _ = oracle.cfl_dt(cur, p)
+        _, dt = oracle.cool_dt(cur, p, dth, c_cool=0.1)
+        assert dt < dth
+        states.append(cur)
+        dts_ref.append(dt)
+        cur = oracle.step(cur, dt, p)
+    assert np.allclose(dts, dts_ref, rtol=1e-13, atol=0)
+    assert max_rel_err(Ud.cpu().numpy(), cur) <= 5e-12
+    gref = g
+    for k in (2, 1, 0):
+        gref = oracle.step_vjp(states[k], dts_ref[k], gref, p)
+    err = np.abs(gd.cpu().numpy() - gref) / np.sqrt(np.mean(gref ** 2))
+    assert err.max() <= 1e-11, float(err.max())
+
+
 def test_option_errors_and_defaults():
     from paper_2512_13403_b200 import dh
     U = random_state((4, 4, 4), 741, 1.4, torch.float32)
