@@ -30,6 +30,8 @@ __device__ __forceinline__ void from_bits(unsigned long long b, float& x) { x = 
 __device__ __forceinline__ void from_bits(unsigned long long b, double& x) { x = __longlong_as_double((long long)b); }
 __device__ __forceinline__ bool finite_(float x) { return isfinite(x); }
 __device__ __forceinline__ bool finite_(double x) { return isfinite(x); }
+__device__ __forceinline__ float round_down(float x) { return x; }
+__device__ __forceinline__ float round_down(double x) { return __double2float_rd(x); }
 
 // ek / eth: the kinetic and thermal energy densities the recipe forms on its way (in T, with the floored density)
 template <class T>
@@ -82,13 +84,36 @@ __device__ __noinline__ double cell_tcool(double rho, double mx, double my, doub
 // proves t > tmin; a well-conditioned E_th <= 0 proves a zero rate.  Everything else (ill conditioned, out of range, NaN)
 // returns true = "evaluate exactly".
 template <class T>
-__device__ __forceinline__ bool tcool_may_decide(T rho_, T E_, T ek_, T eth_, T rho_floor, float c_eth, float c_rho, float lthr) {
-  const float rho = (float)rho_, E = (float)E_, Ek = (float)ek_, Eth = (float)eth_;
+__device__ __forceinline__ bool tcool_may_decide(T rho_, T E_, float Ek, float Eth, T rho_floor, float c_eth, float c_rho, float lthr) {
+  const float rho = (float)rho_, E = (float)E_;
   const float S = fabsf(E) + Ek;
   const bool sure = rho_ >= rho_floor && fabsf(Eth) >= 0.00390625f * S && S > 1e-30f && S < 1e30f && rho > 1e-15f && rho < 1e15f;
   const float lhs = fmaf(c_eth, __log2f(Eth), c_rho * __log2f(rho));
   const bool skip = sure && (Eth <= 0.0f || lhs > lthr);
   return !skip;
+}
+
+// fp32 screen in front of the wave-speed recipe (COOL sweep only; the plain reduction is HBM bound as it is).  The exact
+// recipe's five IEEE divisions and square root are most of the sweep's instructions, and only cells near the maxima matter:
+// a cell whose speeds are provably below exact speeds already found cannot raise the maxima.  Upper bounds from fast fp32:
+// |v_a| <= |m_a| (1/rho) (1 + 1e-5);  P <= gm1 (E_th + 1e-6 (|E| + E_kin)) (the fp32 E_th is within 3e-7 (|E| + E_kin) of the
+// recipe's), floored;  c_s <= sqrt(gamma P / rho) (1 + 1e-5).  Needs rho above the density floor and normal fp32 ranges;
+// anything else (NaN and Inf included, so the non-finite flag is still raised by the recipe) returns true = "run the recipe".
+// Also hands the fp32 E_kin / E_th to the t_cool screen.
+template <class T>
+__device__ __forceinline__ bool speeds_may_decide(T rho_, T mx_, T my_, T mz_, T E_, T rho_floor, float gm1f, float gammaf, float pflf,
+                                                  float bx, float by, float bz, float& Ek, float& Eth) {
+  const float rho = (float)rho_, mx = (float)mx_, my = (float)my_, mz = (float)mz_, E = (float)E_;
+  const float ir = __fdividef(1.0f, rho);
+  Ek = 0.5f * (mx * mx + my * my + mz * mz) * ir;
+  Eth = E - Ek;
+  const float S = fabsf(E) + Ek;
+  const float Pup = fmaxf(gm1f * fmaf(1e-6f, S, Eth), pflf);
+  const float cs = sqrtf(gammaf * Pup * ir) * 1.00002f;
+  const float k = 1.00001f * ir;
+  const bool sure = rho_ >= rho_floor && rho > 1e-15f && rho < 1e15f && S < 1e30f;
+  const bool below = fmaf(fabsf(mx), k, cs) < bx && fmaf(fabsf(my), k, cs) < by && fmaf(fabsf(mz), k, cs) < bz;
+  return !(sure && below);
 }
 
 template <class T> struct Vec;
@@ -114,6 +139,8 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
     // log2 of the safety factor, and the constant terms of log2 t_cool moved to the threshold's side
     const double lconst = log2(1.0 + 1e-3 * (1.0 + fabs(1.0 - p.alpha))) + log2(p.lambda0) + p.alpha * log2(p.gm1d);
     float lthr = __int_as_float(0x7f800000);     // +inf: nothing is skipped before the first exact value
+    const float gm1f = (float)p.gm1, gammaf = (float)p.gamma, pflf = (float)p.p_floor * 1.000001f;
+    float bx = 0.0f, by = 0.0f, bz = 0.0f;       // fp32 lower bounds of the warp's running exact maxima
     const bool vec = (N % W == 0);
     const size_t cnt = vec ? N / W : N;
     const V* r0 = reinterpret_cast<const V*>(p.U);
@@ -139,14 +166,29 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
           n = 1;
         }
       }
-      bool need = false;
+      bool need = false, need_s = false;
 #pragma unroll
       for (int l = 0; l < W; ++l)
         if (l < n) {
-          T ek, eth;
-          cell_speeds<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, sx, sy, sz, bad, ek, eth);
+          float ek, eth;
+          need_s = need_s || speeds_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p.rho_floor, gm1f, gammaf, pflf, bx, by, bz, ek, eth);
           need = need || tcool_may_decide<T>(ca[l], ce[l], ek, eth, p.rho_floor, c_eth, c_rho, lthr);
         }
+      if (__any_sync(full, need_s)) {      // the exact recipe for the lanes that asked, then the warp shares its maxima
+        if (need_s) {
+#pragma unroll
+          for (int l = 0; l < W; ++l)
+            if (l < n) cell_speeds<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p, sx, sy, sz, bad);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const T ox = __shfl_xor_sync(full, sx, o), oy = __shfl_xor_sync(full, sy, o), oz = __shfl_xor_sync(full, sz, o);
+          sx = (ox > sx) ? ox : sx;
+          sy = (oy > sy) ? oy : sy;
+          sz = (oz > sz) ? oz : sz;
+        }
+        bx = round_down(sx); by = round_down(sy); bz = round_down(sz);
+      }
       if (__any_sync(full, need)) {
         if (need) {
 #pragma unroll

@@ -159,8 +159,10 @@ def test_fp32_screen_never_drops_the_minimum(dtype, alpha):
         p = oracle_params(torch.from_numpy(U), gamma, cooling=True, lambda0=0.3, alpha=alpha)
         s = _solver(torch.from_numpy(U), gamma, lambda0=0.3, alpha=alpha)
         t_ora, _ = oracle.cool_dt(U, p, 1.0)
-        t_gpu, _ = s.cool_tmin(torch.from_numpy(U).cuda())
+        t_gpu, dth_gpu = s.cool_tmin(torch.from_numpy(U).cuda())
         assert np.isfinite(t_ora) and t_gpu == pytest.approx(t_ora, rel=1e-14), (k, t_gpu, t_ora)
+        # the same sweep screens the wave-speed recipe in fp32 too (speeds_may_decide): dt_hydro keeps its bits
+        assert dth_gpu == oracle.cfl_dt(U, p)[0], k
 
 
 def test_adjoint_holds_the_limited_dt_constant():
