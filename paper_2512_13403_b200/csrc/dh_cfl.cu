@@ -83,12 +83,11 @@ __device__ __noinline__ double cell_tcool(double rho, double mx, double my, doub
 // (1 + |1 - alpha|) 1e-4 + 1e-4 of the exact value, and lhs > lthr = log2(tmin) + log2(1 + 1e-3 (1 + |1 - alpha|)) + the constants
 // proves t > tmin; a well-conditioned E_th <= 0 proves a zero rate.  Everything else (ill conditioned, out of range, NaN)
 // returns true = "evaluate exactly".
+// (`range_ok`: rho above the density floor and rho, S inside the fp32 range tests of speeds_may_decide, which also formed S)
 template <class T>
-__device__ __forceinline__ bool tcool_may_decide(T rho_, T E_, float Ek, float Eth, T rho_floor, float c_eth, float c_rho, float lthr) {
-  const float rho = (float)rho_, E = (float)E_;
-  const float S = fabsf(E) + Ek;
-  const bool sure = rho_ >= rho_floor && fabsf(Eth) >= 0.00390625f * S && S > 1e-30f && S < 1e30f && rho > 1e-15f && rho < 1e15f;
-  const float lhs = fmaf(c_eth, __log2f(Eth), c_rho * __log2f(rho));
+__device__ __forceinline__ bool tcool_may_decide(T rho_, float Eth, float S, bool range_ok, float c_eth, float c_rho, float lthr) {
+  const bool sure = range_ok && fabsf(Eth) >= 0.00390625f * S && S > 1e-30f;
+  const float lhs = fmaf(c_eth, __log2f(Eth), c_rho * __log2f((float)rho_));
   const bool skip = sure && (Eth <= 0.0f || lhs > lthr);
   return !skip;
 }
@@ -102,16 +101,16 @@ __device__ __forceinline__ bool tcool_may_decide(T rho_, T E_, float Ek, float E
 // Also hands the fp32 E_kin / E_th to the t_cool screen.
 template <class T>
 __device__ __forceinline__ bool speeds_may_decide(T rho_, T mx_, T my_, T mz_, T E_, T rho_floor, float gm1f, float gammaf, float pflf,
-                                                  float bx, float by, float bz, float& Ek, float& Eth) {
+                                                  float bx, float by, float bz, float& Ek, float& Eth, float& S, bool& sure) {
   const float rho = (float)rho_, mx = (float)mx_, my = (float)my_, mz = (float)mz_, E = (float)E_;
   const float ir = __fdividef(1.0f, rho);
   Ek = 0.5f * (mx * mx + my * my + mz * mz) * ir;
   Eth = E - Ek;
-  const float S = fabsf(E) + Ek;
+  S = fabsf(E) + Ek;
   const float Pup = fmaxf(gm1f * fmaf(1e-6f, S, Eth), pflf);
   const float cs = sqrtf(gammaf * Pup * ir) * 1.00002f;
   const float k = 1.00001f * ir;
-  const bool sure = rho_ >= rho_floor && rho > 1e-15f && rho < 1e15f && S < 1e30f;
+  sure = rho_ >= rho_floor && rho > 1e-15f && rho < 1e15f && S < 1e30f;
   const bool below = fmaf(fabsf(mx), k, cs) < bx && fmaf(fabsf(my), k, cs) < by && fmaf(fabsf(mz), k, cs) < bz;
   return !(sure && below);
 }
@@ -170,9 +169,10 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
 #pragma unroll
       for (int l = 0; l < W; ++l)
         if (l < n) {
-          float ek, eth;
-          need_s = need_s || speeds_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p.rho_floor, gm1f, gammaf, pflf, bx, by, bz, ek, eth);
-          need = need || tcool_may_decide<T>(ca[l], ce[l], ek, eth, p.rho_floor, c_eth, c_rho, lthr);
+          float ek, eth, S;
+          bool range_ok;
+          need_s = need_s || speeds_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p.rho_floor, gm1f, gammaf, pflf, bx, by, bz, ek, eth, S, range_ok);
+          need = need || tcool_may_decide<T>(ca[l], eth, S, range_ok, c_eth, c_rho, lthr);
         }
       if (__any_sync(full, need_s)) {      // the exact recipe for the lanes that asked, then the warp shares its maxima
         if (need_s) {
