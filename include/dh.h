@@ -66,8 +66,7 @@ enum {
   DH_OPT_RHO_FLOOR = 8,  /* floors used only inside the primitive conversion, default 1e-10 */
   DH_OPT_P_FLOOR = 9,
   DH_OPT_KERNEL = 10,    /* 0 (default): fused z-sweep stage kernel, 2x2 cells per thread; 1: one-thread-per-cell gather
-                            kernels (same arithmetic, kept for cross-checking and as the fallback for odd nx);
-                            2: the first fused z-sweep kernel (one pack per thread), kept for comparison */
+                            kernels (same arithmetic, kept for cross-checking and as the fallback for odd nx) */
   DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
   DH_OPT_REV_SLAB = 12,  /* planes per z slab of the fused reverse stages' scratch (20 words per cell of a slab);
                             0 (default): as many as fit in min(32 GiB, half of the free device memory) */

@@ -130,5 +130,17 @@ int dho_cool_dt(int nx, int ny, int nz, const Params* p, int dtype, const void* 
   return 0;
 }
 
+// decision margins of one flux-divergence evaluation at U: M is [4][nz][ny][nx] (see dh_oracle.hpp)
+int dho_decision_margins(int nx, int ny, int nz, const Params* p, const double* U, double* M) {
+  decision_margins(mkgrid(nx, ny, nz), *p, U, M);
+  return 0;
+}
+
+// margins of the compares of cool() at the pre-cooling state U1: M is [nz][ny][nx]
+int dho_cooling_margins(int nx, int ny, int nz, const Params* p, double dt, const double* U1, double* M) {
+  cooling_margins(mkgrid(nx, ny, nz), *p, dt, U1, M);
+  return 0;
+}
+
 }  // extern "C"
 

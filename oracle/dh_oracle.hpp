@@ -586,4 +586,152 @@ double limited_dt(double dt_hydro, double tmin, double c_cool, double dt_max) {
   return (double)dt;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Decision margins (test infrastructure for the VJP parity check; "non-smooth operators",
+// PAPER.md:119-127; readings A7 / A17).
+//
+// The scheme is piecewise smooth: its a.e. derivative follows the branch actually taken by every compare the step
+// makes — limiter (a b <= 0, |a| <= |b|), Eq. A3's min / max, the HLLC / HLL select order (S_L >= 0, S_R <= 0,
+// S* >= 0), Rusanov's max of absolute values, the floors of prim().  An implementation that evaluates the same
+// formulas in another precision takes the same branch unless the two compared quantities agree to within its
+// rounding error.  For every compare this routine returns how far the oracle's own operands are from the tie,
+// divided by the magnitude on which rounding errors of those operands scale:
+//   rho: rho;   velocities: |v| + c_s;   pressure: P + (gamma-1) rho |v|^2 / 2  (P is a difference of E and E_kin)
+// (the largest of these over the cells the operands are formed from).  Output M[4][N]:
+//   M[a][i], a = 0..2: min over the five limiter calls at cell i along axis a and the Riemann compares at face i+1/2
+//   M[3][i]: the two floors of prim() at cell i.
+// A compare whose operands are exactly equal because the data are exactly uniform there (a = b = 0) is not a tie in
+// this sense: identical inputs give identical operands in any deterministic arithmetic; it gets +inf.
+// ------------------------------------------------------------------------------------------------
+inline void margin_scales(const double W[5], double gamma, double s[5]) {
+  const double vv = std::sqrt(W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
+  const double cs = std::sqrt(gamma * W[4] / W[0]);
+  s[0] = W[0];
+  s[1] = s[2] = s[3] = vv + cs;
+  s[4] = W[4] + 0.5 * (gamma - 1.0) * W[0] * vv * vv;
+}
+
+inline double limiter_margin(double a, double b, int kind, double s) {
+  const double inf = std::numeric_limits<double>::infinity();
+  if (kind == 3) return inf;
+  if (a == 0.0 && b == 0.0) return inf;
+  const double fa = std::fabs(a), fb = std::fabs(b);
+  double m = (fa < fb ? fa : fb) / s;                       // a b <= 0 flips when either operand crosses zero
+  if (a * b <= 0.0) return m;
+  if (kind == 0) {                                          // minmod: |a| <= |b|
+    m = std::fmin(m, std::fabs(fa - fb) / s);
+  } else if (kind == 2) {                                   // MC: |2a| <= |2b|, then |m| <= |(a+b)/2|
+    m = std::fmin(m, 2.0 * std::fabs(fa - fb) / s);
+    m = std::fmin(m, std::fabs(2.0 * (fa < fb ? fa : fb) - 0.5 * (fa + fb)) / s);
+  }
+  return m;                                                 // van Leer: smooth away from a b = 0
+}
+
+// the compares riemann() makes on the face states L, R (same expressions as riemann() above)
+inline double riemann_margin(const double L[5], const double R[5], int ax, const Params& p) {
+  const double inf = std::numeric_limits<double>::infinity();
+  const double g = p.gamma;
+  const double uL = L[1 + ax], uR = R[1 + ax];
+  const double cL = std::sqrt(g * L[4] / L[0]), cR = std::sqrt(g * R[4] / R[0]);
+  const double s = std::fmax(std::fabs(uL) + cL, std::fabs(uR) + cR);
+  // L and R agree in (rho, u_n, P) to rounding: either the data are uniform there, or both cells' limiters returned the
+  // difference they share, so that L = W_i + d/2 and R = W_{i+1} - d/2 are the same function of the data; whichever
+  // argument Eq. A3's min / max then return, the derivative with respect to the data is the same: not a tie
+  const double rs[3] = {std::fmax(L[0], R[0]), s, std::fmax(L[4], R[4])};
+  const int qs[3] = {0, 1 + ax, 4};
+  bool same = true;
+  for (int m3 = 0; m3 < 3; ++m3) same = same && (std::fabs(L[qs[m3]] - R[qs[m3]]) <= 1e-14 * rs[m3]);
+  const double SL = std::fmin(uL - cL, uR - cR), SR = std::fmax(uL + cL, uR + cR);
+  double m = inf;
+  if (!same) {                                              // which argument Eq. A3's min / max return
+    m = std::fmin(m, std::fabs((uL - cL) - (uR - cR)) / s);
+    m = std::fmin(m, std::fabs((uL + cL) - (uR + cR)) / s);
+  }
+  if (p.riemann == 2) {                                     // max(|S_L|, |S_R|) and the two absolute values
+    m = std::fmin(m, std::fabs(std::fabs(SL) - std::fabs(SR)) / s);
+    m = std::fmin(m, std::fabs(SL) / s);
+    m = std::fmin(m, std::fabs(SR) / s);
+    return m;
+  }
+  m = std::fmin(m, std::fabs(SL) / s);                      // S_L >= 0
+  m = std::fmin(m, std::fabs(SR) / s);                      // S_R <= 0
+  if (p.riemann == 0 && SL < 0.0 && SR > 0.0) {             // S* >= 0
+    const double Ss = (R[4] - L[4] + L[0] * uL * (SL - uL) - R[0] * uR * (SR - uR)) /
+                      (L[0] * (SL - uL) - R[0] * (SR - uR));
+    m = std::fmin(m, std::fabs(Ss) / s);
+  }
+  return m;
+}
+
+inline void decision_margins(const Grid& g, const Params& p, const double* U, double* M) {
+  const size_t N = g.N();
+  std::vector<double> W(5 * N), Sc(5 * N);
+  compute_prims(g, p, U, W.data());
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    double w[5], s[5];
+    for (int q = 0; q < 5; ++q) w[q] = W[q * N + c];
+    margin_scales(w, p.gamma, s);
+    for (int q = 0; q < 5; ++q) Sc[q * N + c] = s[q];
+    // floors of prim(): rho >= rho_floor, P >= p_floor, on the unfloored values
+    const double rho = U[c];
+    const double rr = std::fmax(rho, p.rho_floor);
+    const double Praw = (p.gamma - 1.0) * (U[4 * N + c] - 0.5 * (U[N + c] * U[N + c] + U[2 * N + c] * U[2 * N + c] + U[3 * N + c] * U[3 * N + c]) / rr);
+    const double sP = std::fabs(Praw) + 0.5 * (p.gamma - 1.0) * (U[N + c] * U[N + c] + U[2 * N + c] * U[2 * N + c] + U[3 * N + c] * U[3 * N + c]) / rr;
+    M[3 * N + c] = std::fmin(std::fabs(rho - p.rho_floor) / std::fmax(std::fabs(rho), p.rho_floor),
+                             std::fabs(Praw - p.p_floor) / std::fmax(sP, p.p_floor));
+  }
+  for (int ax = 0; ax < 3; ++ax) {
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          const size_t cm1 = shifted(g, i, j, k, ax, -1), c0 = g.idx(i, j, k);
+          const size_t cp1 = shifted(g, i, j, k, ax, +1), cp2 = shifted(g, i, j, k, ax, +2);
+          double a[5], b[5], c[5], d[5], WL[5], WR[5];
+          for (int q = 0; q < 5; ++q) { a[q] = W[q * N + cm1]; b[q] = W[q * N + c0]; c[q] = W[q * N + cp1]; d[q] = W[q * N + cp2]; }
+          double m = std::numeric_limits<double>::infinity();
+          for (int q = 0; q < 5; ++q) {                     // the limiter call of cell i (Eq. A1)
+            const double s = std::fmax(Sc[q * N + cm1], std::fmax(Sc[q * N + c0], Sc[q * N + cp1]));
+            m = std::fmin(m, limiter_margin(c[q] - b[q], b[q] - a[q], p.limiter, s));
+          }
+          face_states(a, b, c, d, p, WL, WR);
+          m = std::fmin(m, riemann_margin(WL, WR, ax, p));
+          M[(size_t)ax * N + c0] = m;
+        }
+  }
+}
+
+// the compares of cool() at the pre-cooling state U1: T > 0 inside cool_rate() and every max with E_floor,
+// relative to E_kin + |E_th| (E_th is a difference of E and E_kin)
+inline void cooling_margins(const Grid& g, const Params& p, double dt, const double* U1, double* M) {
+  const size_t N = g.N();
+#pragma omp parallel for schedule(static)
+  for (long long c = 0; c < (long long)N; ++c) {
+    const double rho = U1[c];
+    const double Ek = 0.5 * (U1[N + c] * U1[N + c] + U1[2 * N + c] * U1[2 * N + c] + U1[3 * N + c] * U1[3 * N + c]) / rho;
+    double Eth = U1[4 * N + c] - Ek;
+    const double s = Ek + std::fabs(Eth);
+    const double Efloor = rho * p.t_floor / (p.gamma - 1.0);
+    double m = std::fabs(Eth) / s;
+    if (p.cool_mode == 1) {
+      const double En = cool_rate<double>(Eth, rho, p);
+      const double raw = Eth + En * dt;
+      m = std::fmin(m, std::fabs(raw - Efloor) / s);
+      const double Epred = std::fmax(Efloor, raw);
+      const double raw2 = Eth + (0.5 * dt) * (En + cool_rate<double>(Epred, rho, p));
+      m = std::fmin(m, std::fabs(raw2 - Efloor) / s);
+    } else {
+      const int nsub = p.cool_nsub > 1 ? p.cool_nsub : 1;
+      const double ddt = dt / nsub;
+      for (int k = 0; k < nsub; ++k) {
+        const double raw = Eth + cool_rate<double>(Eth, rho, p) * ddt;
+        m = std::fmin(m, std::fabs(raw - Efloor) / s);
+        Eth = std::fmax(Efloor, raw);
+      }
+    }
+    M[c] = m;
+  }
+}
+
 }  // namespace dho

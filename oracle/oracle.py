@@ -232,6 +232,26 @@ def limiter(a, b, kind="minmod"):
     return float(_load().dho_limiter(float(a), float(b), LIMITERS[kind]))
 
 
+def decision_margins(U, p):
+    """[4, nz, ny, nx]: distance from the tie of every compare one evaluation of D(U) makes, relative to the rounding scale
+    of its operands: slots 0-2 = limiter calls at the cell + Riemann compares at the face i+1/2 along x / y / z, slot 3 =
+    the floors of prim().  Test infrastructure for the VJP parity check (dh_oracle.hpp, "Decision margins")."""
+    lib = _load()
+    U = _f64(U)
+    M = np.empty((4,) + U.shape[1:], dtype=np.float64)
+    lib.dho_decision_margins(*_dims(U), ctypes.byref(p), _ptr(U), _ptr(M))
+    return M
+
+
+def cooling_margins(U1, dt, p):
+    """[nz, ny, nx]: margins of the compares of the cooling update applied to the pre-cooling state U1."""
+    lib = _load()
+    U1 = _f64(U1)
+    M = np.empty(U1.shape[1:], dtype=np.float64)
+    lib.dho_cooling_margins(*_dims(U1), ctypes.byref(p), ctypes.c_double(dt), _ptr(U1), _ptr(M))
+    return M
+
+
 def window_step(U_full, dt, p, lo, size, halo=4):
     """Windowed oracle: one step has a finite domain of dependence (+-4 cells per
     axis), so stepping a periodic-wrapped window of `size`+2*halo cells is exact on its interior.

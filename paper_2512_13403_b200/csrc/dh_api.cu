@@ -100,6 +100,17 @@ static void prof_drop(dh_ctx* c) {
   c->prof_n = 0;
 }
 
+// A context lives on the device that was current at dh_create (its scratch, its kernels' attributes): calling it with
+// another device current would launch there on foreign pointers.
+static int check_device(const dh_ctx* c, const char* who) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) {
+    snprintf(g_err, sizeof(g_err), "%s: the context belongs to device %d but device %d is current (cudaSetDevice first)", who, c->device, dev);
+    return DH_ERR_ARG;
+  }
+  return DH_OK;
+}
+
 extern "C" {
 
 const char* dh_last_error(void) { return g_err; }
@@ -125,6 +136,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
+  c->device = dev;
   cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
   if (c->sm_count <= 0) c->sm_count = 148;
   bool ok = cudaMalloc(&c->Us, state_bytes(c)) == cudaSuccess;
@@ -176,12 +188,12 @@ int dh_set_option(dh_ctx* c, int key, double v) {
       if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: box length must be > 0%s");
       c->L[key - DH_OPT_LX] = v; break;
     case DH_OPT_COOLING: c->cooling = (v != 0.0); break;
-    case DH_OPT_LAMBDA0: c->lambda0 = v; break;
-    case DH_OPT_ALPHA: c->alpha = v; break;
-    case DH_OPT_T_FLOOR: c->t_floor = v; break;
+    case DH_OPT_LAMBDA0: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: lambda0 must be >= 0%s"); c->lambda0 = v; break;
+    case DH_OPT_ALPHA: c->alpha = v; break;   /* any finite exponent; the rate is 0 for T <= 0 whatever alpha (cool_rate) */
+    case DH_OPT_T_FLOOR: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: t_floor must be >= 0%s"); c->t_floor = v; break;
     case DH_OPT_RHO_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->rho_floor = v; break;
     case DH_OPT_P_FLOOR: if (v <= 0) return fail(DH_ERR_ARG, "dh_set_option: floors must be > 0%s"); c->p_floor = v; break;
-    case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0, 1 or 2%s"); c->kernel = (int)v; break;
+    case DH_OPT_KERNEL: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: kernel must be 0 or 1%s"); c->kernel = (int)v; break;
     case DH_OPT_REV_SLAB: if (v < 0 || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: rev_slab must be a non-negative integer%s"); c->rev_slab_opt = (int)v; break;
     case DH_OPT_LIMITER: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: limiter must be 0, 1 or 2%s"); c->limiter = (int)v; break;
     case DH_OPT_INTEGRATOR: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: integrator must be 0, 1 or 2%s"); c->integrator = (int)v; break;
@@ -322,14 +334,6 @@ static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void*
       if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
       done = true;
       c->cand_ok = p.cand_list != nullptr;      // only this kernel pushes candidates
-    }
-  }
-  if (!done && c->kernel != 1 && c->riemann == 0) {      // the first fused kernel has the HLLC flux only
-    bool supported = false;
-    cudaError_t e = launch_stage_fused<T>(p, c->limiter, c->sm_count, c->stream, &supported);
-    if (supported) {
-      if (e != cudaSuccess) return cuda_fail(e, "dh_step: fused stage kernel launch");
-      done = true;
     }
   }
   if (!done) DH_CUDA(launch_stage_naive<T>(p, c->limiter, c->riemann, c->stream), "dh_step: stage kernel launch");
@@ -564,6 +568,7 @@ extern "C" {
 
 int dh_cfl_dt_async(dh_ctx* c, const void* U) {
   if (!c || !U) return fail(DH_ERR_ARG, "dh_cfl_dt: NULL argument%s");
+  if (int drc = check_device(c, "dh_cfl_dt_async")) return drc;
   return c->dtype == DH_F32 ? cfl_launch<float>(c, U) : cfl_launch<double>(c, U);
 }
 
@@ -585,6 +590,7 @@ int dh_cfl_dt(dh_ctx* c, const void* U, double* dt_out) {
 
 int dh_step(dh_ctx* c, void* U, double dt) {
   if (!c || !U) return fail(DH_ERR_ARG, "dh_step: NULL argument%s");
+  if (int drc = check_device(c, "dh_step")) return drc;
   if (!(dt > 0.0) || !isfinite(dt)) return fail(DH_ERR_ARG, "dh_step: dt must be finite and > 0%s");
   if (U == c->Us) return fail(DH_ERR_ARG, "dh_step: U aliases library scratch%s");
   return c->dtype == DH_F32 ? step_impl<float>(c, U, dt, false) : step_impl<double>(c, U, dt, false);
@@ -592,11 +598,13 @@ int dh_step(dh_ctx* c, void* U, double dt) {
 
 int dh_step_devdt(dh_ctx* c, void* U) {
   if (!c || !U) return fail(DH_ERR_ARG, "dh_step_devdt: NULL argument%s");
+  if (int drc = check_device(c, "dh_step_devdt")) return drc;
   return c->dtype == DH_F32 ? step_impl<float>(c, U, 0.0, true) : step_impl<double>(c, U, 0.0, true);
 }
 
 int dh_step_vjp(dh_ctx* c, const void* U, double dt, const void* gout, void* gin) {
   if (!c || !U || !gout || !gin) return fail(DH_ERR_ARG, "dh_step_vjp: NULL argument%s");
+  if (int drc = check_device(c, "dh_step_vjp")) return drc;
   if (!(dt > 0.0) || !isfinite(dt)) return fail(DH_ERR_ARG, "dh_step_vjp: dt must be finite and > 0%s");
   if (gin == U || gin == gout) return fail(DH_ERR_ARG, "dh_step_vjp: gU_in must not alias U or gU_out%s");
   return c->dtype == DH_F32 ? vjp_impl<float>(c, U, dt, gout, gin) : vjp_impl<double>(c, U, dt, gout, gin);
@@ -604,6 +612,7 @@ int dh_step_vjp(dh_ctx* c, const void* U, double dt, const void* gout, void* gin
 
 int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
   if (!c || !U || nsteps < 0) return fail(DH_ERR_ARG, "dh_advance: bad argument%s");
+  if (int drc = check_device(c, "dh_advance")) return drc;
   if (U == c->Us) return fail(DH_ERR_ARG, "dh_advance: U aliases library scratch%s");
   const bool f32 = c->dtype == DH_F32;
   // From the second step on, the CFL pass runs on the candidates the previous last stage pushed (DH_OPT_FUSE_CFL)
@@ -640,6 +649,7 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
 
 int dh_cool_tmin(dh_ctx* c, const void* U, double* tcool_min_out, double* dt_hydro_out) {
   if (!c || !U || !tcool_min_out) return fail(DH_ERR_ARG, "dh_cool_tmin: NULL argument%s");
+  if (int drc = check_device(c, "dh_cool_tmin")) return drc;
   int rc = c->dtype == DH_F32 ? cfl_launch<float>(c, U, false, true) : cfl_launch<double>(c, U, false, true);
   if (rc) return rc;
   rc = dh_poll_status(c, nullptr);
@@ -660,6 +670,7 @@ int dh_cfl_stats(dh_ctx* c, unsigned long long* out) {
 
 int dh_adjoint(dh_ctx* c, void* U, void* gU, int nsteps, int every, double* dts_out) {
   if (!c || !U || !gU || nsteps < 0 || every < 1) return fail(DH_ERR_ARG, "dh_adjoint: bad argument%s");
+  if (int drc = check_device(c, "dh_adjoint")) return drc;
   if (U == gU || U == c->Us || gU == c->Us) return fail(DH_ERR_ARG, "dh_adjoint: U and gU must be distinct caller arrays%s");
   if (nsteps == 0) return DH_OK;
   if (every > nsteps) every = nsteps;
@@ -735,6 +746,7 @@ int dh_adjoint(dh_ctx* c, void* U, void* gU, int nsteps, int every, double* dts_
 
 int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {
   if (!c || !U_host || nsteps < 0) return fail(DH_ERR_ARG, "dh_run_host: bad argument%s");
+  if (int drc = check_device(c, "dh_run_host")) return drc;
   int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
   if (rc) return rc;
   DH_CUDA(cudaMemcpyAsync(c->Uhost_dev, U_host, state_bytes(c), cudaMemcpyHostToDevice, c->stream), "dh_run_host: H2D");
@@ -746,6 +758,7 @@ int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {
 
 int dh_step_vjp_host(dh_ctx* c, const void* U_host, double dt, const void* gout_host, void* gin_host) {
   if (!c || !U_host || !gout_host || !gin_host) return fail(DH_ERR_ARG, "dh_step_vjp_host: NULL argument%s");
+  if (int drc = check_device(c, "dh_step_vjp_host")) return drc;
   int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
   if (rc) return rc;
   rc = lazy_alloc(c, &c->gA, state_bytes(c), "the device cotangent (in)");

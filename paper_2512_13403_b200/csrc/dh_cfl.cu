@@ -69,7 +69,7 @@ __device__ __noinline__ double cell_tcool(double rho, double mx, double my, doub
   const double Eth = Ieee::sub(E, Ek);
   const double Tc = Ieee::div(Ieee::mul(gm1d, Eth), rho);
   const double Tpos = (Tc > 0.0) ? Tc : 0.0;
-  const double rate = Ieee::mul(Ieee::mul(Ieee::mul(rho, rho), lambda0), pow(Tpos, alpha));
+  const double rate = Ieee::mul(Ieee::mul(Ieee::mul(rho, rho), lambda0), Tc > 0.0 ? pow(Tpos, alpha) : 0.0);   // rate 0 for T <= 0, as cool_rate()
   const double t = Ieee::div(fabs(Eth), fabs(rate));
   return (rate != 0.0 && t < tmin) ? t : tmin;
 }

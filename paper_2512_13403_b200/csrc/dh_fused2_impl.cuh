@@ -408,11 +408,13 @@ template <class T, int LIM, int RS, int NRW, bool V16, bool CAND>
 cudaError_t launch_one2c(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   using G = Geo2<NRW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
-  static bool configured = false;     // per instantiation; the attribute is per function and sticks
-  if (!configured) {
+  static bool configured[64] = {};    // per instantiation and per device: the attribute belongs to the (function, device) pair
+  int cur_dev = 0;
+  cudaGetDevice(&cur_dev);
+  if (cur_dev < 0 || cur_dev >= 64 || !configured[cur_dev]) {
     cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
   const int bx = (p.nx + TX2 - 1) / TX2, by = (p.ny + G::TY - 1) / G::TY;
   // z chunks: every chunk pays 4 lead-in planes, and blocks run in waves of (blocks per SM) x sm_count;

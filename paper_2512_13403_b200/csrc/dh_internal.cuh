@@ -114,6 +114,7 @@ struct Ctx {
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
   int sm_count;
+  int device;              // the device the context was created on; every entry point checks it is current
   void* Us;                    // U* scratch (always)
   void* gs;                    // cotangent of U* (first VJP)
   void* Ub;                    // base-state combination (Heun / SSPRK3); reused as the scaled cotangent in their VJP
@@ -159,7 +160,6 @@ size_t elem_size(const Ctx* c);
 
 // launchers (each returns the cudaError_t of the launch)
 template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, int riemann, cudaStream_t s);
-template <class T> cudaError_t launch_stage_fused(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s, bool* supported);
 template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);

@@ -204,14 +204,19 @@ DH_DI void riemann2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T
 // cooling of two finished cells (Eqs. 23-24); per lane
 // CFL candidate test (dh_advance): an estimate of max_a |v_a| + c_s for the two cells of a pack of CONSERVED values in
 // fast math (Eq. A8; dh_cfl.cu evaluates the exact recipe on the packs that pass).  No selects: the pressure floor
-// enters as a sum (an upper bound of the recipe's max), a density at or below zero, a negative internal energy and
-// any NaN / Inf turn the estimate into NaN or Inf, and `!(s < thr)` makes such a pack a candidate.
+// enters as a sum on top of max(e_int, 0) (an upper bound of the recipe's max(P, P_floor)), a density at or below zero
+// and any NaN / Inf turn the estimate into NaN or Inf, and `!(s < thr)` makes such a pack a candidate.
 template <class T>
 DH_DI bool cfl_candidate2(const P2<T> U[5], const Consts<T>& c, T thr) {
   const P2<T> r = rcp2(U[0]);
   const P2<T> q = fma2(U[3], U[3], fma2(U[2], U[2], mul2(U[1], U[1])));
-  const P2<T> ei = fma2(bc2(T(-0.5)), mul2(q, r), U[4]);
-  const P2<T> c2 = mul2(fma2(bc2(c.gamma * c.gm1), ei, bc2(c.gamma * c.p_floor)), r);
+  // an internal energy between -p_floor / (gamma - 1) and 0 must not lower the estimate below the recipe's floored
+  // pressure: clamp it at zero before the floor is added (a negative e_int is then simply a floored cell)
+  // (a select, not a max: a NaN must stay a NaN; E = -Inf would be clamped away, so 0 * E, which is NaN for any
+  // non-finite E, rides on the floor term)
+  const P2<T> er = fma2(bc2(T(-0.5)), mul2(q, r), U[4]);
+  const P2<T> ei = {er.x < T(0) ? T(0) : er.x, er.y < T(0) ? T(0) : er.y};
+  const P2<T> c2 = mul2(fma2(bc2(c.gamma * c.gm1), ei, fma2(U[4], bc2(T(0)), bc2(c.gamma * c.p_floor))), r);
   const P2<T> cs = mul2(c2, rsqrt2(c2));
   const T mx = max_(max_(abs_(U[1].x), abs_(U[2].x)), abs_(U[3].x));
   const T my = max_(max_(abs_(U[1].y), abs_(U[2].y)), abs_(U[3].y));

@@ -568,11 +568,13 @@ cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream
   constexpr int NW = sizeof(T) == 4 ? 8 : 6;      // fp64 (parity only): 5 row warps so that shared memory fits
   using G = GeoR<NW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
-  static bool configured = false;
-  if (!configured) {
+  static bool configured[64] = {};    // per device: the attribute belongs to the (function, device) pair
+  int cur_dev = 0;
+  cudaGetDevice(&cur_dev);
+  if (cur_dev < 0 || cur_dev >= 64 || !configured[cur_dev]) {
     cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
   const int bx = (p.nx + RTX - 1) / RTX, by = (p.ny + G::TY - 1) / G::TY;
   // z chunks: waves of sm_count blocks (one block per SM), 4 lead-in planes per chunk

@@ -26,7 +26,7 @@ LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
 COOL_MODES = {"euler": 0, "trapezoid": 1}           # DH_OPT_COOL_MODE
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
-KERNELS = {"fused": 0, "gather": 1, "fused1": 2}
+KERNELS = {"fused": 0, "gather": 1}
 
 # every symbol include/dh.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
