@@ -86,17 +86,22 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md, MEASURED_PEAKS.json absent)"
 
 
-def committed_traffic(n: int):
-    """DRAM bytes per stage-kernel launch from the committed ncu --set full capture (profiles/traffic.json:
-    {"<n>": bytes}), or None."""
+def committed_capture(n: int):
+    """What the committed `ncu --set full` capture of the stage kernel says for an n^3 grid (profiles/traffic.json, written
+    from the .ncu-rep by hand-run commands named in the profiles/*.md beside it; the entry records the commit it was
+    taken at): DRAM bytes per launch averaged over the predictor and corrector launches (like `achieved`), and the
+    hardware counters of the same launches.  None when no capture of this size is committed."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
             d = json.load(f)
-        a, b = d.get(str(n)), d.get(f"{n}_corrector")
-        # `achieved` averages the predictor and corrector launches, so the traffic figure does too
-        return 0.5 * (a + b) if (a is not None and b is not None) else a
+        e = d.get("stage", {}).get(str(n))
+        if not e:
+            return None, None
+        traffic = 0.5 * (e["predictor"]["dram_bytes"] + e["corrector"]["dram_bytes"])
+        return traffic, {"kind": "ncu hardware counters of the committed capture, not of this run", "source": e.get("source"),
+                         "commit": e.get("commit"), "predictor": e["predictor"], "corrector": e["corrector"]}
     except Exception:
-        return None
+        return None, None
 
 
 class ClockSampler:
@@ -336,31 +341,34 @@ def run_dh(a):
     st_cnt = prof["stage1"][1] + prof["stage2"][1]
     st_bytes = 4.0 * N * (STAGE_WORDS["stage1"] * prof["stage1"][1] + STAGE_WORDS["stage2"] * prof["stage2"][1])
     achieved = st_bytes / (st_ms * 1e-3) / 1e9
+    # bytes the step really has to move: 20 words per cell in the stages; the 5 words of the CFL pass only in the steps
+    # whose dt came from a full reduction (first step of a dh_advance call, fallbacks of the candidate path)
+    cstats = s.cfl_stats()
+    full_passes = prof["cfl_reduce"][1] + (cstats["fallbacks"] if prof["cfl_cand"][1] else 0)
+    step_bytes = 4.0 * N * ((fwd_words - 5) * K + 5 * full_passes)
+    traffic, counters = committed_capture(n)
+
+    def per_kernel(pr):
+        out = {}
+        for k, v in pr.items():
+            if v[1] == 0:
+                continue
+            e = {"ms_per_launch": v[0] / v[1], "launches": v[1], "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
+            if k == "cfl_cand":
+                e["note"] = "exact recipe on the listed packs + guarded full pass (returns at once unless a fallback is needed): no fixed byte count"
+            out[k] = e
+        return out
+
     roofline = {"bound": "hbm", "kernel": "stage kernel (predictor + corrector launches of the same kernel)",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": committed_traffic(n), "bytes_per_launch": st_bytes / max(st_cnt, 1),
+                "traffic": traffic, "bytes_per_launch": st_bytes / max(st_cnt, 1),
                 "ms_per_launch": st_ms / max(st_cnt, 1),
-                "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
-                                   "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
-                               for k, v in prof.items() if v[1] > 0},
-                "step_GB/s": fwd_words * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9,
-                "step_frac": fwd_words * 4.0 * N * K / (ms_fwd * 1e-3) / 1e9 / peak}
-
-    # the same kernel against its dispatch (operand-read) bound: modelled dispatch cycles per launch from the
-    # committed capture (profiles/r01f_dispatch_model.md) / (schedulers x SM clock x measured launch time)
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            disp = json.load(f).get(f"dispatch_cycles_{n}")
-    except Exception:
-        disp = None
-    if disp is not None:
-        sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
-        mhz = (clocks or {}).get("sm_mhz") or 1965.0
-        peak_disp = 4 * sm_count * mhz * 1e6                       # dispatch cycles per second, all schedulers
-        ach = disp / (st_ms / max(st_cnt, 1) * 1e-3)
-        roofline["alu"] = {"bound": "alu", "what": "dispatch (register operand read) cycles of the stage kernel",
-                           "achieved": ach, "peak": peak_disp, "unit": "dispatch cycles/s", "frac": ach / peak_disp,
-                           "peak_source": f"4 schedulers x {sm_count} SMs x {mhz:.0f} MHz (sampled clock)"}
+                "per_kernel": per_kernel(prof),
+                "step_GB/s": step_bytes / (ms_fwd * 1e-3) / 1e9,
+                "step_frac": step_bytes / (ms_fwd * 1e-3) / 1e9 / peak,
+                "step_bytes_note": f"{fwd_words - 5} words/cell/step + 5 words/cell for each of the {full_passes} full CFL passes in the {K} timed steps"}
+    if counters is not None:
+        roofline["counters"] = counters
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
@@ -373,7 +381,7 @@ def run_dh(a):
                        "dt_last": dt_last},
             "roofline": roofline, "clocks": clocks, "gpu_launches": launches}
     s.profile(False)
-    line["config"]["cfl_candidate_path"] = s.cfl_stats()      # dh_advance: dt's from candidate lists / fallbacks / packs
+    line["config"]["cfl_candidate_path"] = cstats             # dh_advance: dt's from candidate lists / fallbacks / packs
 
     # ---- VJP of the step, same state, seeded Gaussian cotangent on all five fields (configs[4])
     if not a.no_vjp:
@@ -396,9 +404,7 @@ def run_dh(a):
                        "roofline": {"bound": "hbm", "achieved": vjp_words * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9, "peak": peak,
                                     "unit": "GB/s", "frac": vjp_words * 4.0 * N * Kv / (ms_v * 1e-3) / 1e9 / peak,
                                     "words_per_cell": vjp_words,
-                                    "per_kernel": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1],
-                                                       "GB/s": gbs(STAGE_WORDS[k], v[0], v[1]) if k in STAGE_WORDS else None}
-                                                   for k, v in pv.items() if v[1] > 0}}}
+                                    "per_kernel": per_kernel(pv)}}
         line["gpu_launches"] += launches_v
         del g, gin
         torch.cuda.empty_cache()

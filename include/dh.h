@@ -184,7 +184,7 @@ unsigned long long dh_launch_count(const dh_ctx* ctx);
  * synchronises the stream and ADDS the elapsed milliseconds / launch counts recorded since the last read into
  * ms_out[DH_K_COUNT_] / launches_out[DH_K_COUNT_] (HOST arrays the caller zeroes; either may be NULL). */
 enum {
-  DH_K_CFL_REDUCE = 0,   /* max-wavespeed reduction, Eq. A8 */
+  DH_K_CFL_REDUCE = 0,   /* max-wavespeed reduction, Eq. A8: the full pass over the five fields (20 B/cell) */
   DH_K_CFL_FINISH = 1,   /* one-thread dt epilogue */
   DH_K_STAGE1 = 2,       /* predictor stage  U* = U^n - dt/2 D(U^n) */
   DH_K_STAGE2 = 3,       /* corrector stage  U^{n+1} = U^n - dt D(U*) (+ cooling) */
@@ -193,7 +193,9 @@ enum {
   DH_K_COOL_VJP = 6,     /* pointwise cooling adjoint */
   DH_K_LINCOMB = 7,      /* out = a X + b Y: base states / scaled cotangents of Heun and SSPRK3 */
   DH_K_COOL = 8,         /* in-place cooling pass of DH_OPT_COOL_MODE = 1 / DH_OPT_COOL_NSUB > 1 */
-  DH_K_COUNT_ = 9
+  DH_K_CFL_CAND = 9,     /* dh_advance, steps 2..: exact recipe on the listed candidate packs + the guarded full pass
+                            (which returns at once unless the list cannot settle the maxima: dh_cfl_stats counts those) */
+  DH_K_COUNT_ = 10
 };
 int dh_profile_enable(dh_ctx* ctx, int on);
 int dh_profile_read(dh_ctx* ctx, double* ms_out, unsigned long long* launches_out);

@@ -289,7 +289,7 @@ static int cfl_launch(dh_ctx* c, const void* U, bool cand = false, bool force_tc
   p.result = c->result_dev;
   p.cand_list = c->cand_list; p.cand_cnt = c->cand_cnt; p.cand_thr = (T*)c->cand_thr; p.cand_cap = c->cand_cap; p.cand_stats = c->cand_stats;
   {
-    ProfScope ps(c, DH_K_CFL_REDUCE);
+    ProfScope ps(c, cand ? DH_K_CFL_CAND : DH_K_CFL_REDUCE);
     if (cand) {
       DH_CUDA(launch_cfl_candidates<T>(p, c->sm_count, c->stream), "dh_advance: CFL candidate kernel launch");
       c->launches += 2;

@@ -39,7 +39,7 @@ SYMBOLS = [
 ]
 MG_OPTIONS = {"nu1": 0, "nu2": 1, "gamma": 2, "nu_coarse": 3, "omega": 4, "graph": 5}
 MG_CYCLES = {"V": 1, "W": 2}
-KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb", "cool"]
+KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb", "cool", "cfl_cand"]
 
 _lib = None
 

@@ -83,7 +83,7 @@ def test_config1_smooth_waves_fp64_ten_steps(kernel):
         U_ref = U_new
     drift = max_rel_err(U_free.cpu().numpy(), U_ref)
     assert drift <= 1e-10, drift
-    print(f"config1 [{kernel}] worst per-step rel err {worst:.3e}, free-running drift after 49 steps {drift:.3e}")
+    print(f"config1 [{kernel}] worst per-step rel err {worst:.3e}, free-running drift after 10 steps {drift:.3e}")
 
 
 # ------------------------------------------------------------------------- generic shapes / dtypes
@@ -648,14 +648,26 @@ def _random_state_device(n, seed, gamma, mach=0.7):
 
 
 def _check_vjp_windows(s, U, dt, g, gin, p, los, size, label, max_excluded):
+    """Entry by entry on windows (tests/vjp_margins.py).  Where a window is ill conditioned throughout (a smooth state
+    on a fine grid puts a near-tie into almost every stencil) the entries are additionally held in the weak sense:
+    moving a slope cotangent by one cell is a zero-sum dipole, second order against smooth test fields."""
     worst, excl = 0.0, []
+    kk, jj, ii = np.meshgrid(*(np.arange(m) for m in size), indexing="ij")
+    tests = [np.sin(2 * np.pi * (kk + 0.3) / size[0]) * np.cos(2 * np.pi * jj / size[1]) + np.sin(2 * np.pi * ii / size[2] + 1.0),
+             np.cos(2 * np.pi * (kk + jj) / size[0]) + 0.5 * np.sin(2 * np.pi * (ii - jj) / size[2] + 0.4),
+             np.ones(size)]
     for lo in los:
         Uw, gw = _window(U, lo, size, 8), _window(g, lo, size, 8)
         ref = oracle.step_vjp(Uw, dt, gw, p)[:, 8:-8, 8:-8, 8:-8]
         cond = vjp_margins.vjp_condition(Uw, dt, p)[8:-8, 8:-8, 8:-8]
-        w, e = vjp_margins.check_vjp(_window(gin, lo, size, 0), ref, cond, 2e-5, label=f"{label} window {lo}")
+        got = _window(gin, lo, size, 0)
+        w, e = vjp_margins.check_vjp(got, ref, cond, 2e-5, label=f"{label} window {lo}")
         worst = max(worst, w)
         excl.append(e)
+        for v in tests:
+            for f in range(5):
+                weak = abs(float(((got[f] - ref[f]) * v).sum())) / np.sqrt(float((ref[f] ** 2).sum() * (v ** 2).sum()))
+                assert weak <= 2e-3, (label, lo, f, weak)
     print(f"{label}: worst well-conditioned entry {worst:.3e}; excluded share per window min {min(excl):.3f} "
           f"mean {np.mean(excl):.3f} max {max(excl):.3f}")
     assert np.mean(excl) <= max_excluded, (label, excl)
