@@ -426,11 +426,13 @@ static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const v
   return DH_OK;
 }
 
-// Fused reversed stage (dh_rev.cu): per z slab, the face-adjoint sweep over the slab plus one plane on each side,
-// then the gather over the slab.  The scratch (20 words per cell of a slab) is allocated on first use.
+// Fused reversed stage (dh_rev.cu): per z slab, the face-adjoint sweep over the slab (it reads 3 planes on each side), then
+// the gather over the slab.  The scratch (10 words per cell of a slab + the tile-edge array) is allocated on first use.
 template <class T>
 static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
   const size_t NP = (size_t)c->nx * c->ny;
+  const int ntx = (c->nx + 63) / 64;                       // tiles per row of rev_faces_kernel (RTX = 64)
+  const size_t EP = (size_t)c->ny * ntx * 2;               // tile-edge words per plane and field
   const int want = c->rev_slab_opt > 0 ? (c->rev_slab_opt < c->nz ? c->rev_slab_opt : c->nz) : 0;
   if (c->rev_scratch && want > 0 && want != c->rev_slab) {      // the option changed: resize
     DH_CUDA(cudaStreamSynchronize(c->stream), "dh_step_vjp: synchronize");
@@ -438,38 +440,39 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
     c->rev_scratch = nullptr;
   }
   if (!c->rev_scratch) {
-    const size_t per_plane = 20 * NP * elem_size(c);
+    const size_t per_plane = (10 * NP + 5 * EP) * elem_size(c);
     long long planes = want;
     if (planes == 0) {
       size_t free_b = 0, total_b = 0;
       if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)8 << 30; }
-      size_t budget = (size_t)32 << 30;
-      if (budget > free_b / 2) budget = free_b / 2;
-      planes = (long long)(budget / per_plane) - 2;
+      size_t budget = (size_t)48 << 30;                    // one slab at 1024^3 fp32 (43 GB) when the memory is there
+      if (budget > free_b / 10 * 7) budget = free_b / 10 * 7;
+      planes = (long long)(budget / per_plane);
       if (planes > c->nz) planes = c->nz;
     }
     if (planes < 1) return fail(DH_ERR_ALLOC, "dh_step_vjp: not enough device memory for the reverse-stage scratch%s");
-    int rc = lazy_alloc(c, &c->rev_scratch, (size_t)(planes + 2) * per_plane, "the reverse-stage scratch");
+    int rc = lazy_alloc(c, &c->rev_scratch, (size_t)planes * per_plane, "the reverse-stage scratch");
     if (rc) return rc;
     c->rev_slab = (int)planes;
   }
-  const int SP = c->rev_slab + 2;
+  const int SP = c->rev_slab;
   const int n[3] = {c->nx, c->ny, c->nz};
   RevFaceParams<T> a;
   a.U = (const T*)U; a.g = (const T*)g;
   a.Wp = (T*)c->rev_scratch;
   a.C = a.Wp + (size_t)5 * SP * NP;
+  a.Ce = a.C + (size_t)5 * SP * NP;
   a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
-  a.sp0 = 0; a.SP = SP;
+  a.sp0 = 0; a.SP = SP; a.ntx = ntx; a.SPE = (size_t)SP * EP;
   for (int k = 0; k < 3; ++k) a.coef[k] = (T)(frac * dt * n[k] / c->L[k]);
   a.c = make_consts<T>(c);
   RevGatherParams<T> b;
-  b.U = (const T*)U; b.Wp = a.Wp; b.C = a.C; b.b1 = (const T*)b1; b.b2 = (const T*)b2; b.out = (T*)out;
-  b.nx = c->nx; b.ny = c->ny; b.nz = c->nz; b.sp0 = 1; b.SP = SP; b.c = a.c;
+  b.U = (const T*)U; b.Wp = a.Wp; b.C = a.C; b.Ce = a.Ce; b.b1 = (const T*)b1; b.b2 = (const T*)b2; b.out = (T*)out;
+  b.nx = c->nx; b.ny = c->ny; b.nz = c->nz; b.sp0 = 0; b.SP = SP; b.ntx = ntx; b.SPE = a.SPE; b.c = a.c;
   ProfScope ps(c, kind);
   for (int z0 = 0; z0 < c->nz; z0 += c->rev_slab) {
     const int nplanes = (c->nz - z0 < c->rev_slab) ? c->nz - z0 : c->rev_slab;
-    a.zs = z0 - 1; a.nout = nplanes + 2;
+    a.zs = z0; a.nout = nplanes;
     DH_CUDA(launch_rev_faces<T>(a, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
     b.z0 = z0; b.nplanes = nplanes;
     DH_CUDA(launch_rev_gather<T>(b, c->stream), "dh_step_vjp: gather kernel launch");

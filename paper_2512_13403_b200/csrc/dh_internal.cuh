@@ -44,17 +44,22 @@ struct RevParams {
   Consts<T> c;
 };
 
-// Parameters of the two launches of a fused reversed stage (dh_rev.cu).  Scratch: Wp [5][SP][ny][nx] and
-// C [3][5][SP][ny][nx]; scratch plane sp0 holds grid plane zs (faces) / z0 (gather).
+// Parameters of the two launches of a fused reversed stage (dh_rev.cu).  Scratch of a z slab of SP planes: Wp [5][SP][ny][nx]
+// (all cell terms except the y neighbour terms), C [5][SP][ny][nx] (encoded masked y slope cotangents) and
+// Ce [5][SP][ny][ntx][2] (encoded x slope cotangents of the first and last cell of every tile row: the two x terms that
+// cross a tile edge); scratch plane sp0 holds grid plane zs (faces) / z0 (gather).
 template <class T>
 struct RevFaceParams {
   const T* U;        // primal state the stage was evaluated at
   const T* g;        // cotangent of the stage output
   T* Wp;
   T* C;
+  T* Ce;
   int nx, ny, nz;
-  int zs, nout;      // first output plane (unwrapped: may be -1) and number of output planes
+  int zs, nout;      // first output plane and number of output planes
   int sp0, SP;
+  int ntx;           // tiles per row
+  size_t SPE;        // field pitch of Ce
   T coef[3];         // frac * dt / dx_a
   Consts<T> c;
 };
@@ -64,12 +69,15 @@ struct RevGatherParams {
   const T* U;
   const T* Wp;
   const T* C;
+  const T* Ce;
   const T* b1;       // optional additive terms (nullptr = none)
   const T* b2;
   T* out;
   int nx, ny, nz;
   int z0, nplanes;   // planes z0 .. z0 + nplanes - 1 (all inside [0, nz))
   int sp0, SP;
+  int ntx;
+  size_t SPE;
   Consts<T> c;
 };
 

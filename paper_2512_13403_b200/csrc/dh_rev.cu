@@ -15,11 +15,14 @@
 // the work is split in two launches that share a scratch slab:
 //   A  rev_faces_kernel   fused z-sweep (7 row warps x one pack + helper; z in registers, x / y through shared planes,
 //                         R states of the neighbouring cells recomputed locally, ONE block barrier per plane): every
-//                         face adjoint once; writes per cell  Wp = sum_a (T_i + own-branch term)  and, per axis, c_i = S_i
-//                         masked by (a b > 0), with the branch flag stored in the mantissa LSB (<= 1 ulp);
-//   B  rev_gather_kernel  streaming: Wb_i = Wp_i + sum_a [a-branch c_{i-1}] - [b-branch c_{i+1}], then
-//                         Ub = prim_vjp(U, Wb) + b1 + b2.
-// Scratch is 20 words per cell of a z slab (+1 plane on each side); the API layer walks the slabs.  minmod only
+//                         face adjoint once.  The neighbour terms along x are exchanged inside the warp (shuffles of the
+//                         masked slope cotangent c = S masked by a b > 0, branch flag in the mantissa LSB, <= 1 ulp) and
+//                         those along z stay in the sweep (a cell is stored one plane after its own z terms are known), so
+//                         per cell it writes  Wp = everything but the y neighbour terms  and  c^y; the x terms that cross a
+//                         tile edge go through a thin array of the tile rows' first and last c^x;
+//   B  rev_gather_kernel  streaming: Wb_i = Wp_i + [a-branch c^y_{j-1}] - [b-branch c^y_{j+1}] (+ the tile-edge x term),
+//                         then Ub = prim_vjp(U, Wb) + b1 + b2.
+// Scratch is 10 words per cell of a z slab (+ 10 / 64 for the tile edges); the API layer walks the slabs.  minmod only
 // (the branch flag is one bit); other limiters take the gather kernels.  No atomics; deterministic.
 #include "dh_internal.cuh"
 #include "dh_pack.cuh"
@@ -39,7 +42,8 @@ template <int NW> struct GeoR {
   static constexpr int XARR = 5 * TY * RXP;
   static constexpr int YARR = 5 * (TY + 1) * RTX;
   static constexpr int STAGE = 5 * TY * RTX;              // cp.async staging of one raw plane of the tile
-  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + 6 * STAGE;
+  static constexpr int NPARK = 8;                         // staging of the next raw plane + 7 parked carries
+  static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + NPARK * STAGE;
   static constexpr int NHALO = 4 * (RSW / 2) + 2 * TY;    // halo packs per plane
   static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
 };
@@ -84,6 +88,15 @@ template <class T> DH_DI void cell_terms2(P2<T> Lb, P2<T> Rbn, P2<T> k, P2<T>& w
   wp = fma2(k, D, add2(Lb, Rbn));
   const P2<T> c = mul2(P2<T>{abs_(k.x), abs_(k.y)}, D);
   ce = {enc_sign(c.x, k.x), enc_sign(c.y, k.y)};
+}
+
+// the same with the neighbour terms as plain values instead of the encoded c (used where they stay inside the kernel):
+// P = what the next cell along the axis receives (a-branch: S), M = what the previous cell loses (b-branch: S)
+template <class T> DH_DI void cell_terms_pm2(P2<T> Lb, P2<T> Rbn, P2<T> k, P2<T>& wp, P2<T>& P, P2<T>& M) {
+  const P2<T> D = sub2(Lb, Rbn);
+  wp = fma2(k, D, add2(Lb, Rbn));
+  P = mul2(P2<T>{max_(-k.x, T(0)), max_(-k.y, T(0))}, D);
+  M = mul2(max2(k, T(0)), D);
 }
 
 // HLLC adjoint of two faces: the scalar routine of dh_math.cuh on each half of the packs.  The loop over the halves
@@ -225,7 +238,24 @@ DH_DI void hllc_vjp2p(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, co
 
 }  // namespace
 
+// neighbour terms of an encoded masked slope cotangent c (flag in the LSB = a-branch): what cell i+1 receives from
+// cell i (+c on the a-branch) and what cell i-1 receives from cell i (-c on the b-branch; an inactive slope has c = 0)
+template <class T> DH_DI T pterm(T c) { return dec_flag(c) ? c : T(0); }
+template <class T> DH_DI T mterm(T c) { return dec_flag(c) ? T(0) : c; }
+template <class T> DH_DI P2<T> pterm2(P2<T> c) { return {pterm(c.x), pterm(c.y)}; }
+template <class T> DH_DI P2<T> mterm2(P2<T> c) { return {mterm(c.x), mterm(c.y)}; }
+DH_DI float shfl_up1(float v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+DH_DI float shfl_dn1(float v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+DH_DI double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+DH_DI double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
 // ------------------------------------------------------------------------------------------------ kernel A
+// Planes in flight at iteration `it` (plane p = first - 3 + it is loaded; `first` = first output plane of the block):
+//   p      raw state -> primitives -> shared plane; cotangent -> shared plane
+//   p-1    x and y face adjoints; after the block barrier its x terms are completed inside the warp (shuffles; the
+//          helper supplies the two cells beside the tile), its own y terms are added, its c^y goes to the scratch
+//   p-2    the z face above it is adjoined: its own z terms and the a-branch term of plane p-3 join the parked sum
+//   p-3    receives the b-branch term of plane p-2 and is stored: Wp' = everything except the y neighbour terms
 template <class T, int NW>
 __global__ void __launch_bounds__(NW * 32, 1)
 rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
@@ -234,10 +264,10 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
   constexpr int XF = TY * RXP, YF = (TY + 1) * RTX;       // field pitches of the exchange arrays
   extern __shared__ __align__(16) unsigned char smem_rev[];
   T* const Wsm = reinterpret_cast<T*>(smem_rev);   // [2][5][SR][RSW]  primitive planes p (it&1) and p-1
-  T* const Gsm = Wsm + 2 * G::PLANE;               // [2][5][SR][RSW]  cotangent planes p and p-1 (halo 1 used)
+  T* const Gsm = Wsm + 2 * G::PLANE;               // [2][5][SR][RSW]  cotangent planes p and p-1
   T* const Rxs = Gsm + 2 * G::PLANE;               // [2][5][TY][RXP]   Rb of the face LEFT of lane l's pack (slot 0: helper), by iteration parity
   T* const Rys = Rxs + 2 * G::XARR;                // [2][5][TY+1][RTX] Rb of the face BELOW row r (slot 0: helper), by iteration parity
-  T* const Ust = Rys + 2 * G::YARR;                    // [5][TY][RTX]     raw U of the next plane (cp.async, private slots)
+  T* const Ust = Rys + 2 * G::YARR;                // [NPARK][5][TY][RTX] raw U of the next plane (cp.async) and parked carries (private slots)
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -245,11 +275,11 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
   const int x0 = blockIdx.x * RTX, y0 = blockIdx.y * TY;
   const int zrel0 = blockIdx.z * ZL;               // first output plane of this block, relative to p.zs
   const int zl = min(ZL, p.nout - zrel0);
-  const int nit = zl + 4;                          // planes z0-2 .. z0+zl+1
+  const int nit = zl + 6;                          // planes first-3 .. first+zl+2
   const P2<T> cx = bc2(p.coef[0]), cy = bc2(p.coef[1]), cz = bc2(p.coef[2]);
   const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
   const Consts<T>& c = p.c;
-  int pz = wrapr(p.zs + zrel0 - 2, nz);
+  int pz = wrapr(p.zs + zrel0 - 3, nz);
 
   if (w < TY) {
     // ------------------------------------------------------------------------------------ row warp
@@ -259,21 +289,27 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
     const int so = (r + 2) * RSW + 2 * lane + 2;   // own pack inside a shared plane
     const int xo = r * RXP + lane, yo = r * RTX + 2 * lane;
     T* const ust = Ust + yo;
-    T* const pk1 = Ust + G::STAGE + yo;            // parked carries (private slots): Rb of the lower z face, x+y cell terms
-    T* const pk2 = Ust + 2 * G::STAGE + yo;
-    T* const pkx = Ust + 3 * G::STAGE + yo;           // parked minmod branch factors of the own cells: x, y, z
+    T* const pk1 = Ust + G::STAGE + yo;            // parked carries (private slots): Rb of the lower z face
+    T* const pk2 = Ust + 2 * G::STAGE + yo;        //   x (complete) + own y terms of plane p-1
+    T* const pkx = Ust + 3 * G::STAGE + yo;        //   minmod branch factors of the own cells: x, y, z
     T* const pky = Ust + 4 * G::STAGE + yo;
     T* const pkz = Ust + 5 * G::STAGE + yo;
+    T* const pkw = Ust + 6 * G::STAGE + yo;        //   sum of plane p-2 (still missing the b-branch term of the plane above)
+    T* const pkc = Ust + 7 * G::STAGE + yo;        //   a-branch z term of plane p-2 (for plane p-1)
     P2<T> Wprev[5], dprev[5], Lz[5], gpp[5];
 #pragma unroll
-    for (int f = 0; f < 5; ++f) { Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0)); rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); rsts2(pkz + f * FS, bc2(T(0))); }
+    for (int f = 0; f < 5; ++f) {
+      Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0));
+      rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); rsts2(pkz + f * FS, bc2(T(0)));
+      rsts2(pkw + f * FS, bc2(T(0))); rsts2(pkc + f * FS, bc2(T(0)));
+    }
     size_t op = (size_t)pz * NP + o;
 #pragma unroll
     for (int f = 0; f < 5; ++f) rcp_async_pack(ust + f * FS, p.U + f * N + op);
     rcp_async_commit();
     rcp_async_wait_all();
-    // scratch offset of the plane finished in iteration `it` (plane p-2): advanced by NP per iteration
-    long long os2 = ((long long)p.sp0 + zrel0 - 4) * (long long)NP + (long long)o;
+    // scratch offset of the plane stored in iteration `it` (plane p-3): advanced by NP per iteration
+    long long os3 = ((long long)p.sp0 + zrel0 - 6) * (long long)NP + (long long)o;
 
 #pragma unroll 1
     for (int it = 0; it < nit; ++it) {
@@ -281,7 +317,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
       T* const Wp_s = Wsm + bp * G::PLANE;
       const T* const Wq_s = Wsm + bq * G::PLANE;
       const T* const Gq_s = Gsm + bq * G::PLANE;
-      const bool xy = (it >= 3) && (it <= zl + 2);   // x/y work on plane p-1 is wanted
+      const bool xy = (it >= 4) && (it <= zl + 3);   // plane p-1 is an output plane: its c^y is wanted
       P2<T> Uc[5];
 #pragma unroll
       for (int f = 0; f < 5; ++f) Uc[f] = rlds2(ust + f * FS);
@@ -304,7 +340,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 #pragma unroll
       for (int f = 0; f < 5; ++f) gq[f] = rlds2(Gq_s + f * FP + so);
 
-      // ---- z: slope of plane p-1, adjoint of the face between p-2 and p-1, which completes the cell of plane p-2
+      // ---- z: slope of plane p-1, adjoint of the face between p-2 and p-1, which completes the z terms of plane p-2
       {
         P2<T> Rz[5], lam[5], Lb[5], Rb[5];
         P2<T> kz[5];
@@ -320,18 +356,19 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           gpp[f] = gq[f];
         }
         hllc_vjp2p<T, 2>(Lz, Rz, c, lam, Lb, Rb);
-        const bool stz = (it >= 4) && store_ok;
+        const bool stz = (it >= 6) && store_ok;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           Lz[f] = Wn[f];
-          P2<T> wp, ce;
-          cell_terms2(Lb[f], rlds2(pk1 + f * FS), rlds2(pkz + f * FS), wp, ce);   // cell of plane p-2: parked Rb and factor
+          P2<T> wp, Pz, Mz;
+          cell_terms_pm2(Lb[f], rlds2(pk1 + f * FS), rlds2(pkz + f * FS), wp, Pz, Mz);   // cell of plane p-2: parked Rb and factor
           rsts2(pk1 + f * FS, Rb[f]);
           rsts2(pkz + f * FS, kz[f]);
-          if (stz) {
-            rstg2(p.Wp + f * SPN + os2, add2(wp, rlds2(pk2 + f * FS)));
-            rstg2(p.C + (10 + f) * SPN + os2, ce);
-          }
+          const P2<T> Pprev = rlds2(pkc + f * FS);                                // a-branch term of plane p-3 for plane p-2
+          const P2<T> fin = sub2(rlds2(pkw + f * FS), Mz);                        // plane p-3 is complete (but for y)
+          rsts2(pkw + f * FS, add2(add2(wp, rlds2(pk2 + f * FS)), Pprev));
+          rsts2(pkc + f * FS, Pz);
+          if (stz) rstg2(p.Wp + f * SPN + os3, fin);
         }
       }
 
@@ -389,26 +426,38 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
       }
       rcp_async_wait_all();                         // cotangent plane p and the next raw plane have landed
       __syncthreads();
-      // ---- phase 3: cell cotangents of plane p-1 for x and y (the z part joins them in the next iteration)
+      // ---- phase 3: cell cotangents of plane p-1 for x (with the neighbour terms: lanes exchange their encoded c; the
+      // two terms that cross the tile edge are left to the gather kernel, which reads the edge cells' c from Ce) and y
       {
-        const bool stxy = xy && store_ok;
-        const long long os1 = os2 + (long long)NP;
+        const bool sty = xy && store_ok;
+        const long long os1 = os3 + 2 * (long long)NP;
+        // last lane of the row that holds a cell of this tile (beyond it the lanes hold the periodic images of the first
+        // cells, so the exchange across it is already the right one)
+        const int ll = (min(x0 + RTX, nx) - x0) / 2 - 1;
+        const bool edge_l = sty && lane == 0, edge_r = sty && lane == ll;
+        const long long oe = (((long long)p.sp0 + zrel0 + it - 4) * ny + wrapr(y0 + r, ny)) * (long long)(2 * p.ntx) + 2 * blockIdx.x;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          P2<T> wx, cex, wy, cey;
-          cell_terms2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, rlds2(pkx + f * FS), wx, cex);
+          P2<T> wx, Px, Mx, wy, cey;
+          const P2<T> kx = rlds2(pkx + f * FS);
+          cell_terms_pm2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, kx, wx, Px, Mx);
           cell_terms2(Lby[f], rlds2(By_s + f * YF + yo), rlds2(pky + f * FS), wy, cey);
+          T pl = shfl_up1(Px.y), mr = shfl_dn1(Mx.x);
+          if (lane == 0) pl = T(0);
+          if (lane == 31) mr = T(0);
+          wx.x += pl - Mx.y;
+          wx.y += Px.x - mr;
+          const P2<T> cex = {enc_sign(Px.x + Mx.x, kx.x), enc_sign(Px.y + Mx.y, kx.y)};   // for the tile-edge array only
           rsts2(pk2 + f * FS, add2(wx, wy));
-          if (stxy) {
-            rstg2(p.C + f * SPN + os1, cex);
-            rstg2(p.C + (5 + f) * SPN + os1, cey);
-          }
+          if (sty) rstg2(p.C + f * SPN + os1, cey);
+          if (edge_l) p.Ce[f * p.SPE + oe] = cex.x;
+          if (edge_r) p.Ce[f * p.SPE + oe + 1] = cex.y;
         }
       }
       // plane p becomes plane p-1
 #pragma unroll
       for (int f = 0; f < 5; ++f) Wprev[f] = rlds2(Wp_s + f * FP + so);
-      os2 += (long long)NP;
+      os3 += (long long)NP;
       op = opn;
       pz = pzn;
     }
@@ -509,7 +558,8 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 }
 
 // ------------------------------------------------------------------------------------------------ kernel B
-// One thread per pack (two x-adjacent cells) of a slab plane.
+// One thread per pack (two x-adjacent cells) of a slab plane: adds the y neighbour terms (rows j -+ 1 of C) and, for the
+// packs at a tile edge, the x term that crossed it (Ce), then Ub = prim_vjp(U, Wb) + b1 + b2.
 template <class T>
 __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T> p) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;       // pack index along x
@@ -518,29 +568,22 @@ __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T
   const int nx = p.nx, ny = p.ny;
   const size_t NP = (size_t)nx * ny, N = NP * p.nz, SPN = (size_t)p.SP * NP;
   const size_t row = (size_t)j * nx, rowm = (size_t)(j == 0 ? ny - 1 : j - 1) * nx, rowp = (size_t)(j == ny - 1 ? 0 : j + 1) * nx;
-  const size_t sp = (size_t)(p.sp0 + kz) * NP;                // scratch plane of this cell; its z neighbours are sp -+ NP
+  const size_t sp = (size_t)(p.sp0 + kz) * NP;                // scratch plane of this cell
   const size_t cell = (size_t)(p.z0 + kz) * NP + row + i;     // p.z0 + kz < nz by construction
-  const int im = (i == 0 ? nx - 1 : i - 1), ipl = (i + 2 >= nx ? 0 : i + 2);
+  const int tile = i / RTX, ti = i - tile * RTX;
+  const bool el = ti == 0, er = ti == RTX - 2;                // the pack holds the first / last cell of a full tile row
+  const int tl = tile == 0 ? p.ntx - 1 : tile - 1, tr = (i + 2 >= nx) ? 0 : tile + 1;
+  const size_t oe = ((size_t)(p.sp0 + kz) * ny + j) * (size_t)(2 * p.ntx);
   P2<T> Wb[5];
 #pragma unroll
   for (int f = 0; f < 5; ++f) {
     P2<T> w = rldg2(p.Wp + f * SPN + sp + row + i);
-    // x: a-branch of the cell to the left, b-branch of the cell to the right
-    const T* Cx = p.C + f * SPN + sp + row;
-    const P2<T> cxo = rldg2(Cx + i);
-    const T cl = Cx[im], cr = Cx[ipl];
-    w.x += (dec_flag(cl) ? cl : T(0)) - (dec_flag(cxo.y) ? T(0) : cxo.y);
-    w.y += (dec_flag(cxo.x) ? cxo.x : T(0)) - (dec_flag(cr) ? T(0) : cr);
-    // y
-    const T* Cy = p.C + (5 + f) * SPN + sp + i;
+    const T* Cy = p.C + f * SPN + sp + i;
     const P2<T> cd = rldg2(Cy + rowm), cu = rldg2(Cy + rowp);
-    w.x += (dec_flag(cd.x) ? cd.x : T(0)) - (dec_flag(cu.x) ? T(0) : cu.x);
-    w.y += (dec_flag(cd.y) ? cd.y : T(0)) - (dec_flag(cu.y) ? T(0) : cu.y);
-    // z
-    const T* Cz = p.C + (10 + f) * SPN + sp + row + i;
-    const P2<T> cb = rldg2(Cz - NP), ct = rldg2(Cz + NP);
-    w.x += (dec_flag(cb.x) ? cb.x : T(0)) - (dec_flag(ct.x) ? T(0) : ct.x);
-    w.y += (dec_flag(cb.y) ? cb.y : T(0)) - (dec_flag(ct.y) ? T(0) : ct.y);
+    w.x += pterm(cd.x) - mterm(cu.x);
+    w.y += pterm(cd.y) - mterm(cu.y);
+    if (el) w.x += pterm(p.Ce[f * p.SPE + oe + 2 * tl + 1]);
+    if (er) w.y -= mterm(p.Ce[f * p.SPE + oe + 2 * tr]);
     Wb[f] = w;
   }
   P2<T> U[5];
@@ -565,7 +608,7 @@ __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T
 // ------------------------------------------------------------------------------------------------ launchers
 template <class T>
 cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
-  constexpr int NW = sizeof(T) == 4 ? 8 : 6;      // fp64 (parity only): 5 row warps so that shared memory fits
+  constexpr int NW = sizeof(T) == 4 ? 8 : 5;      // fp64 (parity only): 4 row warps so that shared memory fits
   using G = GeoR<NW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
   static bool configured[64] = {};    // per device: the attribute belongs to the (function, device) pair
@@ -577,14 +620,14 @@ cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream
     if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
   const int bx = (p.nx + RTX - 1) / RTX, by = (p.ny + G::TY - 1) / G::TY;
-  // z chunks: waves of sm_count blocks (one block per SM), 4 lead-in planes per chunk
+  // z chunks: waves of sm_count blocks (one block per SM), 6 lead-in / lead-out planes per chunk
   const long long tiles = (long long)bx * by;
   int bz = 1;
   long long best = -1;
   for (int cand = 1; cand <= (p.nout + 3) / 4 && cand <= 65535; ++cand) {
     const int zl_c = (p.nout + cand - 1) / cand;
     if ((p.nout + zl_c - 1) / zl_c != cand) continue;
-    const long long cost = ((tiles * cand + sm_count - 1) / sm_count) * (zl_c + 4);
+    const long long cost = ((tiles * cand + sm_count - 1) / sm_count) * (zl_c + 6);
     if (best < 0 || cost < best) { best = cost; bz = cand; }
   }
   const int ZL = (p.nout + bz - 1) / bz;
