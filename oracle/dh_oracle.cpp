@@ -87,7 +87,7 @@ int dho_cooling(long long N, const Params* p, double dt, const double* U, double
   for (long long c = 0; c < N; ++c) {
     double u[5], o[5];
     for (int f = 0; f < 5; ++f) u[f] = U[f * N + c];
-    cool(u, dt, *p, o);
+    cool(u, dt, *p, p->tab, o);
     for (int f = 0; f < 5; ++f) Uout[f * N + c] = o[f];
   }
   return 0;
@@ -139,6 +139,23 @@ int dho_decision_margins(int nx, int ny, int nz, const Params* p, const double* 
 // margins of the compares of cool() at the pre-cooling state U1: M is [nz][ny][nx]
 int dho_cooling_margins(int nx, int ny, int nz, const Params* p, double dt, const double* U1, double* M) {
   cooling_margins(mkgrid(nx, ny, nz), *p, dt, U1, M);
+  return 0;
+}
+
+// Lambda-side pieces for the pins: Edot(E_th, rho) of cool_rate() and the tabulated Lambda_CIE(T) of Eq. 19
+double dho_cool_rate(const Params* p, double Eth, double rho) { return cool_rate<double>(Eth, rho, *p, p->tab); }
+double dho_lambda_table(const Params* p, double T) { return lambda_table<double>(T, *p, p->tab); }
+
+// gradient of sum(gout_E * E_out) with respect to the table nodes, at the pre-cooling state U1 (ntab <= 32)
+int dho_cooling_table_vjp(int nx, int ny, int nz, const Params* p, double dt, const double* U1, const double* gout, double* gtab) {
+  return cooling_table_vjp(mkgrid(nx, ny, nz), *p, dt, U1, gout, gtab);
+}
+
+// the pre-cooling state of a step (what cooling_vjp / cooling_table_vjp are evaluated at): the step with cooling off
+int dho_step_nocool(int nx, int ny, int nz, const Params* p, const double* U, double dt, double* Uout) {
+  Params q = *p;
+  q.cooling = 0;
+  step<double>(mkgrid(nx, ny, nz), q, U, dt, Uout);
   return 0;
 }
 

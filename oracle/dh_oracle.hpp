@@ -41,6 +41,16 @@ struct Params {
   double t_floor;     // temperature floor, Eq. 24 with R=1
   int cool_mode;      // 0: Euler + floor of Eq. 23, sub-cycled; 1: trapezoid of Eq. 22, reading A20
   int cool_nsub;      // N_sub >= 1 substeps of size dt / N_sub in mode 0
+  // --- the two-branch law of Eqs. 17-19 and the masked choice of integrator ---
+  int cool_law;       // 0: Lambda = lambda0 T^alpha, Gamma = 0 (reading A10); 1: Eq. 17: Koyama-Inutsuka fit + uniform heating below
+                      //    t_switch, tabulated Lambda_CIE above it (reading A25)
+  double t_switch;    // the 10^4 K of Eq. 17, in code units
+  double lambda1, alpha1, lambda2, alpha2;   // Eq. 18: Lambda_KI = lambda1 T^alpha1 + lambda2 T^alpha2
+  double gamma0;      // uniform heating rate Gamma_0 for T < t_switch; enters as n_H Gamma (Eq. 20)
+  const double* tab;  // log10 Lambda_CIE at the nodes log10 T = tab_logT0 + k tab_dlogT, k = 0 .. ntab-1 (Eq. 19)
+  int ntab;
+  double tab_logT0, tab_dlogT;
+  double f_sub;       // cool_mode 2: a cell is sub-cycled (Eq. 23) when dt |Edot(T^n)| > f_sub |E_th^n|, else Eq. 22 (reading A26)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -77,6 +87,11 @@ template <int N> inline double val(const Dual<N>& a) { return a.v; }
 inline double ssqrt(double a) { return std::sqrt(a); }
 inline float ssqrt(float a) { return std::sqrt(a); }
 template <int N> inline Dual<N> ssqrt(const Dual<N>& a) { Dual<N> r; r.v = std::sqrt(a.v); for (int i = 0; i < N; ++i) r.d[i] = a.d[i] / (2.0 * r.v); return r; }
+
+inline double slog10(double a) { return std::log10(a); }
+template <int N> inline Dual<N> slog10(const Dual<N>& a) { Dual<N> r; r.v = std::log10(a.v); for (int i = 0; i < N; ++i) r.d[i] = a.d[i] / (a.v * 2.302585092994045684); return r; }
+inline double spow10(double a) { return std::pow(10.0, a); }
+template <int N> inline Dual<N> spow10(const Dual<N>& a) { Dual<N> r; r.v = std::pow(10.0, a.v); for (int i = 0; i < N; ++i) r.d[i] = 2.302585092994045684 * r.v * a.d[i]; return r; }
 
 inline double spow(double a, double p) { return std::pow(a, p); }
 template <int N> inline Dual<N> spow(const Dual<N>& a, double p) { Dual<N> r; r.v = std::pow(a.v, p); double g = (a.v > 0.0) ? p * std::pow(a.v, p - 1.0) : 0.0; for (int i = 0; i < N; ++i) r.d[i] = g * a.d[i]; return r; }
@@ -228,28 +243,59 @@ inline void face_flux(const S Wm1[5], const S W0[5], const S Wp1[5], const S Wp2
 //   E_pred = max(E_floor, E_th^n + Edot(T^n) dt), and floors the result by Eq. 24 as well.
 // Floor: Eq. 24 with R = 1.
 // ------------------------------------------------------------------------------------------------
+// Lambda_CIE(T) of Eq. 19: linear interpolation in log10 T - log10 Lambda between the table nodes.
+// Reading A25: outside the table the end values are held (T >= t_switch >= first node in every use).
 template <class S>
-inline S cool_rate(const S& Eth, const S& rho, const Params& p) {
+inline S lambda_table(const S& T, const Params& p, const S* tab) {
+  S u = (slog10(T) - p.tab_logT0) / p.tab_dlogT;
+  int k = (int)std::floor(val(u));
+  if (k < 0) k = 0;
+  if (k > p.ntab - 2) k = p.ntab - 2;
+  S w = u - (double)k;
+  if (val(w) < 0.0) w = S(0.0);
+  if (val(w) > 1.0) w = S(1.0);
+  return spow10(S(tab[k] + w * (tab[k + 1] - tab[k])));
+}
+
+// Edot = n_H Gamma - n_H^2 Lambda (Eqs. 15, 20 with chi = 1) in code units n_H = rho, T = (gamma-1) E_th / rho
+template <class S>
+inline S cool_rate(const S& Eth, const S& rho, const Params& p, const S* tab) {
   S T = (p.gamma - 1.0) * Eth / rho;
   S Tpos = smax(T, S(0.0));
-  return -1.0 * rho * rho * p.lambda0 * spow(Tpos, p.alpha);
+  if (p.cool_law == 0) return -1.0 * rho * rho * p.lambda0 * spow(Tpos, p.alpha);
+  if (val(T) < p.t_switch)                                   // Eq. 17, lower branch: Eq. 18 and Gamma_0
+    return rho * p.gamma0 - rho * rho * (p.lambda1 * spow(Tpos, p.alpha1) + p.lambda2 * spow(Tpos, p.alpha2));
+  return -1.0 * rho * rho * lambda_table(T, p, tab);         // upper branch: Eq. 19, no heating
+}
+
+// the table as scalars of type S (constants unless the caller seeds derivative slots)
+template <class S>
+inline std::vector<S> table_as(const Params& p) {
+  std::vector<S> t((size_t)(p.cool_law == 1 && p.tab ? p.ntab : 0));
+  for (size_t k = 0; k < t.size(); ++k) t[k] = S(p.tab[k]);
+  return t;
 }
 
 template <class S>
-inline void cool(const S U[5], double dt, const Params& p, S out[5]) {
+inline void cool(const S U[5], double dt, const Params& p, const S* tab, S out[5]) {
   S rho = U[0];
   S Ek = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
   S Eth = U[4] - Ek;
   S Efloor = rho * p.t_floor / (p.gamma - 1.0);
-  if (p.cool_mode == 1) {                       // Eq. 22
-    S Edot_n = cool_rate(Eth, rho, p);
+  int mode = p.cool_mode;
+  if (mode == 2) {                              // masked choice per cell, reading A26
+    S Edot_n = cool_rate(Eth, rho, p, tab);
+    mode = (dt * std::fabs(val(Edot_n)) > p.f_sub * std::fabs(val(Eth))) ? 0 : 1;
+  }
+  if (mode == 1) {                              // Eq. 22
+    S Edot_n = cool_rate(Eth, rho, p, tab);
     S Epred = smax(Efloor, S(Eth + Edot_n * dt));
-    S Edot_p = cool_rate(Epred, rho, p);
+    S Edot_p = cool_rate(Epred, rho, p, tab);
     Eth = smax(Efloor, S(Eth + (0.5 * dt) * (Edot_n + Edot_p)));
   } else {                                      // Eq. 23
     const int nsub = p.cool_nsub > 1 ? p.cool_nsub : 1;
     const double ddt = dt / nsub;
-    for (int k = 0; k < nsub; ++k) Eth = smax(Efloor, S(Eth + cool_rate(Eth, rho, p) * ddt));
+    for (int k = 0; k < nsub; ++k) Eth = smax(Efloor, S(Eth + cool_rate(Eth, rho, p, tab) * ddt));
   }
   out[0] = U[0]; out[1] = U[1]; out[2] = U[2]; out[3] = U[3];
   out[4] = Ek + Eth;
@@ -320,11 +366,12 @@ void flux_divergence(const Grid& g, const Params& p, const S* U, S* D) {
 template <class S>
 void apply_cooling(const Grid& g, const Params& p, double dt, S* U) {
   const size_t N = g.N();
+  const std::vector<S> tab = table_as<S>(p);
 #pragma omp parallel for schedule(static)
   for (long long c = 0; c < (long long)N; ++c) {
     S u[5], o[5];
     for (int f = 0; f < 5; ++f) u[f] = U[f * N + c];
-    cool(u, dt, p, o);
+    cool(u, dt, p, tab.data(), o);
     U[4 * N + c] = o[4];
   }
 }
@@ -423,11 +470,12 @@ inline void stage_vjp_accumulate(const Grid& g, const Params& p, const double* U
 inline void cooling_vjp(const Grid& g, const Params& p, double dt, const double* U1, const double* gout,
                         double* gbar) {
   const size_t N = g.N();
+  const std::vector<Dual<5>> tab = table_as<Dual<5>>(p);
 #pragma omp parallel for schedule(static)
   for (long long c = 0; c < (long long)N; ++c) {
     Dual<5> u[5], o[5];
     for (int q = 0; q < 5; ++q) { u[q] = Dual<5>(U1[q * N + c]); u[q].d[q] = 1.0; }
-    cool(u, dt, p, o);
+    cool(u, dt, p, tab.data(), o);
     for (int q = 0; q < 5; ++q) {
       double acc = 0.0;
       for (int r = 0; r < 5; ++r) acc += o[r].d[q] * gout[r * N + c];
@@ -560,7 +608,7 @@ inline double t_cool_cell(const double U[5], const Params& p) {
   double rho = U[0];
   double Ek = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
   double Eth = U[4] - Ek;
-  double Edot = cool_rate<double>(Eth, rho, p);
+  double Edot = cool_rate<double>(Eth, rho, p, p.tab);
   if (Edot == 0.0) return std::numeric_limits<double>::infinity();
   return std::fabs(Eth) / std::fabs(Edot);
 }
@@ -702,8 +750,26 @@ inline void decision_margins(const Grid& g, const Params& p, const double* U, do
   }
 }
 
-// the compares of cool() at the pre-cooling state U1: T > 0 inside cool_rate() and every max with E_floor,
-// relative to E_kin + |E_th| (E_th is a difference of E and E_kin)
+// the compares of cool() at the pre-cooling state U1: T > 0 and (law 1) T < t_switch and the table interval inside every
+// cool_rate(), every max with E_floor, and (mode 2) the masked choice of the integrator; relative to E_kin + |E_th| (E_th is
+// a difference of E and E_kin)
+inline double rate_margin(double Eth, double rho, double s, const Params& p) {
+  double m = std::fabs(Eth) / s;                                               // T > 0
+  if (p.cool_law == 1) {
+    const double Esw = rho * p.t_switch / (p.gamma - 1.0);
+    m = std::fmin(m, std::fabs(Eth - Esw) / s);                                // T < t_switch
+    const double T = (p.gamma - 1.0) * Eth / rho;
+    if (T >= p.t_switch) {                                                     // kinks of the interpolant at the nodes
+      const double u = (std::log10(T) - p.tab_logT0) / p.tab_dlogT;
+      if (u > 0.0 && u < (double)(p.ntab - 1)) {
+        const double fr = u - std::floor(u);
+        m = std::fmin(m, 2.302585092994045684 * p.tab_dlogT * std::fmin(fr, 1.0 - fr) * std::fabs(Eth) / s);
+      }
+    }
+  }
+  return m;
+}
+
 inline void cooling_margins(const Grid& g, const Params& p, double dt, const double* U1, double* M) {
   const size_t N = g.N();
 #pragma omp parallel for schedule(static)
@@ -713,25 +779,54 @@ inline void cooling_margins(const Grid& g, const Params& p, double dt, const dou
     double Eth = U1[4 * N + c] - Ek;
     const double s = Ek + std::fabs(Eth);
     const double Efloor = rho * p.t_floor / (p.gamma - 1.0);
-    double m = std::fabs(Eth) / s;
-    if (p.cool_mode == 1) {
-      const double En = cool_rate<double>(Eth, rho, p);
+    double m = rate_margin(Eth, rho, s, p);
+    int mode = p.cool_mode;
+    if (mode == 2) {
+      const double En = cool_rate<double>(Eth, rho, p, p.tab);
+      m = std::fmin(m, std::fabs(dt * std::fabs(En) - p.f_sub * std::fabs(Eth)) / (p.f_sub * s));
+      mode = (dt * std::fabs(En) > p.f_sub * std::fabs(Eth)) ? 0 : 1;
+    }
+    if (mode == 1) {
+      const double En = cool_rate<double>(Eth, rho, p, p.tab);
       const double raw = Eth + En * dt;
       m = std::fmin(m, std::fabs(raw - Efloor) / s);
       const double Epred = std::fmax(Efloor, raw);
-      const double raw2 = Eth + (0.5 * dt) * (En + cool_rate<double>(Epred, rho, p));
+      m = std::fmin(m, rate_margin(Epred, rho, s, p));
+      const double raw2 = Eth + (0.5 * dt) * (En + cool_rate<double>(Epred, rho, p, p.tab));
       m = std::fmin(m, std::fabs(raw2 - Efloor) / s);
     } else {
       const int nsub = p.cool_nsub > 1 ? p.cool_nsub : 1;
       const double ddt = dt / nsub;
       for (int k = 0; k < nsub; ++k) {
-        const double raw = Eth + cool_rate<double>(Eth, rho, p) * ddt;
+        if (k > 0) m = std::fmin(m, rate_margin(Eth, rho, s, p));
+        const double raw = Eth + cool_rate<double>(Eth, rho, p, p.tab) * ddt;
         m = std::fmin(m, std::fabs(raw - Efloor) / s);
         Eth = std::fmax(Efloor, raw);
       }
     }
     M[c] = m;
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Gradient with respect to the cooling table itself ("... and even the cooling tables themselves"):
+//   gtab[k] = sum_cells gout_E(cell) * d E_out(cell) / d tab[k]     at the pre-cooling state U1,
+// by dual numbers with one derivative slot per table node through the same cool() (ntab <= 32).
+// ------------------------------------------------------------------------------------------------
+inline int cooling_table_vjp(const Grid& g, const Params& p, double dt, const double* U1, const double* gout, double* gtab) {
+  constexpr int NT = 32;
+  if (p.cool_law != 1 || !p.tab || p.ntab > NT) return -1;
+  const size_t N = g.N();
+  std::vector<Dual<NT>> tab((size_t)p.ntab);
+  for (int k = 0; k < p.ntab; ++k) { tab[k] = Dual<NT>(p.tab[k]); tab[k].d[k] = 1.0; }
+  for (int k = 0; k < p.ntab; ++k) gtab[k] = 0.0;
+  for (size_t c = 0; c < N; ++c) {                 // plain serial sum: a fixed order
+    Dual<NT> u[5], o[5];
+    for (int q = 0; q < 5; ++q) u[q] = Dual<NT>(U1[q * N + c]);
+    cool(u, dt, p, tab.data(), o);
+    for (int k = 0; k < p.ntab; ++k) gtab[k] += o[4].d[k] * gout[4 * N + c];
+  }
+  return 0;
 }
 
 }  // namespace dho

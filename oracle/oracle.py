@@ -27,7 +27,8 @@ _lib = None
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2, "constant": 3}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}
-COOL_MODES = {"euler": 0, "trapezoid": 1}
+COOL_MODES = {"euler": 0, "trapezoid": 1, "masked": 2}
+COOL_LAWS = {"powerlaw": 0, "twobranch": 1}
 
 
 class _Params(ctypes.Structure):
@@ -45,6 +46,18 @@ class _Params(ctypes.Structure):
         ("t_floor", ctypes.c_double),
         ("cool_mode", ctypes.c_int),
         ("cool_nsub", ctypes.c_int),
+        ("cool_law", ctypes.c_int),
+        ("t_switch", ctypes.c_double),
+        ("lambda1", ctypes.c_double),
+        ("alpha1", ctypes.c_double),
+        ("lambda2", ctypes.c_double),
+        ("alpha2", ctypes.c_double),
+        ("gamma0", ctypes.c_double),
+        ("tab", ctypes.POINTER(ctypes.c_double)),
+        ("ntab", ctypes.c_int),
+        ("tab_logT0", ctypes.c_double),
+        ("tab_dlogT", ctypes.c_double),
+        ("f_sub", ctypes.c_double),
     ]
 
 
@@ -85,7 +98,8 @@ def set_num_threads(n: int) -> None:
 
 def params(gamma=5.0 / 3.0, dx=None, shape=None, rho_floor=1e-10, p_floor=1e-10, limiter="minmod",
            riemann="hllc", integrator="vl2", cooling=False, lambda0=1e-3, alpha=0.5, t_floor=0.01,
-           cool_mode="euler", cool_nsub=1):
+           cool_mode="euler", cool_nsub=1, cool_law="powerlaw", t_switch=1.0, lambda1=0.0, alpha1=1.0, lambda2=0.0, alpha2=0.5,
+           gamma0=0.0, table=None, f_sub=0.1):
     """Scheme parameters.  ``dx`` defaults to the unit box, dx_a = 1/n_a (reading A13)."""
     p = _Params()
     p.gamma = float(gamma)
@@ -103,6 +117,20 @@ def params(gamma=5.0 / 3.0, dx=None, shape=None, rho_floor=1e-10, p_floor=1e-10,
     p.cool_mode, p.cool_nsub = COOL_MODES[cool_mode], int(cool_nsub)
     if p.cool_nsub < 1:
         raise ValueError("cool_nsub must be >= 1")
+    # Eqs. 17-19: Koyama-Inutsuka fit + uniform heating below t_switch, tabulated Lambda_CIE above it
+    # (reading A25); table = (log10_T0, dlog10_T, [log10 Lambda at the nodes]); cool_mode "masked": reading A26
+    p.cool_law = COOL_LAWS[cool_law]
+    p.t_switch, p.lambda1, p.alpha1, p.lambda2, p.alpha2, p.gamma0 = (float(v) for v in (t_switch, lambda1, alpha1, lambda2, alpha2, gamma0))
+    p.f_sub = float(f_sub)
+    p.ntab = 0
+    if table is not None:
+        logT0, dlogT, vals = table
+        arr = np.ascontiguousarray(vals, dtype=np.float64)
+        p._table_keepalive = arr                      # the struct only holds a pointer
+        p.tab = arr.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+        p.ntab, p.tab_logT0, p.tab_dlogT = int(arr.size), float(logT0), float(dlogT)
+    if p.cool_law == 1 and p.ntab < 2:
+        raise ValueError("cool_law='twobranch' needs a table with at least two nodes")
     return p
 
 
@@ -250,6 +278,40 @@ def cooling_margins(U1, dt, p):
     M = np.empty(U1.shape[1:], dtype=np.float64)
     lib.dho_cooling_margins(*_dims(U1), ctypes.byref(p), ctypes.c_double(dt), _ptr(U1), _ptr(M))
     return M
+
+
+def cool_rate(Eth, rho, p):
+    """Edot = n_H Gamma - n_H^2 Lambda of the law selected in p at thermal energy Eth and density rho."""
+    lib = _load()
+    lib.dho_cool_rate.restype = ctypes.c_double
+    return float(lib.dho_cool_rate(ctypes.byref(p), ctypes.c_double(Eth), ctypes.c_double(rho)))
+
+
+def lambda_table(T, p):
+    """Lambda_CIE(T) of Eq. 19: log-log interpolation of p's table."""
+    lib = _load()
+    lib.dho_lambda_table.restype = ctypes.c_double
+    return float(lib.dho_lambda_table(ctypes.byref(p), ctypes.c_double(T)))
+
+
+def step_nocool(U, dt, p):
+    """The pre-cooling state of a step: the hydro stages of step() without the cooling update."""
+    lib = _load()
+    U = _f64(U)
+    out = np.empty_like(U)
+    lib.dho_step_nocool(*_dims(U), ctypes.byref(p), _ptr(U), ctypes.c_double(dt), _ptr(out))
+    return out
+
+
+def cooling_table_vjp(U1, dt, g_out, p):
+    """d sum(g_out_E * E_out) / d table nodes at the pre-cooling state U1, by dual numbers (ntab <= 32)."""
+    lib = _load()
+    U1, g_out = _f64(U1), _f64(g_out)
+    gt = np.zeros(p.ntab, dtype=np.float64)
+    rc = lib.dho_cooling_table_vjp(*_dims(U1), ctypes.byref(p), ctypes.c_double(dt), _ptr(U1), _ptr(g_out), _ptr(gt))
+    if rc != 0:
+        raise ValueError("cooling_table_vjp needs cool_law='twobranch' and a table of at most 32 nodes")
+    return gt
 
 
 def window_step(U_full, dt, p, lo, size, halo=4):

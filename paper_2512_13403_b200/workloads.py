@@ -203,6 +203,26 @@ def cotangent(shape, seed: int = 2005, dtype=torch.float32, device="cpu") -> tor
     return torch.randn((5,) + tuple(shape[-3:]), generator=_gen(seed, device), device=device, dtype=dtype)
 
 
+def cooling_table(seed: int = 1719, n: int = 24, log10_t_lo: float = 0.0, log10_t_hi: float = 2.0,
+                  lambda_lo: float = 3.0e-2):
+    """Synthetic stand-in for the tabulated collisional-ionisation-equilibrium cooling curve of Eq. 19 (the
+    paper's SD93 table is not available): n nodes equally spaced in log10 T on [log10_t_lo, log10_t_hi]; log10 Lambda = a linear
+    trend plus three seeded Gaussian bumps in log T (the shape of a line-cooling curve: peaks and valleys of about a decade),
+    shifted so that the first node equals log10(lambda_lo) (the caller matches it to the low-temperature branch at the switch
+    temperature, as the two branches of Eq. 17 meet in the KO15 prescription).  Returns (log10_t_lo, dlog10_T, values[n]) as
+    Python floats / a float64 tensor: an INPUT of the cooling law, no arithmetic of the scheme."""
+    g = torch.Generator(device="cpu")
+    g.manual_seed(int(seed))
+    r = torch.rand(10, generator=g, dtype=torch.float64)
+    x = torch.linspace(0.0, 1.0, n, dtype=torch.float64)
+    y = (r[0] - 0.5) * x
+    for j in range(3):
+        amp, cen, wid = -0.8 + 1.8 * r[1 + 3 * j], 0.1 + 0.8 * r[2 + 3 * j], 0.08 + 0.17 * r[3 + 3 * j]
+        y = y + amp * (torch.exp(-((x - cen) / wid) ** 2) - torch.exp(-((0.0 - cen) / wid) ** 2))
+    vals = math.log10(lambda_lo) + y
+    return float(log10_t_lo), float((log10_t_hi - log10_t_lo) / (n - 1)), vals
+
+
 def make_config(cfg: int, n: int | None = None, device="cpu", dtype=None) -> Workload:
     """BASELINE.json `configs[cfg]` (0-based), optionally at a reduced size `n` for tests."""
     if cfg == 0:

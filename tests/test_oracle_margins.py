@@ -37,6 +37,7 @@ LINE_CASES = [
     dict(integrator="heun"), dict(integrator="ssprk3"),
     dict(cooling=True, lambda0=40.0, t_floor=0.6), dict(cooling=True, lambda0=40.0, t_floor=0.6, cool_nsub=3),
     dict(cooling=True, lambda0=40.0, t_floor=0.6, cool_mode="trapezoid"),
+    dict(twobranch=True), dict(twobranch=True, cool_mode="masked", cool_nsub=3, f_sub=0.3),
 ]
 
 
@@ -45,6 +46,11 @@ def test_every_jump_of_the_vjp_along_a_line_is_flagged_and_only_its_neighbourhoo
     kw = dict(kw)
     mach = kw.pop("mach", 0.5)
     shape = (6, 7, 8)
+    if kw.pop("twobranch", False):                       # Eqs. 17-19: switch temperature and table nodes inside the gas' range
+        from paper_2512_13403_b200 import workloads
+        logT0, dlogT, vals = workloads.cooling_table(log10_t_lo=-0.13, log10_t_hi=0.6, n=5)   # t_switch inside the first interval
+        kw.update(cooling=True, cool_law="twobranch", t_switch=1.0, lambda1=8.0, alpha1=2.0, lambda2=4.0, alpha2=0.5, gamma0=3.0,
+                  table=(logT0, dlogT, vals.numpy() + 2.3), t_floor=0.3)
     p = oracle.params(shape=shape, **kw)
     found = 0
     for seed in range(6):
@@ -150,6 +156,26 @@ def test_cooling_margin_is_the_distance_to_the_floor():
     expect = np.abs(free - 0.3) / T                       # |E_th' - E_floor| / E_th
     assert np.allclose(M, np.minimum(expect, 1.0), rtol=1e-12)
     assert ((Tn == 0.3) == (free < 0.3)).all() or np.allclose(Tn[free < 0.3], 0.3)
+
+
+def test_masked_integrator_choice_has_the_distance_to_its_criterion_as_margin():
+    """A cell whose dt |Edot| equals f_sub |E_th| (found by bisection on the oracle's own rate) has margin ~ 0; moved
+    away from it by a relative d the margin is ~ d."""
+    g = 5 / 3
+    p = oracle.params(shape=(1, 1, 1), dx=(1, 1, 1), gamma=g, cooling=True, lambda0=2.0, alpha=0.5, t_floor=1e-3,
+                      cool_mode="masked", cool_nsub=4, f_sub=0.2)
+    rho, dt = 1.4, 0.3
+    crit = lambda E: dt * abs(oracle.cool_rate(E, rho, p)) - 0.2 * E
+    lo, hi = 1e-3, 1e3                                    # rate ~ sqrt(E): rapid (crit > 0) at small E, slow at large E
+    assert crit(lo) > 0 > crit(hi)
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        lo, hi = (mid, hi) if crit(mid) > 0 else (lo, mid)
+    E0 = 0.5 * (lo + hi)
+    for d in (0.0, 1e-6, 1e-3):
+        U = np.array([rho, 0.0, 0.0, 0.0, E0 * (1 + d)]).reshape(5, 1, 1, 1)
+        m = float(oracle.cooling_margins(U, dt, p)[0, 0, 0])
+        assert (m <= 1e-12) if d == 0.0 else (0.2 * d <= m <= 5 * d), (d, m)
 
 
 @pytest.mark.parametrize("case", ["random", "turbulence"])
