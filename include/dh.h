@@ -84,8 +84,9 @@ enum {
                             dh_step_vjp / dh_adjoint with 1 or 2: the one-thread-per-cell gather kernels */
   DH_OPT_COOL_MODE = 16, /* integrator of the cooling source: 0 (default) the Euler update with floor of Eq. 23,
                             sub-cycled DH_OPT_COOL_NSUB times; 1 the trapezoid of Eq. 22 with T^pred from the Euler-predicted,
-                            floored energy (reading A20).  (0, N_sub = 1) runs in the last stage's epilogue; the others
-                            as one streaming pass over the finished state (DH_K_COOL) */
+                            floored energy (reading A20); 2 either of them per cell (DH_OPT_COOL_FSUB).  (0, N_sub = 1) with
+                            the power law runs in the last stage's epilogue; the others as one streaming pass over the
+                            finished state (DH_K_COOL) */
   DH_OPT_COOL_NSUB = 17, /* N_sub of Eq. 23: integer in 1 .. 64, default 1; substeps dt / N_sub, rate and floor every substep */
   DH_OPT_C_COOL = 18,    /* c_cool of Eq. 21, finite >= 0, default 0 = no cooling-time limit.  With DH_OPT_COOLING = 1 and
                             c_cool > 0 every CFL pass (dh_cfl_dt, dh_cfl_dt_async, dh_advance, dh_adjoint, dh_run_host) also reduces
@@ -95,6 +96,20 @@ enum {
                             rate do not count; the candidates are compared in the dtype (reading A24).  dt is
                             bit-identical to Eq. A8 whenever the hydro candidate is the smallest */
   DH_OPT_DT_MAX = 19,    /* Delta t_max of Eq. 21, finite >= 0, default 0 = none; applies with or without cooling */
+  DH_OPT_COOL_LAW = 20,  /* 0 (default): Lambda = Lambda0 T^alpha, Gamma = 0; 1: the two-branch law of Eqs. 17-19:
+                            T < t_switch: Lambda = lambda1 T^alpha1 + lambda2 T^alpha2 (Eq. 18) and uniform heating n_H Gamma0;
+                            T >= t_switch: Lambda_CIE(T) by linear interpolation in log T - log Lambda of the table given to
+                            dh_set_cooling_table (Eq. 19; end values held outside), no heating.  Code units n_H = rho, T = P / rho.
+                            Needs a table first.  The update runs as the streaming pass DH_K_COOL; Eq. 20's t_cool follows the law */
+  DH_OPT_T_SWITCH = 21,  /* the 10^4 K of Eq. 17 in code units, > 0, default 1 */
+  DH_OPT_LAMBDA1 = 22,   /* Eq. 18, >= 0, default 0 */
+  DH_OPT_ALPHA1 = 23,    /* default 1 */
+  DH_OPT_LAMBDA2 = 24,   /* >= 0, default 0 */
+  DH_OPT_ALPHA2 = 25,    /* default 0.5 */
+  DH_OPT_GAMMA0 = 26,    /* Gamma_0 of PAPER.md:286, 294, >= 0, default 0 */
+  DH_OPT_COOL_FSUB = 27, /* DH_OPT_COOL_MODE = 2 (the masked per-cell choice of PAPER.md:342): a cell takes the sub-cycled update
+                            of Eq. 23 (DH_OPT_COOL_NSUB substeps) when dt |Edot(T^n)| > f_sub |E_th^n|, else the trapezoid of
+                            Eq. 22 (reading A26); > 0, default 0.1 */
   DH_OPT_COUNT_
 };
 
@@ -110,6 +125,17 @@ int dh_set_stream(dh_ctx* ctx, void* cuda_stream);
 
 int dh_set_option(dh_ctx* ctx, int key, double value);
 int dh_get_option(const dh_ctx* ctx, int key, double* value_out);
+
+/* The table of Eq. 19 for DH_OPT_COOL_LAW = 1: log10_lambda[n] (HOST, copied) = log10 Lambda_CIE at the
+ * nodes log10 T = log10_t0 + k dlog10_t, k = 0 .. n-1, 2 <= n <= 256, dlog10_t > 0.  Synchronises the context's stream.
+ * DH_ERR_ARG on a non-finite value or a bad size. */
+int dh_set_cooling_table(dh_ctx* ctx, const double* log10_lambda, int n, double log10_t0, double dlog10_t);
+
+/* Gradient with respect to the cooling table itself: for the step U^n -> U^{n+1} of dh_step at this dt and
+ * the cotangent gU_out = dL/dU^{n+1} (DEVICE, like dh_step_vjp), gtab_out[n] (HOST) = dL / d log10_lambda[k].  The
+ * pre-cooling state is recomputed; per-block partial sums are added in a fixed order.  Synchronises the stream.
+ * Needs DH_OPT_COOLING = 1 and DH_OPT_COOL_LAW = 1. */
+int dh_cool_table_vjp(dh_ctx* ctx, const void* U, double dt, const void* gU_out, double* gtab_out);
 
 /* CFL time step, Eq. A8: one block-reduced max-wavespeed kernel over the 5 fields, then
  * dt = C * min_a(dx_a / S_a) formed on the device in T with IEEE-rounded, non-contracted operations, so

@@ -54,6 +54,16 @@ static Consts<T> make_consts(const dh_ctx* c) {
   k.alpha_is_half = (c->alpha == 0.5);
   k.cool_mode = c->cool_mode;
   k.cool_nsub = c->cool_nsub;
+  k.cool_law = (c->cool_law != 0 && c->ntab >= 2) ? 1 : 0;
+  k.t_switch = (T)c->t_switch;
+  k.lambda1 = (T)c->lambda1; k.alpha1 = (T)c->alpha1; k.lambda2 = (T)c->lambda2; k.alpha2 = (T)c->alpha2;
+  k.gamma0 = (T)c->gamma0;
+  k.f_sub = (T)c->f_sub;
+  k.tab = sizeof(T) == 8 ? (const T*)c->tab_dev_d : (const T*)c->tab_dev;
+  k.ntab = c->ntab;
+  const double l2_10 = 3.321928094887362;                      // the table is held in log2 units (dh_set_cooling_table)
+  k.tab_l2t0 = (T)(c->tab_log10t0 * l2_10);
+  k.tab_inv_dl2t = (T)(c->ntab >= 2 ? 1.0 / (c->tab_dlog10t * l2_10) : 0.0);
   return k;
 }
 
@@ -134,6 +144,8 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
   c->L[0] = c->L[1] = c->L[2] = 1.0;
   c->cooling = 0; c->kernel = 0; c->limiter = 0; c->riemann = 0; c->integrator = 0; c->cool_mode = 0; c->cool_nsub = 1; c->fuse_cfl = 1; c->c_cool = 0.0; c->dt_max = 0.0;
   c->lambda0 = 1e-3; c->alpha = 0.5; c->t_floor = 0.01;
+  c->cool_law = 0; c->t_switch = 1.0; c->lambda1 = 0.0; c->alpha1 = 1.0; c->lambda2 = 0.0; c->alpha2 = 0.5; c->gamma0 = 0.0; c->f_sub = 0.1;
+  c->ntab = 0; c->tab_log10t0 = 0.0; c->tab_dlog10t = 1.0;
   c->rho_floor = 1e-10; c->p_floor = 1e-10;
   c->stream = 0;
   c->device = dev;
@@ -163,7 +175,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev};
+  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev, c->tab_dev, c->tab_dev_d, c->tab_part};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
@@ -201,7 +213,18 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_C_COOL: if (!(v >= 0.0) || !isfinite(v)) return fail(DH_ERR_ARG, "dh_set_option: c_cool must be finite and >= 0%s"); c->c_cool = v; break;
     case DH_OPT_DT_MAX: if (!(v >= 0.0) || !isfinite(v)) return fail(DH_ERR_ARG, "dh_set_option: dt_max must be finite and >= 0%s"); c->dt_max = v; break;
     case DH_OPT_RIEMANN: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: riemann must be 0, 1 or 2%s"); c->riemann = (int)v; break;
-    case DH_OPT_COOL_MODE: if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: cool_mode must be 0 or 1%s"); c->cool_mode = (int)v; break;
+    case DH_OPT_COOL_MODE: if (v != 0.0 && v != 1.0 && v != 2.0) return fail(DH_ERR_ARG, "dh_set_option: cool_mode must be 0, 1 or 2%s"); c->cool_mode = (int)v; break;
+    case DH_OPT_COOL_LAW:
+      if (v != 0.0 && v != 1.0) return fail(DH_ERR_ARG, "dh_set_option: cool_law must be 0 or 1%s");
+      if (v == 1.0 && c->ntab < 2) return fail(DH_ERR_ARG, "dh_set_option: cool_law = 1 needs a table (dh_set_cooling_table first)%s");
+      c->cool_law = (int)v; break;
+    case DH_OPT_T_SWITCH: if (!(v > 0)) return fail(DH_ERR_ARG, "dh_set_option: t_switch must be > 0%s"); c->t_switch = v; break;
+    case DH_OPT_LAMBDA1: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: lambda1 must be >= 0%s"); c->lambda1 = v; break;
+    case DH_OPT_ALPHA1: c->alpha1 = v; break;
+    case DH_OPT_LAMBDA2: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: lambda2 must be >= 0%s"); c->lambda2 = v; break;
+    case DH_OPT_ALPHA2: c->alpha2 = v; break;
+    case DH_OPT_GAMMA0: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: gamma0 must be >= 0%s"); c->gamma0 = v; break;
+    case DH_OPT_COOL_FSUB: if (!(v > 0)) return fail(DH_ERR_ARG, "dh_set_option: cool_fsub must be > 0%s"); c->f_sub = v; break;
     case DH_OPT_COOL_NSUB:
       if (v < 1 || v > DH_COOL_NSUB_MAX || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: cool_nsub must be an integer in 1 .. 64%s");
       c->cool_nsub = (int)v; break;
@@ -230,6 +253,14 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_DT_MAX: *out = c->dt_max; break;
     case DH_OPT_RIEMANN: *out = c->riemann; break;
     case DH_OPT_COOL_MODE: *out = c->cool_mode; break;
+    case DH_OPT_COOL_LAW: *out = c->cool_law; break;
+    case DH_OPT_T_SWITCH: *out = c->t_switch; break;
+    case DH_OPT_LAMBDA1: *out = c->lambda1; break;
+    case DH_OPT_ALPHA1: *out = c->alpha1; break;
+    case DH_OPT_LAMBDA2: *out = c->lambda2; break;
+    case DH_OPT_ALPHA2: *out = c->alpha2; break;
+    case DH_OPT_GAMMA0: *out = c->gamma0; break;
+    case DH_OPT_COOL_FSUB: *out = c->f_sub; break;
     case DH_OPT_COOL_NSUB: *out = c->cool_nsub; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
@@ -274,6 +305,7 @@ static int cfl_launch(dh_ctx* c, const void* U, bool cand = false, bool force_tc
   // Eq. 21: the reduction also evaluates Eq. 20 when cooling is on and c_cool > 0 (or for dh_cool_tmin)
   p.cool_lim = (force_tcool || (c->cooling != 0 && c->c_cool > 0.0)) ? 1 : 0;
   p.gm1d = c->gamma - 1.0; p.lambda0 = c->lambda0; p.alpha = c->alpha; p.c_cool = c->cooling != 0 ? c->c_cool : 0.0; p.dt_max = c->dt_max;
+  p.cd = make_consts<double>(c);                    // Eq. 20 with the law of DH_OPT_COOL_LAW, in double
   if (p.cool_lim) cand = false;
   p.U = (const T*)U;
   p.N = c->N;
@@ -389,7 +421,7 @@ template <class T>
 static int step_impl(dh_ctx* c, void* U, double dt, bool devdt, bool cand = false) {
   // default cooling update (Eq. 23, N_sub = 1): epilogue of the last stage; the others: a pass of their own, and the
   // CFL candidates (pushed by the last stage from the pre-cooling values) are not used
-  const bool split_cool = c->cooling != 0 && (c->cool_mode != 0 || c->cool_nsub > 1);
+  const bool split_cool = c->cooling != 0 && (c->cool_mode != 0 || c->cool_nsub > 1 || c->cool_law != 0);
   const bool fused_cool = c->cooling != 0 && !split_cool;
   if (c->integrator != 0) {
     // Heun / SSPRK3 in Shu-Osher form: every stage is  out = B - w dt D(state)
@@ -660,6 +692,71 @@ int dh_cool_tmin(dh_ctx* c, const void* U, double* tcool_min_out, double* dt_hyd
   *tcool_min_out = c->result_host->tcool_min;
   if (dt_hydro_out) *dt_hydro_out = c->result_host->dt_hydro;
   return DH_OK;
+}
+
+int dh_set_cooling_table(dh_ctx* c, const double* log10_lambda, int n, double log10_t0, double dlog10_t) {
+  if (!c || !log10_lambda) return fail(DH_ERR_ARG, "dh_set_cooling_table: NULL argument%s");
+  if (int drc = check_device(c, "dh_set_cooling_table")) return drc;
+  if (n < 2 || n > 256) return fail(DH_ERR_ARG, "dh_set_cooling_table: the table needs 2 .. 256 nodes%s");
+  if (!(dlog10_t > 0.0) || !isfinite(dlog10_t) || !isfinite(log10_t0)) return fail(DH_ERR_ARG, "dh_set_cooling_table: node spacing must be finite and > 0%s");
+  double h64[256];
+  float h32[256];
+  const double l2_10 = 3.321928094887362;           // held as log2 Lambda: one lg2 / ex2 pair evaluates the interpolant
+  for (int k = 0; k < n; ++k) {
+    if (!isfinite(log10_lambda[k])) return fail(DH_ERR_ARG, "dh_set_cooling_table: non-finite table value%s");
+    h64[k] = log10_lambda[k] * l2_10;
+    h32[k] = (float)h64[k];
+  }
+  int rc = lazy_alloc(c, &c->tab_dev, 256 * sizeof(double), "the cooling table");
+  if (rc) return rc;
+  rc = lazy_alloc(c, (void**)&c->tab_dev_d, 256 * sizeof(double), "the cooling table (double)");
+  if (rc) return rc;
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_set_cooling_table: synchronize");      // kernels in flight may read the old table
+  DH_CUDA(cudaMemcpy(c->tab_dev_d, h64, n * sizeof(double), cudaMemcpyHostToDevice), "dh_set_cooling_table: upload");
+  if (c->dtype == DH_F32) DH_CUDA(cudaMemcpy(c->tab_dev, h32, n * sizeof(float), cudaMemcpyHostToDevice), "dh_set_cooling_table: upload");
+  else DH_CUDA(cudaMemcpy(c->tab_dev, h64, n * sizeof(double), cudaMemcpyHostToDevice), "dh_set_cooling_table: upload");
+  c->ntab = n; c->tab_log10t0 = log10_t0; c->tab_dlog10t = dlog10_t;
+  return DH_OK;
+}
+
+}  // extern "C"
+
+template <class T>
+static int table_vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout, double* gtab_host) {
+  int rc = lazy_alloc(c, &c->U1, state_bytes(c), "the pre-cooling state");
+  if (rc) return rc;
+  rc = lazy_alloc(c, (void**)&c->tab_part, ((size_t)cool_table_blocks() + 1) * 256 * sizeof(double), "the table-gradient partial sums");
+  if (rc) return rc;
+  // the pre-cooling state of the step (nothing was stored by dh_step)
+  if (c->integrator == 0) {
+    rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, false, 0.5, false);
+    if (rc) return rc;
+    rc = stage_launch<T>(c, DH_K_STAGE2, c->Us, U, c->U1, dt, false, 1.0, false);
+  } else {
+    const void* last_in = nullptr;
+    double w = 0.0;
+    rc = rk_prefix<T>(c, U, dt, false, &last_in, &w);
+    if (rc) return rc;
+    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, c->U1, dt, false, w, false);
+  }
+  if (rc) return rc;
+  double* const res = c->tab_part + (size_t)cool_table_blocks() * 256;
+  DH_CUDA(launch_cool_table_vjp<T>((const T*)c->U1, (const T*)gout, c->N, (T)dt, make_consts<T>(c), c->tab_part, res, c->stream),
+          "dh_cool_table_vjp: kernel launch");
+  c->launches += 2;
+  DH_CUDA(cudaMemcpyAsync(gtab_host, res, c->ntab * sizeof(double), cudaMemcpyDeviceToHost, c->stream), "dh_cool_table_vjp: copy");
+  DH_CUDA(cudaStreamSynchronize(c->stream), "dh_cool_table_vjp: synchronize");
+  return DH_OK;
+}
+
+extern "C" {
+
+int dh_cool_table_vjp(dh_ctx* c, const void* U, double dt, const void* gU_out, double* gtab_out) {
+  if (!c || !U || !gU_out || !gtab_out) return fail(DH_ERR_ARG, "dh_cool_table_vjp: NULL argument%s");
+  if (int drc = check_device(c, "dh_cool_table_vjp")) return drc;
+  if (!(dt > 0.0) || !isfinite(dt)) return fail(DH_ERR_ARG, "dh_cool_table_vjp: dt must be finite and > 0%s");
+  if (!c->cooling || c->cool_law != 1 || c->ntab < 2) return fail(DH_ERR_ARG, "dh_cool_table_vjp: needs DH_OPT_COOLING = 1 and DH_OPT_COOL_LAW = 1%s");
+  return c->dtype == DH_F32 ? table_vjp_impl<float>(c, U, dt, gU_out, gtab_out) : table_vjp_impl<double>(c, U, dt, gU_out, gtab_out);
 }
 
 int dh_cfl_stats(dh_ctx* c, unsigned long long* out) {

@@ -74,6 +74,17 @@ __device__ __noinline__ double cell_tcool(double rho, double mx, double my, doub
   return (rate != 0.0 && t < tmin) ? t : tmin;
 }
 
+// t_cool of Eq. 20 for the two-branch law of Eqs. 17-19 (DH_OPT_COOL_LAW = 1): |E_th| / |n_H Gamma - n_H^2 Lambda| with the rate
+// of cool_rate() in double (no fp32 screen: with heating the rate has no closed log form, every cell is evaluated)
+__device__ __noinline__ double cell_tcool_law(double rho, double mx, double my, double mz, double E, const Consts<double>& cd, double tmin) {
+  const double q = Ieee::add(Ieee::add(Ieee::mul(mx, mx), Ieee::mul(my, my)), Ieee::mul(mz, mz));
+  const double Ek = Ieee::div(Ieee::mul(0.5, q), rho);
+  const double Eth = Ieee::sub(E, Ek);
+  const double rate = cool_rate<double>(Eth, rho, 1.0 / rho, cd);
+  const double t = Ieee::div(fabs(Eth), fabs(rate));
+  return (rate != 0.0 && t < tmin) ? t : tmin;
+}
+
 // fp32 screen in front of cell_tcool (whose fp64 power function would make the pass ALU bound: 1.92 ms instead of the 0.41 ms
 // the 20 B/cell take at 512^3).  Any exact t_cool already evaluated is an upper bound of the global minimum, so a cell whose
 // exact value provably exceeds the warp's running minimum need not be evaluated.  The screen works in log2 on the E_kin / E_th
@@ -134,6 +145,7 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
     const unsigned full = 0xffffffffu;
     const int lane = threadIdx.x & 31;
     const size_t w0 = tid - lane;
+    const bool law1 = p.cd.cool_law != 0;
     const float c_eth = (float)(1.0 - p.alpha), c_rho = (float)(p.alpha - 2.0);
     // log2 of the safety factor, and the constant terms of log2 t_cool moved to the threshold's side
     const double lconst = log2(1.0 + 1e-3 * (1.0 + fabs(1.0 - p.alpha))) + log2(p.lambda0) + p.alpha * log2(p.gm1d);
@@ -172,7 +184,7 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
           float ek, eth, S;
           bool range_ok;
           need_s = need_s || speeds_may_decide<T>(ca[l], cb[l], cc[l], cd[l], ce[l], p.rho_floor, gm1f, gammaf, pflf, bx, by, bz, ek, eth, S, range_ok);
-          need = need || tcool_may_decide<T>(ca[l], eth, S, range_ok, c_eth, c_rho, lthr);
+          need = need || law1 || tcool_may_decide<T>(ca[l], eth, S, range_ok, c_eth, c_rho, lthr);
         }
       if (__any_sync(full, need_s)) {      // the exact recipe for the lanes that asked, then the warp shares its maxima
         if (need_s) {
@@ -193,7 +205,8 @@ __global__ void __launch_bounds__(256, COOL ? 4 : 1) cfl_reduce_kernel(const Cfl
         if (need) {
 #pragma unroll
           for (int l = 0; l < W; ++l)
-            if (l < n) tmin = cell_tcool((double)ca[l], (double)cb[l], (double)cc[l], (double)cd[l], (double)ce[l], p.gm1d, p.lambda0, p.alpha, tmin);
+            if (l < n) tmin = law1 ? cell_tcool_law((double)ca[l], (double)cb[l], (double)cc[l], (double)cd[l], (double)ce[l], p.cd, tmin)
+                               : cell_tcool((double)ca[l], (double)cb[l], (double)cc[l], (double)cd[l], (double)ce[l], p.gm1d, p.lambda0, p.alpha, tmin);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {

@@ -102,6 +102,7 @@ struct CflParams {
   // Eq. 21: cool_lim != 0 makes the reduction evaluate Eq. 20 per cell (in double, reading A24)
   int cool_lim;
   double gm1d, lambda0, alpha, c_cool, dt_max;
+  Consts<double> cd;         // the cooling law in double (DH_OPT_COOL_LAW = 1: its table pointer is the double copy)
   T* dt_dev;                 // dt in T for the stage kernels
   CflResult* result;         // device copy of the result block
   // candidate path (all nullptr = plain reduction): see StageParams
@@ -117,7 +118,14 @@ struct Ctx {
   size_t N;
   double gamma, cfl, L[3];
   int cooling, kernel, limiter, riemann, integrator;
-  int cool_mode, cool_nsub;    // DH_OPT_COOL_MODE (0 Euler sub-cycled, 1 trapezoid), DH_OPT_COOL_NSUB
+  int cool_mode, cool_nsub;    // DH_OPT_COOL_MODE (0 Euler sub-cycled, 1 trapezoid, 2 masked per cell), DH_OPT_COOL_NSUB
+  int cool_law;                // DH_OPT_COOL_LAW (0 power law, 1 the two-branch law of Eqs. 17-19)
+  double t_switch, lambda1, alpha1, lambda2, alpha2, gamma0, f_sub;
+  void* tab_dev;               // the table in the array dtype (log2 Lambda at nodes equally spaced in log2 T), 256 slots
+  double* tab_dev_d;           // the same in double (cooling-time limit, table gradient)
+  double* tab_part;            // per-block partial sums of the table gradient
+  int ntab;
+  double tab_log10t0, tab_dlog10t;
   double c_cool, dt_max;       // DH_OPT_C_COOL, DH_OPT_DT_MAX (Eq. 21; 0 = candidate off)
   double lambda0, alpha, t_floor, rho_floor, p_floor;
   cudaStream_t stream;
@@ -175,6 +183,8 @@ template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int s
 template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
 template <class T> cudaError_t launch_cool_fwd(T* U, size_t N, T dt, const T* dt_dev, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
+template <class T> cudaError_t launch_cool_table_vjp(const T* U1, const T* g, size_t N, T dt, const Consts<T>& c, double* part, double* gtab, cudaStream_t s);
+int cool_table_blocks();
 template <class T> cudaError_t launch_lincomb(T* out, T a, const T* X, T b, const T* Y, size_t n, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_candidates(const CflParams<T>& p, int sm_count, cudaStream_t s);   // candidates, then the guarded full pass

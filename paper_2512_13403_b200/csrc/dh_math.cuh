@@ -39,7 +39,23 @@ struct Consts {
   T lambda0, alpha, t_floor;
   int alpha_is_half;
   int cool_mode, cool_nsub;   // DH_OPT_COOL_MODE / DH_OPT_COOL_NSUB; (0, 1) is the update fused into the stage kernels
+  // two-branch law of Eqs. 17-19 (DH_OPT_COOL_LAW = 1): Koyama-Inutsuka fit + uniform heating below
+  // t_switch, tabulated Lambda_CIE above it.  The table holds log2 Lambda at nodes equally spaced in log2 T (the same
+  // interpolant as in log10-log10: a change of base is linear), so that one lg2 / ex2 pair evaluates it.
+  int cool_law;
+  T t_switch, lambda1, alpha1, lambda2, alpha2, gamma0;
+  T f_sub;                    // DH_OPT_COOL_FSUB: cool_mode 2 sub-cycles a cell when dt |Edot| > f_sub |E_th| (reading A26)
+  const T* tab;               // DEVICE, ntab values of log2 Lambda
+  int ntab;
+  T tab_l2t0, tab_inv_dl2t;   // first node and 1 / spacing, in log2 T
 };
+
+__device__ __forceinline__ float log2_(float x) { return __log2f(x); }
+__device__ __forceinline__ double log2_(double x) { return log2(x); }
+__device__ __forceinline__ float exp2_(float x) { return exp2f(x); }
+__device__ __forceinline__ double exp2_(double x) { return exp2(x); }
+__device__ __forceinline__ float floor_(float x) { return floorf(x); }
+__device__ __forceinline__ double floor_(double x) { return floor(x); }
 
 // ------------------------------------------------------------------------------------------------
 // primitives  W = (rho, vx, vy, vz, P); floors act only here (reading A6)
@@ -445,23 +461,68 @@ __device__ __forceinline__ void cool_vjp(const T U[5], T dt, const Consts<T>& c,
 // ------------------------------------------------------------------------------------------------
 constexpr int DH_COOL_NSUB_MAX = 64;
 
+// Lambda_CIE(T) of Eq. 19 and d Lambda / dT: interpolation between the nodes, end values held (reading A25)
 template <class T>
-__device__ __forceinline__ T cool_rate(T Eth, T rho, T r, const Consts<T>& c) {
-  const T Tg = max_(c.gm1 * Eth * r, T(0));
-  const T Ta = c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0));
-  return -(rho * rho * c.lambda0) * Ta;
+__device__ __forceinline__ T lambda_table(T Tg, const Consts<T>& c, T& dlam, int& kout, T& wout) {
+  const T u = (log2_(Tg) - c.tab_l2t0) * c.tab_inv_dl2t;
+  int k = (int)floor_(u);
+  k = k < 0 ? 0 : (k > c.ntab - 2 ? c.ntab - 2 : k);
+  T w = u - T(k);
+  const bool held = (w < T(0)) || (w > T(1));
+  w = w < T(0) ? T(0) : (w > T(1) ? T(1) : w);
+  const T a = c.tab[k], slope = c.tab[k + 1] - a;
+  const T lam = exp2_(a + w * slope);
+  dlam = held ? T(0) : lam * slope * c.tab_inv_dl2t * rcp_(Tg);    // d/dT exp2(a + slope (log2 T - l0) / dl)
+  kout = k; wout = w;
+  return lam;
 }
 
-// (Ethb, rhob) += (dEdot/dE_th, dEdot/drho) * rateb
+// Edot = n_H Gamma - n_H^2 Lambda (Eqs. 15, 20), n_H = rho, T = (gamma-1) E_th / rho
 template <class T>
-__device__ __forceinline__ void cool_rate_vjp(T Eth, T rho, T r, const Consts<T>& c, T rateb, T& Ethb, T& rhob) {
+__device__ __forceinline__ T cool_rate(T Eth, T rho, T r, const Consts<T>& c) {
+  const T Traw = c.gm1 * Eth * r;
+  const T Tg = max_(Traw, T(0));
+  if (c.cool_law == 0) {
+    const T Ta = c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0));
+    return -(rho * rho * c.lambda0) * Ta;
+  }
+  if (Traw < c.t_switch) {                                  // Eq. 17, lower branch: Eq. 18 and Gamma_0
+    const T lam = (Tg > T(0)) ? c.lambda1 * pow_(Tg, c.alpha1) + c.lambda2 * pow_(Tg, c.alpha2) : T(0);
+    return rho * c.gamma0 - rho * rho * lam;
+  }
+  T dlam, w;
+  int k;
+  return -(rho * rho) * lambda_table(Tg, c, dlam, k, w);
+}
+
+// (Ethb, rhob) += (dEdot/dE_th, dEdot/drho) * rateb;  tabacc != NULL: also tabacc[k] += d Edot / d tab[k] * rateb
+// (shared-memory accumulator of the table gradient, in the table's own units of log2 Lambda)
+template <class T>
+__device__ __forceinline__ void cool_rate_vjp(T Eth, T rho, T r, const Consts<T>& c, T rateb, T& Ethb, T& rhob, double* tabacc = nullptr) {
   const T Traw = c.gm1 * Eth * r;
   const bool Tpos = (Traw >= T(0));
   const T Tg = Tpos ? Traw : T(0);
-  const T Ta = c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0));
-  const T dTa = (Tpos && Tg > T(0)) ? c.alpha * Ta * rcp_(Tg) : T(0);
-  const T Tb = -rateb * rho * rho * c.lambda0 * dTa;
-  rhob += -rateb * T(2) * rho * c.lambda0 * Ta;
+  T lam, dlam, g0 = T(0);                                  // rate = rho g0 - rho^2 lam
+  if (c.cool_law == 0) {
+    lam = c.lambda0 * (c.alpha_is_half ? sqrt_(Tg) : ((Tg > T(0)) ? pow_(Tg, c.alpha) : T(0)));
+    dlam = (Tpos && Tg > T(0)) ? c.alpha * lam * rcp_(Tg) : T(0);
+  } else if (Traw < c.t_switch) {
+    const T l1 = (Tg > T(0)) ? c.lambda1 * pow_(Tg, c.alpha1) : T(0), l2 = (Tg > T(0)) ? c.lambda2 * pow_(Tg, c.alpha2) : T(0);
+    lam = l1 + l2;
+    dlam = (Tpos && Tg > T(0)) ? (c.alpha1 * l1 + c.alpha2 * l2) * rcp_(Tg) : T(0);
+    g0 = c.gamma0;
+  } else {
+    int k;
+    T w;
+    lam = lambda_table(Tg, c, dlam, k, w);
+    if (tabacc) {                                          // d lam / d tab[k] = lam ln2 (1 - w), d lam / d tab[k+1] = lam ln2 w
+      const double t = -(double)rateb * (double)(rho * rho) * (double)lam * 0.6931471805599453;
+      atomicAdd(tabacc + k, t * (1.0 - (double)w));
+      atomicAdd(tabacc + k + 1, t * (double)w);
+    }
+  }
+  const T Tb = -rateb * rho * rho * dlam;
+  rhob += rateb * (g0 - T(2) * rho * lam);
   Ethb += Tb * c.gm1 * r;
   rhob += -Tb * Traw * r;
 }
@@ -473,7 +534,9 @@ __device__ __forceinline__ T cool_energy_general(const T U[5], T dt, const Const
   const T Ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * r;
   T Eth = U[4] - Ek;
   const T Efl = rho * c.t_floor * c.inv_gm1;
-  if (c.cool_mode == 1) {
+  int mode = c.cool_mode;
+  if (mode == 2) mode = (dt * abs_(cool_rate(Eth, rho, r, c)) > c.f_sub * abs_(Eth)) ? 0 : 1;   // masked choice per cell
+  if (mode == 1) {
     const T rn = cool_rate(Eth, rho, r, c);
     const T Ep = max_(Efl, Eth + rn * dt);
     const T rp = cool_rate(Ep, rho, r, c);
@@ -488,7 +551,7 @@ __device__ __forceinline__ T cool_energy_general(const T U[5], T dt, const Const
 
 // gbar = J_cool(U1)^T g for the integrators above (U1: pre-cooling state); max(E_floor, x) ties -> the floor
 template <class T>
-__device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Consts<T>& c, const T g[5], T gb[5]) {
+__device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Consts<T>& c, const T g[5], T gb[5], double* tabacc = nullptr) {
   const T rho = U[0];
   const T r = rcp_(rho);
   const T Ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) * r;
@@ -497,7 +560,9 @@ __device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Const
   const T dfl = c.t_floor * c.inv_gm1;          // dE_floor / drho
   const T gE = g[4];
   T Ethb = T(0), rhob = T(0);                   // cotangents of E_th^0 and rho
-  if (c.cool_mode == 1) {
+  int mode = c.cool_mode;
+  if (mode == 2) mode = (dt * abs_(cool_rate(Eth0, rho, r, c)) > c.f_sub * abs_(Eth0)) ? 0 : 1;   // the choice itself has no derivative
+  if (mode == 1) {
     const T rn = cool_rate(Eth0, rho, r, c);
     const T candp = Eth0 + rn * dt;
     const bool flp = !(Efl < candp);
@@ -511,9 +576,9 @@ __device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Const
       T rnb = T(0.5) * dt * gE;
       const T rpb = rnb;
       T Epb = T(0);
-      cool_rate_vjp(Ep, rho, r, c, rpb, Epb, rhob);
+      cool_rate_vjp(Ep, rho, r, c, rpb, Epb, rhob, tabacc);
       if (flp) rhob += Epb * dfl; else { Ethb += Epb; rnb += Epb * dt; }
-      cool_rate_vjp(Eth0, rho, r, c, rnb, Ethb, rhob);
+      cool_rate_vjp(Eth0, rho, r, c, rnb, Ethb, rhob, tabacc);
     }
   } else {
     const int nsub = c.cool_nsub;
@@ -532,7 +597,7 @@ __device__ __forceinline__ void cool_vjp_general(const T U[5], T dt, const Const
       const T cand = Es[k] + cool_rate(Es[k], rho, r, c) * ddt;
       if (!(Efl < cand)) { rhob += eb * dfl; eb = T(0); break; }   // floored: nothing earlier matters
       T ekb = eb;
-      cool_rate_vjp(Es[k], rho, r, c, eb * ddt, ekb, rhob);
+      cool_rate_vjp(Es[k], rho, r, c, eb * ddt, ekb, rhob, tabacc);
       eb = ekb;
     }
     Ethb = eb;

@@ -171,17 +171,62 @@ __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
   }
 }
 
+constexpr int DH_TAB_MAX = 256;
+
+// the table of the two-branch law into shared memory (DH_OPT_COOL_LAW = 1); returns the Consts to use in this block
+template <class T>
+__device__ __forceinline__ Consts<T> stage_table(const Consts<T>& c, T* stab) {
+  Consts<T> cc = c;
+  if (c.cool_law != 0) {
+    for (int i = threadIdx.x; i < c.ntab; i += blockDim.x) stab[i] = c.tab[i];
+    __syncthreads();
+    cc.tab = stab;
+  }
+  return cc;
+}
+
 template <class T>
 __global__ void __launch_bounds__(256) cool_vjp_kernel(const T* __restrict__ U1, const T* __restrict__ g, T* __restrict__ gout,
                                                        size_t N, T dt, Consts<T> c) {
+  __shared__ T stab[DH_TAB_MAX];
+  const Consts<T> cc = stage_table(c, stab);
+  const bool general = cc.cool_mode != 0 || cc.cool_nsub > 1 || cc.cool_law != 0;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
     T u[5], gi[5], gb[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) { u[f] = U1[f * N + i]; gi[f] = g[f * N + i]; }
-    if (c.cool_mode != 0 || c.cool_nsub > 1) cool_vjp_general(u, dt, c, gi, gb); else cool_vjp(u, dt, c, gi, gb);
+    if (general) cool_vjp_general(u, dt, cc, gi, gb); else cool_vjp(u, dt, cc, gi, gb);
 #pragma unroll
     for (int f = 0; f < 5; ++f) gout[f * N + i] = gb[f];
   }
+}
+
+// Gradient of sum(g_E * E_out) with respect to the table nodes, at the pre-cooling state U1: every block
+// accumulates the contributions of its cells in shared memory (fp64), writes its partial sums, and cool_table_sum_kernel
+// adds the blocks in a fixed order.
+template <class T>
+__global__ void __launch_bounds__(256) cool_table_vjp_kernel(const T* __restrict__ U1, const T* __restrict__ g, size_t N, T dt, Consts<T> c,
+                                                             double* __restrict__ part) {
+  __shared__ T stab[DH_TAB_MAX];
+  __shared__ double acc[DH_TAB_MAX];
+  for (int i = threadIdx.x; i < c.ntab; i += blockDim.x) acc[i] = 0.0;
+  const Consts<T> cc = stage_table(c, stab);          // (its barrier also publishes the zeroed accumulator)
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
+    T u[5], gi[5], gb[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) { u[f] = U1[f * N + i]; gi[f] = (f == 4) ? g[f * N + i] : T(0); }
+    cool_vjp_general(u, dt, cc, gi, gb, acc);
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < c.ntab; i += blockDim.x) part[(size_t)blockIdx.x * c.ntab + i] = acc[i];
+}
+
+__global__ void cool_table_sum_kernel(const double* __restrict__ part, int nblocks, int ntab, double scale, double* __restrict__ out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= ntab) return;
+  double s = 0.0;
+  for (int b = 0; b < nblocks; ++b) s += part[(size_t)b * ntab + k];
+  out[k] = s * scale;
 }
 
 // limiter in {0, 1, 2} x riemann in {0, 1, 2} -> one instantiation each
@@ -216,12 +261,14 @@ cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cu
 // Eq. 22; DH_OPT_COOL_MODE / DH_OPT_COOL_NSUB): reads the 5 fields, rewrites E.  dt from the device when dt_dev != NULL.
 template <class T>
 __global__ void __launch_bounds__(256) cool_fwd_kernel(T* __restrict__ U, size_t N, T dt_host, const T* __restrict__ dt_dev, Consts<T> c) {
+  __shared__ T stab[DH_TAB_MAX];
+  const Consts<T> cc = stage_table(c, stab);
   const T dt = dt_dev ? *dt_dev : dt_host;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) {
     T u[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) u[f] = U[f * N + i];
-    U[4 * N + i] = cool_energy_general(u, dt, c);
+    U[4 * N + i] = cool_energy_general(u, dt, cc);
   }
 }
 
@@ -241,6 +288,23 @@ cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, co
   return cudaGetLastError();
 }
 
+// gtab (DEVICE, ntab doubles) = d sum(g_E E_out) / d (log10 Lambda at the nodes); part: DEVICE scratch of cool_table_blocks() x ntab
+int cool_table_blocks() { return 148 * 4; }
+
+template <class T>
+cudaError_t launch_cool_table_vjp(const T* U1, const T* g, size_t N, T dt, const Consts<T>& c, double* part, double* gtab, cudaStream_t s) {
+  int blocks = (int)((N + 255) / 256);
+  if (blocks > cool_table_blocks()) blocks = cool_table_blocks();
+  cool_table_vjp_kernel<T><<<blocks, 256, 0, s>>>(U1, g, N, dt, c, part);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  // the table is held as log2 Lambda: d / d log10 Lambda = log2(10) d / d log2 Lambda
+  cool_table_sum_kernel<<<(c.ntab + 63) / 64, 64, 0, s>>>(part, blocks, c.ntab, 3.321928094887362, gtab);
+  return cudaGetLastError();
+}
+
+template cudaError_t launch_cool_table_vjp<float>(const float*, const float*, size_t, float, const Consts<float>&, double*, double*, cudaStream_t);
+template cudaError_t launch_cool_table_vjp<double>(const double*, const double*, size_t, double, const Consts<double>&, double*, double*, cudaStream_t);
 template cudaError_t launch_stage_naive<float>(const StageParams<float>&, int, int, cudaStream_t);
 template cudaError_t launch_stage_naive<double>(const StageParams<double>&, int, int, cudaStream_t);
 template cudaError_t launch_rev_naive<float>(const RevParams<float>&, int, int, cudaStream_t);

@@ -20,11 +20,13 @@ DH_OK, DH_ERR_ARG, DH_ERR_CUDA, DH_ERR_ALLOC, DH_ERR_NONFINITE = 0, -1, -2, -3, 
 OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
-    "riemann": 15, "cool_mode": 16, "cool_nsub": 17, "c_cool": 18, "dt_max": 19,
+    "riemann": 15, "cool_mode": 16, "cool_nsub": 17, "c_cool": 18, "dt_max": 19, "cool_law": 20, "t_switch": 21,
+    "lambda1": 22, "alpha1": 23, "lambda2": 24, "alpha2": 25, "gamma0": 26, "f_sub": 27,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
-COOL_MODES = {"euler": 0, "trapezoid": 1}           # DH_OPT_COOL_MODE
+COOL_MODES = {"euler": 0, "trapezoid": 1, "masked": 2}   # DH_OPT_COOL_MODE
+COOL_LAWS = {"powerlaw": 0, "twobranch": 1}         # DH_OPT_COOL_LAW
 INTEGRATORS = {"vl2": 0, "heun": 1, "ssprk3": 2}    # DH_OPT_INTEGRATOR
 KERNELS = {"fused": 0, "gather": 1}
 
@@ -33,7 +35,7 @@ SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
-    "dh_cfl_stats", "dh_cool_tmin",
+    "dh_cfl_stats", "dh_cool_tmin", "dh_set_cooling_table", "dh_cool_table_vjp",
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
     "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
@@ -84,6 +86,10 @@ def load(rebuild: bool = False):
     lib.dh_cfl_stats.restype = ci
     lib.dh_cool_tmin.argtypes = [vp, vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.dh_cool_tmin.restype = ci
+    lib.dh_set_cooling_table.argtypes = [vp, pd, ci, cd, cd]
+    lib.dh_set_cooling_table.restype = ci
+    lib.dh_cool_table_vjp.argtypes = [vp, vp, cd, vp, pd]
+    lib.dh_cool_table_vjp.restype = ci
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
@@ -222,6 +228,20 @@ def dh_cool_tmin(ctx, U_ptr: int):
     return t.value, d.value
 
 
+def dh_set_cooling_table(ctx, log10_lambda, log10_t0: float, dlog10_t: float) -> None:
+    """The table of Eq. 19 for DH_OPT_COOL_LAW = 1 (include/dh.h): log10 Lambda at equally spaced log10 T nodes."""
+    vals = [float(v) for v in log10_lambda]
+    arr = (ctypes.c_double * len(vals))(*vals)
+    _check(load().dh_set_cooling_table(ctx, arr, len(vals), float(log10_t0), float(dlog10_t)))
+
+
+def dh_cool_table_vjp(ctx, U: int, dt: float, g_out: int, n: int) -> list:
+    """dL / d log10_lambda[k] for the step at this dt and the cotangent g_out (device pointers), include/dh.h."""
+    out = (ctypes.c_double * n)()
+    _check(load().dh_cool_table_vjp(ctx, U, float(dt), g_out, out))
+    return [float(v) for v in out]
+
+
 def dh_cfl_stats(ctx) -> dict:
     """Counters of the CFL candidate path of dh_advance (include/dh.h)."""
     out = (ctypes.c_ulonglong * 3)()
@@ -253,6 +273,9 @@ class Solver:
         stream = stream if stream is not None else torch.cuda.current_stream()
         dh_set_stream(self.ctx, stream.cuda_stream)
         self.stream = stream
+        table = options.pop("table", None)            # (log10_t0, dlog10_t, values): must precede cool_law = 1
+        if table is not None:
+            self.set_cooling_table(*table)
         self.set_options(**options)
 
     def set_options(self, **options):
@@ -261,6 +284,8 @@ class Solver:
                 v = LIMITERS[v]
             if k == "cool_mode" and isinstance(v, str):
                 v = COOL_MODES[v]
+            if k == "cool_law" and isinstance(v, str):
+                v = COOL_LAWS[v]
             if k == "riemann" and isinstance(v, str):
                 v = RIEMANN[v]
             if k == "integrator" and isinstance(v, str):
@@ -309,6 +334,13 @@ class Solver:
             g_in = torch.empty_like(U)
         dh_step_vjp(self.ctx, self._dev(U, "U"), dt, self._dev(g_out, "g_out"), self._dev(g_in, "g_in"))
         return g_in
+
+    def set_cooling_table(self, log10_t0: float, dlog10_t: float, log10_lambda) -> None:
+        self._ntab = len(log10_lambda)
+        dh_set_cooling_table(self.ctx, log10_lambda, log10_t0, dlog10_t)
+
+    def cool_table_vjp(self, U, dt: float, g_out) -> list:
+        return dh_cool_table_vjp(self.ctx, self._dev(U, "U"), dt, self._dev(g_out, "g_out"), self._ntab)
 
     def run_host(self, U_host, nsteps: int) -> float:
         return dh_run_host(self.ctx, self._host(U_host, "U_host"), nsteps)

@@ -1094,7 +1094,7 @@ def test_cooling_integrator_option_errors():
     from paper_2512_13403_b200 import dh
     U = random_state((4, 4, 4), 631, 1.4, torch.float32)
     s = _solver(U, 1.4)
-    for key, bad in (("cool_nsub", 0), ("cool_nsub", 65), ("cool_nsub", 2.5), ("cool_mode", 2), ("riemann", 3)):
+    for key, bad in (("cool_nsub", 0), ("cool_nsub", 65), ("cool_nsub", 2.5), ("cool_mode", 3), ("riemann", 3)):
         with pytest.raises(dh.DhError):
             s.set_options(**{key: bad})
     assert s.get_option("cool_nsub") == 1 and s.get_option("cool_mode") == 0
