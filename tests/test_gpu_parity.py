@@ -757,6 +757,35 @@ def test_step_and_vjp_are_bitwise_reproducible(dtype):
     assert torch.equal(grads[0], grads[1]) and torch.equal(grads[0], grads[2])
 
 
+@pytest.mark.parametrize("dtype", [torch.float32, torch.float64])
+def test_results_do_not_depend_on_scheduling_noise(dtype):
+    """The race detector of this suite (compute-sanitizer is closed on the pool, profiles/r02_sanitizer.md): the same step and
+    VJP repeated while a second stream keeps the SMs and the memory system busy with unrelated work of varying size, so
+    that block placement, residency and warp interleaving differ between repeats.  The kernels exchange data only
+    through barrier-ordered shared slots and never through atomics, so every repeat must give the same bits."""
+    U = random_state((70, 45, 200), 321, 5 / 3, dtype, mach=1.0).cuda()
+    s = _solver(U, 5 / 3, rev_slab=16)
+    dt = s.cfl_dt(U)
+    g = torch.randn_like(U)
+    ref_out = U.clone()
+    s.step(ref_out, dt)
+    ref_g = s.step_vjp(U, dt, g).clone()
+    side = torch.cuda.Stream()
+    a = torch.randn(2048, 2048, device="cuda")
+    big = torch.empty(64 * 1024 * 1024, device="cuda")
+    for rep in range(8):
+        with torch.cuda.stream(side):                     # noise: GEMMs and fills of rep-dependent length
+            for _ in range(1 + rep % 4):
+                a = (a @ a).tanh_()
+                big.fill_(float(rep))
+        V = U.clone()
+        s.step(V, dt)
+        gin = s.step_vjp(U, dt, g)
+        torch.cuda.synchronize()
+        assert torch.equal(V, ref_out), rep
+        assert torch.equal(gin, ref_g), rep
+
+
 # ------------------------------------------------------------------ multi-step adjoint (SURVEY §8(f) item 1)
 @pytest.mark.parametrize("every", [1, 2, 5, 7])
 def test_adjoint_checkpointed_fp64_matches_oracle_composition(every):
