@@ -282,6 +282,25 @@ int dh_mg_solve(dh_mg* ctx, const void* F, void* phi, int ncycles, double* rel_r
  * the forward solve is stored. */
 int dh_mg_solve_vjp(dh_mg* ctx, const void* g_phi, void* g_F, int ncycles, double* rel_residual);
 
+/* ---- Self-gravity as a source term of the hydro step (section 6; the force-class form of PAPER.md:88-107) ----
+ * g = -grad phi by second-order central differences on the periodic grid (reading A27), then the operator-split
+ * update  u <- u + s_g dt,  s_g = (0, rho g, m . g)  with rho, m of the incoming u.  phi: DEVICE [nz][ny][nx] of the
+ * context's dtype (e.g. from dh_mg_solve).  In place, asynchronous on the context's stream; dx_a = L_a / n_a. */
+int dh_gravity_source(dh_ctx* ctx, void* U, const void* phi, double dt);
+
+/* Transpose of dh_gravity_source at (U, phi): gU_in = dL/dU (DEVICE state, overwritten), gphi = dL/dphi (DEVICE field,
+ * overwritten) from gU_out = dL/d(out).  gU_in must not alias U or gU_out. */
+int dh_gravity_source_vjp(dh_ctx* ctx, const void* U, const void* phi, double dt, const void* gU_out, void* gU_in, void* gphi);
+
+/* One self-gravitating step (reading A27): phi from ncycles multigrid cycles on 4 pi G rho of the incoming U (mean removed,
+ * reading A23; `mg` must have the grid of `ctx` with h = dx and the same dtype; it is switched to ctx's stream), the hydro step
+ * dh_step(U, dt) (cooling, limiter, ... as configured), then the kick dh_gravity_source with that phi.  In place. */
+int dh_step_gravity(dh_ctx* ctx, dh_mg* mg, void* U, double dt, double four_pi_g, int ncycles);
+
+/* VJP of dh_step_gravity, dt held constant: through the kick (the post-hydro state is recomputed), the Poisson solve (another
+ * solve, Eqs. 46-48) and the hydro step (dh_step_vjp).  U = U^n (pre-step); gU_in overwritten, must not alias U or gU_out. */
+int dh_step_gravity_vjp(dh_ctx* ctx, dh_mg* mg, const void* U, double dt, double four_pi_g, int ncycles, const void* gU_out, void* gU_in);
+
 #ifdef __cplusplus
 }
 #endif

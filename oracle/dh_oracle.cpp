@@ -136,6 +136,12 @@ int dho_decision_margins(int nx, int ny, int nz, const Params* p, const double* 
   return 0;
 }
 
+// conditioning of the limiter's derivative at U: C is [3][nz][ny][nx] (van Leer; zero for minmod / MC)
+int dho_limiter_conditioning(int nx, int ny, int nz, const Params* p, const double* U, double* C) {
+  limiter_conditioning(mkgrid(nx, ny, nz), *p, U, C);
+  return 0;
+}
+
 // margins of the compares of cool() at the pre-cooling state U1: M is [nz][ny][nx]
 int dho_cooling_margins(int nx, int ny, int nz, const Params* p, double dt, const double* U1, double* M) {
   cooling_margins(mkgrid(nx, ny, nz), *p, dt, U1, M);

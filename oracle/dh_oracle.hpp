@@ -750,6 +750,41 @@ inline void decision_margins(const Grid& g, const Params& p, const double* U, do
   }
 }
 
+// Conditioning of the limiter's derivative (van Leer only): d lim / da = 2 b^2 / (a + b)^2 is smooth but depends on the RATIO of the
+// two differences: an error eps s in them (s: the rounding scale of margin_scales) changes it by at most ~ 12 eps s / (|a| + |b|)
+// (|d/da|, |d/db| of 2 b^2 / (a+b)^2 are bounded by 4 / (a + b) for a b > 0).
+// C[a][i] = max over the five fields of s / (|a| + |b|) at cell i along axis a where the slope is active (a b > 0), else 0.
+// minmod and MC have piecewise-constant derivatives: C = 0.
+inline void limiter_conditioning(const Grid& g, const Params& p, const double* U, double* C) {
+  const size_t N = g.N();
+  std::vector<double> W(5 * N);
+  compute_prims(g, p, U, W.data());
+  for (int ax = 0; ax < 3; ++ax) {
+#pragma omp parallel for schedule(static)
+    for (int k = 0; k < g.n[2]; ++k)
+      for (int j = 0; j < g.n[1]; ++j)
+        for (int i = 0; i < g.n[0]; ++i) {
+          const size_t cm1 = shifted(g, i, j, k, ax, -1), c0 = g.idx(i, j, k), cp1 = shifted(g, i, j, k, ax, +1);
+          double worst = 0.0;
+          if (p.limiter == 1) {
+            double w[3][5], sc[3][5];
+            const size_t cs[3] = {cm1, c0, cp1};
+            for (int m = 0; m < 3; ++m) {
+              for (int q = 0; q < 5; ++q) w[m][q] = W[q * N + cs[m]];
+              margin_scales(w[m], p.gamma, sc[m]);
+            }
+            for (int q = 0; q < 5; ++q) {
+              const double a = w[2][q] - w[1][q], b = w[1][q] - w[0][q];
+              if (a * b <= 0.0) continue;
+              const double s = std::fmax(sc[0][q], std::fmax(sc[1][q], sc[2][q]));
+              worst = std::fmax(worst, s / (std::fabs(a) + std::fabs(b)));
+            }
+          }
+          C[(size_t)ax * N + c0] = worst;
+        }
+  }
+}
+
 // the compares of cool() at the pre-cooling state U1: T > 0 and (law 1) T < t_switch and the table interval inside every
 // cool_rate(), every max with E_floor, and (mode 2) the masked choice of the integrator; relative to E_kin + |E_th| (E_th is
 // a difference of E and E_kin)

@@ -271,6 +271,16 @@ def decision_margins(U, p):
     return M
 
 
+def limiter_conditioning(U, p):
+    """[3, nz, ny, nx]: s / (|a| + |b|) of the active slopes at every cell and axis (van Leer: the relative sensitivity of the
+    limiter's derivative to rounding of the differences; zero for minmod / MC).  dh_oracle.hpp, "Conditioning of the limiter"."""
+    lib = _load()
+    U = _f64(U)
+    C = np.empty((3,) + U.shape[1:], dtype=np.float64)
+    lib.dho_limiter_conditioning(*_dims(U), ctypes.byref(p), _ptr(U), _ptr(C))
+    return C
+
+
 def cooling_margins(U1, dt, p):
     """[nz, ny, nx]: margins of the compares of the cooling update applied to the pre-cooling state U1."""
     lib = _load()

@@ -175,7 +175,7 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev, c->tab_dev, c->tab_dev_d, c->tab_part};
+  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev, c->tab_dev, c->tab_dev_d, c->tab_part, c->grav_phi, c->grav_F, c->grav_gb, c->grav_U1, c->grav_g1};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
@@ -466,13 +466,14 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
   const int ntx = (c->nx + 63) / 64;                       // tiles per row of rev_faces_kernel (RTX = 64)
   const size_t EP = (size_t)c->ny * ntx * 2;               // tile-edge words per plane and field
   const int want = c->rev_slab_opt > 0 ? (c->rev_slab_opt < c->nz ? c->rev_slab_opt : c->nz) : 0;
-  if (c->rev_scratch && want > 0 && want != c->rev_slab) {      // the option changed: resize
+  const int words = rev_scratch_words(c->limiter);
+  if (c->rev_scratch && ((want > 0 && want != c->rev_slab) || words != c->rev_words)) {      // an option changed: resize
     DH_CUDA(cudaStreamSynchronize(c->stream), "dh_step_vjp: synchronize");
     cudaFree(c->rev_scratch);
     c->rev_scratch = nullptr;
   }
   if (!c->rev_scratch) {
-    const size_t per_plane = (10 * NP + 5 * EP) * elem_size(c);
+    const size_t per_plane = ((size_t)words * NP + 5 * EP) * elem_size(c);
     long long planes = want;
     if (planes == 0) {
       size_t free_b = 0, total_b = 0;
@@ -486,6 +487,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
     int rc = lazy_alloc(c, &c->rev_scratch, (size_t)planes * per_plane, "the reverse-stage scratch");
     if (rc) return rc;
     c->rev_slab = (int)planes;
+    c->rev_words = words;
   }
   const int SP = c->rev_slab;
   const int n[3] = {c->nx, c->ny, c->nz};
@@ -493,7 +495,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
   a.U = (const T*)U; a.g = (const T*)g;
   a.Wp = (T*)c->rev_scratch;
   a.C = a.Wp + (size_t)5 * SP * NP;
-  a.Ce = a.C + (size_t)5 * SP * NP;
+  a.Ce = a.C + (size_t)(words - 5) * SP * NP;
   a.nx = c->nx; a.ny = c->ny; a.nz = c->nz;
   a.sp0 = 0; a.SP = SP; a.ntx = ntx; a.SPE = (size_t)SP * EP;
   for (int k = 0; k < 3; ++k) a.coef[k] = (T)(frac * dt * n[k] / c->L[k]);
@@ -505,9 +507,9 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
   for (int z0 = 0; z0 < c->nz; z0 += c->rev_slab) {
     const int nplanes = (c->nz - z0 < c->rev_slab) ? c->nz - z0 : c->rev_slab;
     a.zs = z0; a.nout = nplanes;
-    DH_CUDA(launch_rev_faces<T>(a, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
+    DH_CUDA(launch_rev_faces<T>(a, c->limiter, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
     b.z0 = z0; b.nplanes = nplanes;
-    DH_CUDA(launch_rev_gather<T>(b, c->stream), "dh_step_vjp: gather kernel launch");
+    DH_CUDA(launch_rev_gather<T>(b, c->limiter, c->stream), "dh_step_vjp: gather kernel launch");
     c->launches += 2;
   }
   return DH_OK;
@@ -515,8 +517,8 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
 
 template <class T>
 static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
-  // the fused pair handles minmod on even nx; everything else takes the one-thread-per-cell gather kernel
-  if (c->kernel == 0 && c->limiter == 0 && c->riemann == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
+  // the fused pair handles HLLC (any limiter) on even nx; everything else takes the one-thread-per-cell gather kernel
+  if (c->kernel == 0 && c->riemann == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
   return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
 }
 
@@ -842,6 +844,114 @@ int dh_adjoint(dh_ctx* c, void* U, void* gU, int nsteps, int every, double* dts_
   }
   if (g != gU) DH_CUDA(cudaMemcpyAsync(gU, g, sb, cudaMemcpyDeviceToDevice, c->stream), "dh_adjoint: result copy");
   return DH_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ self-gravity
+template <class T>
+static int grav_source_impl(dh_ctx* c, void* U, const void* phi, double dt) {
+  const double dx[3] = {c->L[0] / c->nx, c->L[1] / c->ny, c->L[2] / c->nz};
+  DH_CUDA(launch_grav_source<T>((T*)U, (const T*)phi, c->nx, c->ny, c->nz, dx, (T)dt, nullptr, c->stream), "dh_gravity_source: kernel launch");
+  c->launches += 1;
+  return DH_OK;
+}
+
+template <class T>
+static int grav_source_vjp_impl(dh_ctx* c, const void* U, const void* phi, double dt, const void* gout, void* gin, void* gphi) {
+  int rc = lazy_alloc(c, &c->grav_gb, 3 * c->N * elem_size(c), "the acceleration cotangents");
+  if (rc) return rc;
+  const double dx[3] = {c->L[0] / c->nx, c->L[1] / c->ny, c->L[2] / c->nz};
+  DH_CUDA(launch_grav_source_vjp<T>((const T*)U, (const T*)phi, (const T*)gout, (T*)gin, (T*)c->grav_gb, (T*)gphi, c->nx, c->ny, c->nz, dx, (T)dt, c->stream),
+          "dh_gravity_source_vjp: kernel launch");
+  c->launches += 2;
+  return DH_OK;
+}
+
+static int grav_check(dh_ctx* c, dh_mg* mg, const char* who) {
+  if (!c || !mg) return fail(DH_ERR_ARG, "%s: NULL context", who);
+  if (int drc = check_device(c, who)) return drc;
+  return DH_OK;
+}
+
+// phi of the incoming density into c->grav_phi (Eq. 27; the solver removes the mean of the right-hand side, reading A23)
+template <class T>
+static int grav_potential(dh_ctx* c, dh_mg* mg, const void* U, double four_pi_g, int ncycles) {
+  int rc = lazy_alloc(c, &c->grav_phi, c->N * elem_size(c), "the gravitational potential");
+  if (rc) return rc;
+  rc = lazy_alloc(c, &c->grav_F, c->N * elem_size(c), "the Poisson right-hand side");
+  if (rc) return rc;
+  DH_CUDA(launch_grav_rhs<T>((const T*)U, (T*)c->grav_F, c->N, (T)four_pi_g, c->stream), "dh_step_gravity: right-hand side kernel");
+  c->launches += 1;
+  if (dh_mg_set_stream(mg, (void*)c->stream) != DH_OK) return fail(DH_ERR_ARG, "dh_step_gravity: %s", dh_last_error());
+  if (dh_mg_solve(mg, c->grav_F, c->grav_phi, ncycles, nullptr) != DH_OK) return fail(DH_ERR_CUDA, "dh_step_gravity: Poisson solve: %s", dh_last_error());
+  return DH_OK;
+}
+
+template <class T>
+static int step_gravity_impl(dh_ctx* c, dh_mg* mg, void* U, double dt, double four_pi_g, int ncycles) {
+  int rc = grav_potential<T>(c, mg, U, four_pi_g, ncycles);
+  if (rc) return rc;
+  rc = dh_step(c, U, dt);
+  if (rc) return rc;
+  return grav_source_impl<T>(c, U, c->grav_phi, dt);
+}
+
+template <class T>
+static int step_gravity_vjp_impl(dh_ctx* c, dh_mg* mg, const void* U, double dt, double four_pi_g, int ncycles, const void* gout, void* gin) {
+  int rc = lazy_alloc(c, &c->grav_U1, state_bytes(c), "the post-hydro state");
+  if (rc) return rc;
+  rc = lazy_alloc(c, &c->grav_g1, state_bytes(c), "the post-hydro cotangent");
+  if (rc) return rc;
+  rc = grav_potential<T>(c, mg, U, four_pi_g, ncycles);                       // recompute: nothing was stored
+  if (rc) return rc;
+  DH_CUDA(cudaMemcpyAsync(c->grav_U1, U, state_bytes(c), cudaMemcpyDeviceToDevice, c->stream), "dh_step_gravity_vjp: copy");
+  rc = dh_step(c, c->grav_U1, dt);
+  if (rc) return rc;
+  // through the kick at the post-hydro state: cotangents of that state and of phi (into grav_F)
+  rc = grav_source_vjp_impl<T>(c, c->grav_U1, c->grav_phi, dt, gout, c->grav_g1, c->grav_F);
+  if (rc) return rc;
+  // through the Poisson solve: another solve (Eqs. 46-48), result into grav_phi (the potential is dead)
+  if (dh_mg_solve_vjp(mg, c->grav_F, c->grav_phi, ncycles, nullptr) != DH_OK) return fail(DH_ERR_CUDA, "dh_step_gravity_vjp: adjoint Poisson solve: %s", dh_last_error());
+  // through the hydro step, then the density cotangent of the right-hand side F = 4 pi G rho
+  rc = dh_step_vjp(c, U, dt, c->grav_g1, gin);
+  if (rc) return rc;
+  DH_CUDA(launch_grav_rhs_vjp<T>((const T*)c->grav_phi, (T*)gin, c->N, (T)four_pi_g, c->stream), "dh_step_gravity_vjp: right-hand side transpose");
+  c->launches += 1;
+  return DH_OK;
+}
+
+extern "C" {
+
+int dh_gravity_source(dh_ctx* c, void* U, const void* phi, double dt) {
+  if (!c || !U || !phi) return fail(DH_ERR_ARG, "dh_gravity_source: NULL argument%s");
+  if (int drc = check_device(c, "dh_gravity_source")) return drc;
+  if (!isfinite(dt)) return fail(DH_ERR_ARG, "dh_gravity_source: dt must be finite%s");
+  return c->dtype == DH_F32 ? grav_source_impl<float>(c, U, phi, dt) : grav_source_impl<double>(c, U, phi, dt);
+}
+
+int dh_gravity_source_vjp(dh_ctx* c, const void* U, const void* phi, double dt, const void* gU_out, void* gU_in, void* gphi) {
+  if (!c || !U || !phi || !gU_out || !gU_in || !gphi) return fail(DH_ERR_ARG, "dh_gravity_source_vjp: NULL argument%s");
+  if (int drc = check_device(c, "dh_gravity_source_vjp")) return drc;
+  if (!isfinite(dt)) return fail(DH_ERR_ARG, "dh_gravity_source_vjp: dt must be finite%s");
+  if (gU_in == gU_out || gU_in == U) return fail(DH_ERR_ARG, "dh_gravity_source_vjp: gU_in must not alias gU_out or U%s");
+  return c->dtype == DH_F32 ? grav_source_vjp_impl<float>(c, U, phi, dt, gU_out, gU_in, gphi) : grav_source_vjp_impl<double>(c, U, phi, dt, gU_out, gU_in, gphi);
+}
+
+int dh_step_gravity(dh_ctx* c, dh_mg* mg, void* U, double dt, double four_pi_g, int ncycles) {
+  if (int rc = grav_check(c, mg, "dh_step_gravity")) return rc;
+  if (!U || ncycles < 1) return fail(DH_ERR_ARG, "dh_step_gravity: bad argument%s");
+  if (!(dt > 0.0) || !isfinite(dt) || !isfinite(four_pi_g)) return fail(DH_ERR_ARG, "dh_step_gravity: dt must be finite and > 0, four_pi_g finite%s");
+  return c->dtype == DH_F32 ? step_gravity_impl<float>(c, mg, U, dt, four_pi_g, ncycles) : step_gravity_impl<double>(c, mg, U, dt, four_pi_g, ncycles);
+}
+
+int dh_step_gravity_vjp(dh_ctx* c, dh_mg* mg, const void* U, double dt, double four_pi_g, int ncycles, const void* gU_out, void* gU_in) {
+  if (int rc = grav_check(c, mg, "dh_step_gravity_vjp")) return rc;
+  if (!U || !gU_out || !gU_in || ncycles < 1) return fail(DH_ERR_ARG, "dh_step_gravity_vjp: bad argument%s");
+  if (!(dt > 0.0) || !isfinite(dt) || !isfinite(four_pi_g)) return fail(DH_ERR_ARG, "dh_step_gravity_vjp: dt must be finite and > 0, four_pi_g finite%s");
+  if (gU_in == U || gU_in == gU_out) return fail(DH_ERR_ARG, "dh_step_gravity_vjp: gU_in must not alias U or gU_out%s");
+  return c->dtype == DH_F32 ? step_gravity_vjp_impl<float>(c, mg, U, dt, four_pi_g, ncycles, gU_out, gU_in)
+                            : step_gravity_vjp_impl<double>(c, mg, U, dt, four_pi_g, ncycles, gU_out, gU_in);
 }
 
 int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {

@@ -138,11 +138,17 @@ struct Ctx {
   void* ga;                    // cotangent of the first stage state (SSPRK3 VJP)
   void* U1;                    // pre-cooling state, cooling VJP only
   void* g1;                    // cotangent of U1, cooling VJP only
+  void* grav_phi;              // self-gravity (dh_step_gravity*): potential, right-hand side / its cotangent, the three acceleration
+  void* grav_F;                //   cotangents, the post-hydro state and the cotangent handed to the hydro VJP
+  void* grav_gb;
+  void* grav_U1;
+  void* grav_g1;
   void* Uhost_dev;             // device state for the HOST entry points
   void* gA;                    // device cotangent buffers for dh_step_vjp_host
   void* gB;
   void* rev_scratch;           // 20 words per cell of a z slab (+2 planes), fused reverse stages
   int rev_slab;                // planes per slab the scratch was sized for
+  int rev_words;               // scratch words per cell it was sized for (depends on the limiter)
   int rev_slab_opt;            // DH_OPT_REV_SLAB (0 = automatic)
   void* adj_states;            // dh_adjoint: checkpoints, one segment of states, one cotangent
   size_t adj_count;            // states allocated there
@@ -179,12 +185,19 @@ template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int l
 template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s, bool* supported);
 template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);
-template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s);
-template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s);
+template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int sm_count, cudaStream_t s);
+int rev_scratch_words(int limiter);
+template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, int limiter, cudaStream_t s);
 template <class T> cudaError_t launch_cool_fwd(T* U, size_t N, T dt, const T* dt_dev, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cool_vjp(const T* U1, const T* g, T* gout, size_t N, T dt, const Consts<T>& c, cudaStream_t s);
 template <class T> cudaError_t launch_cool_table_vjp(const T* U1, const T* g, size_t N, T dt, const Consts<T>& c, double* part, double* gtab, cudaStream_t s);
 int cool_table_blocks();
+// self-gravity source (dh_gravity.cu)
+template <class T> cudaError_t launch_grav_rhs(const T* rho, T* F, size_t N, T four_pi_g, cudaStream_t s);
+template <class T> cudaError_t launch_grav_rhs_vjp(const T* gF, T* grho, size_t N, T four_pi_g, cudaStream_t s);
+template <class T> cudaError_t launch_grav_source(T* U, const T* phi, int nx, int ny, int nz, const double dx[3], T dt, const T* dt_dev, cudaStream_t s);
+template <class T> cudaError_t launch_grav_source_vjp(const T* U, const T* phi, const T* gout, T* gin, T* gb, T* gphi, int nx, int ny, int nz,
+                                                      const double dx[3], T dt, cudaStream_t s);
 template <class T> cudaError_t launch_lincomb(T* out, T a, const T* X, T b, const T* Y, size_t n, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_reduce(const CflParams<T>& p, int sm_count, cudaStream_t s);
 template <class T> cudaError_t launch_cfl_candidates(const CflParams<T>& p, int sm_count, cudaStream_t s);   // candidates, then the guarded full pass

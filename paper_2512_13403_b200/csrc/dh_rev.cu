@@ -42,7 +42,8 @@ template <int NW> struct GeoR {
   static constexpr int XARR = 5 * TY * RXP;
   static constexpr int YARR = 5 * (TY + 1) * RTX;
   static constexpr int STAGE = 5 * TY * RTX;              // cp.async staging of one raw plane of the tile
-  static constexpr int NPARK = 8;                         // staging of the next raw plane + 7 parked carries
+  static constexpr int NPARK = 11;                        // staging of the next raw plane + 7 parked carries (+ 3 for the second
+                                                          // branch factor of the limiters other than minmod)
   static constexpr int TOTAL = 4 * PLANE + 2 * XARR + 2 * YARR + NPARK * STAGE;
   static constexpr int NHALO = 4 * (RSW / 2) + 2 * TY;    // halo packs per plane
   static constexpr int HP = (NHALO + 31) / 32;            // halo packs per helper lane
@@ -238,6 +239,40 @@ DH_DI void hllc_vjp2p(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, co
 
 }  // namespace
 
+// The two halved partial derivatives of the limiter on the branch taken, ha = (d lim / da) / 2, hb = (d lim / db) / 2
+// (a = W_{i+1} - W_i, b = W_i - W_{i-1}): with D = Lb - Rbn (S = D / 2) cell i keeps (hb - ha) D, cell i+1 receives ha D and
+// cell i-1 loses hb D.  minmod has (ha, hb) in {(0,0), (1/2,0), (0,1/2)} and travels as the single factor k = hb - ha
+// (kfac above); van Leer and MC carry both.
+template <class T, int LIM> DH_DI void hfac(T a, T b, T& ha, T& hb) {
+  T da, db;
+  limit_grad<T, LIM>(a, b, da, db);
+  ha = T(0.5) * da; hb = T(0.5) * db;
+}
+// park / fetch the factors of the two cells of a pack (LIM == 0: one array, k; else two arrays)
+template <class T, int LIM> DH_DI void park_h(T* pk, T* pkb, P2<T> a, P2<T> b) {
+  if (LIM == 0) { rsts2(pk, kfac2(a, b)); return; }
+  P2<T> ha, hb;
+  hfac<T, LIM>(a.x, b.x, ha.x, hb.x);
+  hfac<T, LIM>(a.y, b.y, ha.y, hb.y);
+  rsts2(pk, ha); rsts2(pkb, hb);
+}
+template <class T, int LIM> DH_DI void fetch_h(const T* pk, const T* pkb, P2<T>& ha, P2<T>& hb) {
+  if (LIM == 0) {
+    const P2<T> k = rlds2(pk);
+    ha = {max_(-k.x, T(0)), max_(-k.y, T(0))};
+    hb = max2(k, T(0));
+  } else {
+    ha = rlds2(pk); hb = rlds2(pkb);
+  }
+}
+// cell cotangents of one axis: wp = T + own-branch term, P = what the next cell receives, M = what the previous cell loses
+template <class T> DH_DI void cell_terms_h2(P2<T> Lb, P2<T> Rbn, P2<T> ha, P2<T> hb, P2<T>& wp, P2<T>& P, P2<T>& M) {
+  const P2<T> D = sub2(Lb, Rbn);
+  wp = fma2(sub2(hb, ha), D, add2(Lb, Rbn));
+  P = mul2(ha, D);
+  M = mul2(hb, D);
+}
+
 // neighbour terms of an encoded masked slope cotangent c (flag in the LSB = a-branch): what cell i+1 receives from
 // cell i (+c on the a-branch) and what cell i-1 receives from cell i (-c on the b-branch; an inactive slope has c = 0)
 template <class T> DH_DI T pterm(T c) { return dec_flag(c) ? c : T(0); }
@@ -256,7 +291,7 @@ DH_DI double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 //          helper supplies the two cells beside the tile), its own y terms are added, its c^y goes to the scratch
 //   p-2    the z face above it is adjoined: its own z terms and the a-branch term of plane p-3 join the parked sum
 //   p-3    receives the b-branch term of plane p-2 and is stored: Wp' = everything except the y neighbour terms
-template <class T, int NW>
+template <class T, int NW, int LIM>
 __global__ void __launch_bounds__(NW * 32, 1)
 rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
   using G = GeoR<NW>;
@@ -296,11 +331,14 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
     T* const pkz = Ust + 5 * G::STAGE + yo;
     T* const pkw = Ust + 6 * G::STAGE + yo;        //   sum of plane p-2 (still missing the b-branch term of the plane above)
     T* const pkc = Ust + 7 * G::STAGE + yo;        //   a-branch z term of plane p-2 (for plane p-1)
+    T* const pkxb = Ust + 8 * G::STAGE + yo;       //   second branch factors (limiters other than minmod)
+    T* const pkyb = Ust + 9 * G::STAGE + yo;
+    T* const pkzb = Ust + 10 * G::STAGE + yo;
     P2<T> Wprev[5], dprev[5], Lz[5], gpp[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) {
       Wprev[f] = dprev[f] = Lz[f] = gpp[f] = bc2(T(0));
-      rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); rsts2(pkz + f * FS, bc2(T(0)));
+      rsts2(pk1 + f * FS, bc2(T(0))); rsts2(pk2 + f * FS, bc2(T(0))); rsts2(pkz + f * FS, bc2(T(0))); rsts2(pkzb + f * FS, bc2(T(0)));
       rsts2(pkw + f * FS, bc2(T(0))); rsts2(pkc + f * FS, bc2(T(0)));
     }
     size_t op = (size_t)pz * NP + o;
@@ -343,12 +381,12 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
       // ---- z: slope of plane p-1, adjoint of the face between p-2 and p-1, which completes the z terms of plane p-2
       {
         P2<T> Rz[5], lam[5], Lb[5], Rb[5];
-        P2<T> kz[5];
+        P2<T> az[5], bz[5];                          // the differences of plane p-1's slopes, for its branch factors
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
           const P2<T> a = sub2(Wn[f], Wprev[f]);
-          const P2<T> s = limit2<T, 0>(a, dprev[f]);
-          kz[f] = kfac2(a, dprev[f]);
+          const P2<T> s = limit2<T, LIM>(a, dprev[f]);
+          az[f] = a; bz[f] = dprev[f];
           Rz[f] = fma2(nhalf, s, Wprev[f]);
           Wn[f] = fma2(half, s, Wprev[f]);           // left state of the NEXT z face
           dprev[f] = a;
@@ -361,9 +399,15 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         for (int f = 0; f < 5; ++f) {
           Lz[f] = Wn[f];
           P2<T> wp, Pz, Mz;
-          cell_terms_pm2(Lb[f], rlds2(pk1 + f * FS), rlds2(pkz + f * FS), wp, Pz, Mz);   // cell of plane p-2: parked Rb and factor
+          if (LIM == 0) {
+            cell_terms_pm2(Lb[f], rlds2(pk1 + f * FS), rlds2(pkz + f * FS), wp, Pz, Mz);   // cell of plane p-2: parked Rb and factor
+          } else {
+            P2<T> ha, hb;
+            fetch_h<T, LIM>(pkz + f * FS, pkzb + f * FS, ha, hb);
+            cell_terms_h2(Lb[f], rlds2(pk1 + f * FS), ha, hb, wp, Pz, Mz);
+          }
           rsts2(pk1 + f * FS, Rb[f]);
-          rsts2(pkz + f * FS, kz[f]);
+          park_h<T, LIM>(pkz + f * FS, pkzb + f * FS, az[f], bz[f]);
           const P2<T> Pprev = rlds2(pkc + f * FS);                                // a-branch term of plane p-3 for plane p-2
           const P2<T> fin = sub2(rlds2(pkw + f * FS), Mz);                        // plane p-3 is complete (but for y)
           rsts2(pkw + f * FS, add2(add2(wp, rlds2(pk2 + f * FS)), Pprev));
@@ -393,11 +437,11 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
             const P2<T> W = Wprev[f];
             const T wr = row[2], wr2 = row[3];
             const T d0 = W.x - row[-1], d1 = W.y - W.x, d2 = wr - W.y;
-            const P2<T> s = {minmod_(d1, d0), minmod_(d2, d1)};
-            rsts2(pkx + f * FS, P2<T>{kfac(d1, d0), kfac(d2, d1)});
+            const P2<T> s = {limit1<T, LIM>(d1, d0), limit1<T, LIM>(d2, d1)};
+            park_h<T, LIM>(pkx + f * FS, pkxb + f * FS, P2<T>{d1, d2}, P2<T>{d0, d1});
             Lf[f] = fma2(half, s, W);
             const T Rown = fma_(T(-0.5), s.y, W.y);                         // R state of the second own cell
-            const T Rnext = fma_(T(-0.5), minmod_(wr2 - wr, d2), wr);       // R state of the cell right of the pack
+            const T Rnext = fma_(T(-0.5), limit1<T, LIM>(wr2 - wr, d2), wr);   // R state of the cell right of the pack
             Rf[f] = {Rown, Rnext};
             const T gr = Gq_s[f * FP + so + 2];
             lam[f] = mul2(cx, P2<T>{gq[f].y - gq[f].x, gr - gq[f].y});
@@ -408,10 +452,10 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
             const T* row = Wq_s + f * FP + so;
             const P2<T> W = Wprev[f], Wu = rlds2(row + RSW), Wu2 = rlds2(row + 2 * RSW);
             const P2<T> a = sub2(Wu, W), b = sub2(W, rlds2(row - RSW));
-            const P2<T> s = limit2<T, 0>(a, b);
-            rsts2(pky + f * FS, kfac2(a, b));
+            const P2<T> s = limit2<T, LIM>(a, b);
+            park_h<T, LIM>(pky + f * FS, pkyb + f * FS, a, b);
             Lf[PY[f]] = fma2(half, s, W);
-            Rf[PY[f]] = fma2(nhalf, limit2<T, 0>(sub2(Wu2, Wu), a), Wu);    // R state of the row above
+            Rf[PY[f]] = fma2(nhalf, limit2<T, LIM>(sub2(Wu2, Wu), a), Wu);  // R state of the row above
             lam[PY[f]] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
           }
         }
@@ -438,20 +482,34 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         const long long oe = (((long long)p.sp0 + zrel0 + it - 4) * ny + wrapr(y0 + r, ny)) * (long long)(2 * p.ntx) + 2 * blockIdx.x;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
-          P2<T> wx, Px, Mx, wy, cey;
-          const P2<T> kx = rlds2(pkx + f * FS);
-          cell_terms_pm2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, kx, wx, Px, Mx);
-          cell_terms2(Lby[f], rlds2(By_s + f * YF + yo), rlds2(pky + f * FS), wy, cey);
+          P2<T> wx, Px, Mx, wy, Py, My, cey;
+          if (LIM == 0) {                                  // one factor k per slope; the y term leaves as one encoded word
+            const P2<T> kx = rlds2(pkx + f * FS);
+            cell_terms_pm2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, kx, wx, Px, Mx);
+            cell_terms2(Lby[f], rlds2(By_s + f * YF + yo), rlds2(pky + f * FS), wy, cey);
+            Py = {enc_sign(Px.x + Mx.x, kx.x), enc_sign(Px.y + Mx.y, kx.y)};    // (reused below as the encoded c^x of the pack)
+          } else {
+            P2<T> hxa, hxb, hya, hyb;
+            fetch_h<T, LIM>(pkx + f * FS, pkxb + f * FS, hxa, hxb);
+            fetch_h<T, LIM>(pky + f * FS, pkyb + f * FS, hya, hyb);
+            cell_terms_h2(Lbx[f], P2<T>{Bx_s[f * XF + xo], RbxA[f]}, hxa, hxb, wx, Px, Mx);
+            cell_terms_h2(Lby[f], rlds2(By_s + f * YF + yo), hya, hyb, wy, Py, My);
+          }
           T pl = shfl_up1(Px.y), mr = shfl_dn1(Mx.x);
           if (lane == 0) pl = T(0);
           if (lane == 31) mr = T(0);
           wx.x += pl - Mx.y;
           wx.y += Px.x - mr;
-          const P2<T> cex = {enc_sign(Px.x + Mx.x, kx.x), enc_sign(Px.y + Mx.y, kx.y)};   // for the tile-edge array only
           rsts2(pk2 + f * FS, add2(wx, wy));
-          if (sty) rstg2(p.C + f * SPN + os1, cey);
-          if (edge_l) p.Ce[f * p.SPE + oe] = cex.x;
-          if (edge_r) p.Ce[f * p.SPE + oe + 1] = cex.y;
+          if (LIM == 0) {                                   // one of P, M is zero: one word with the branch flag in its LSB
+            if (sty) rstg2(p.C + f * SPN + os1, cey);
+            if (edge_l) p.Ce[f * p.SPE + oe] = Py.x;
+            if (edge_r) p.Ce[f * p.SPE + oe + 1] = Py.y;
+          } else {                                          // both branches contribute: P and M travel separately
+            if (sty) { rstg2(p.C + f * SPN + os1, Py); rstg2(p.C + (5 + f) * SPN + os1, My); }
+            if (edge_l) p.Ce[f * p.SPE + oe] = Mx.x;        // what the last cell of the tile on the left loses
+            if (edge_r) p.Ce[f * p.SPE + oe + 1] = Px.y;    // what the first cell of the tile on the right receives
+          }
         }
       }
       // plane p becomes plane p-1
@@ -513,8 +571,8 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           const T* col = Wq_s + f * FP + 2 * lane + 2;
           const P2<T> Wm2 = rlds2(col), Wm1 = rlds2(col + RSW), W0 = rlds2(col + 2 * RSW), W1 = rlds2(col + 3 * RSW);
           const P2<T> d0 = sub2(W0, Wm1);
-          Lf[f] = fma2(half, limit2<T, 0>(d0, sub2(Wm1, Wm2)), Wm1);
-          Rf[f] = fma2(nhalf, limit2<T, 0>(sub2(W1, W0), d0), W0);
+          Lf[f] = fma2(half, limit2<T, LIM>(d0, sub2(Wm1, Wm2)), Wm1);
+          Rf[f] = fma2(nhalf, limit2<T, LIM>(sub2(W1, W0), d0), W0);
           const T* gc = Gq_s + f * FP + 2 * lane + 2;
           lam[f] = mul2(cy, sub2(rlds2(gc + 2 * RSW), rlds2(gc + RSW)));
         }
@@ -525,8 +583,8 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
         for (int f = 0; f < 5; ++f) {
           const T* rw = Wq_s + f * FP + (rl + 2) * RSW;
           const T dc = rw[2] - rw[1];
-          Lf[f] = bc2(fma_(T(0.5), minmod_(dc, rw[1] - rw[0]), rw[1]));
-          Rf[f] = bc2(fma_(T(-0.5), minmod_(rw[3] - rw[2], dc), rw[2]));
+          Lf[f] = bc2(fma_(T(0.5), limit1<T, LIM>(dc, rw[1] - rw[0]), rw[1]));
+          Rf[f] = bc2(fma_(T(-0.5), limit1<T, LIM>(rw[3] - rw[2], dc), rw[2]));
           const T* gr = Gq_s + f * FP + (rl + 2) * RSW;
           lam[f] = bc2(p.coef[0] * (gr[2] - gr[1]));
         }
@@ -560,7 +618,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 // ------------------------------------------------------------------------------------------------ kernel B
 // One thread per pack (two x-adjacent cells) of a slab plane: adds the y neighbour terms (rows j -+ 1 of C) and, for the
 // packs at a tile edge, the x term that crossed it (Ce), then Ub = prim_vjp(U, Wb) + b1 + b2.
-template <class T>
+template <class T, int LIM>
 __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T> p) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;       // pack index along x
   const int i = 2 * ip, j = blockIdx.y, kz = blockIdx.z;      // kz: plane relative to p.z0
@@ -578,12 +636,20 @@ __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T
 #pragma unroll
   for (int f = 0; f < 5; ++f) {
     P2<T> w = rldg2(p.Wp + f * SPN + sp + row + i);
-    const T* Cy = p.C + f * SPN + sp + i;
-    const P2<T> cd = rldg2(Cy + rowm), cu = rldg2(Cy + rowp);
-    w.x += pterm(cd.x) - mterm(cu.x);
-    w.y += pterm(cd.y) - mterm(cu.y);
-    if (el) w.x += pterm(p.Ce[f * p.SPE + oe + 2 * tl + 1]);
-    if (er) w.y -= mterm(p.Ce[f * p.SPE + oe + 2 * tr]);
+    if (LIM == 0) {                                           // encoded c: the flag says which neighbour it belongs to
+      const T* Cy = p.C + f * SPN + sp + i;
+      const P2<T> cd = rldg2(Cy + rowm), cu = rldg2(Cy + rowp);
+      w.x += pterm(cd.x) - mterm(cu.x);
+      w.y += pterm(cd.y) - mterm(cu.y);
+      if (el) w.x += pterm(p.Ce[f * p.SPE + oe + 2 * tl + 1]);
+      if (er) w.y -= mterm(p.Ce[f * p.SPE + oe + 2 * tr]);
+    } else {                                                  // P of the row below, M of the row above
+      const P2<T> pd = rldg2(p.C + f * SPN + sp + i + rowm), mu = rldg2(p.C + (5 + f) * SPN + sp + i + rowp);
+      w.x += pd.x - mu.x;
+      w.y += pd.y - mu.y;
+      if (el) w.x += p.Ce[f * p.SPE + oe + 2 * tl + 1];
+      if (er) w.y -= p.Ce[f * p.SPE + oe + 2 * tr];
+    }
     Wb[f] = w;
   }
   P2<T> U[5];
@@ -606,16 +672,20 @@ __global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
-template <class T>
-cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
-  constexpr int NW = sizeof(T) == 4 ? 8 : 5;      // fp64 (parity only): 4 row warps so that shared memory fits
+// words of scratch per cell of a slab: Wp 5 + c^y 5 (minmod: one encoded word; van Leer / MC: P and M separately, 10)
+int rev_scratch_words(int limiter) { return limiter == 0 ? 10 : 15; }
+
+namespace {
+template <class T, int LIM>
+cudaError_t launch_rev_faces_l(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
+  constexpr int NW = sizeof(T) == 4 ? 8 : 4;      // fp64 (parity only): 3 row warps so that shared memory fits
   using G = GeoR<NW>;
   const size_t smem = (size_t)G::TOTAL * sizeof(T);
   static bool configured[64] = {};    // per device: the attribute belongs to the (function, device) pair
   int cur_dev = 0;
   cudaGetDevice(&cur_dev);
   if (cur_dev < 0 || cur_dev >= 64 || !configured[cur_dev]) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
@@ -632,20 +702,31 @@ cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int sm_count, cudaStream
   }
   const int ZL = (p.nout + bz - 1) / bz;
   dim3 grid(bx, by, bz), block(NW * 32);
-  rev_faces_kernel<T, NW><<<grid, block, smem, s>>>(p, ZL);
+  rev_faces_kernel<T, NW, LIM><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
+}
+}  // namespace
+
+template <class T>
+cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int sm_count, cudaStream_t s) {
+  switch (limiter) {
+    case 1: return launch_rev_faces_l<T, 1>(p, sm_count, s);
+    case 2: return launch_rev_faces_l<T, 2>(p, sm_count, s);
+    default: return launch_rev_faces_l<T, 0>(p, sm_count, s);
+  }
 }
 
 template <class T>
-cudaError_t launch_rev_gather(const RevGatherParams<T>& p, cudaStream_t s) {
+cudaError_t launch_rev_gather(const RevGatherParams<T>& p, int limiter, cudaStream_t s) {
   dim3 block(128), grid((p.nx / 2 + 127) / 128, p.ny, p.nplanes);
-  rev_gather_kernel<T><<<grid, block, 0, s>>>(p);
+  if (limiter == 0) rev_gather_kernel<T, 0><<<grid, block, 0, s>>>(p);
+  else rev_gather_kernel<T, 1><<<grid, block, 0, s>>>(p);
   return cudaGetLastError();
 }
 
-template cudaError_t launch_rev_faces<float>(const RevFaceParams<float>&, int, cudaStream_t);
-template cudaError_t launch_rev_faces<double>(const RevFaceParams<double>&, int, cudaStream_t);
-template cudaError_t launch_rev_gather<float>(const RevGatherParams<float>&, cudaStream_t);
-template cudaError_t launch_rev_gather<double>(const RevGatherParams<double>&, cudaStream_t);
+template cudaError_t launch_rev_faces<float>(const RevFaceParams<float>&, int, int, cudaStream_t);
+template cudaError_t launch_rev_faces<double>(const RevFaceParams<double>&, int, int, cudaStream_t);
+template cudaError_t launch_rev_gather<float>(const RevGatherParams<float>&, int, cudaStream_t);
+template cudaError_t launch_rev_gather<double>(const RevGatherParams<double>&, int, cudaStream_t);
 
 }  // namespace dh

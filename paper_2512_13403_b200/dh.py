@@ -36,6 +36,7 @@ SYMBOLS = [
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
     "dh_cfl_stats", "dh_cool_tmin", "dh_set_cooling_table", "dh_cool_table_vjp",
+    "dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp",
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
     "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
@@ -90,6 +91,12 @@ def load(rebuild: bool = False):
     lib.dh_set_cooling_table.restype = ci
     lib.dh_cool_table_vjp.argtypes = [vp, vp, cd, vp, pd]
     lib.dh_cool_table_vjp.restype = ci
+    lib.dh_gravity_source.argtypes = [vp, vp, vp, cd]
+    lib.dh_gravity_source_vjp.argtypes = [vp, vp, vp, cd, vp, vp, vp]
+    lib.dh_step_gravity.argtypes = [vp, vp, vp, cd, cd, ci]
+    lib.dh_step_gravity_vjp.argtypes = [vp, vp, vp, cd, cd, ci, vp, vp]
+    for fn in ("dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp"):
+        getattr(lib, fn).restype = ci
     lib.dh_last_error.restype = ctypes.c_char_p
     lib.dh_version.restype = ctypes.c_char_p
     for fn in ("dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_cfl_dt_async", "dh_poll_status",
@@ -341,6 +348,29 @@ class Solver:
 
     def cool_table_vjp(self, U, dt: float, g_out) -> list:
         return dh_cool_table_vjp(self.ctx, self._dev(U, "U"), dt, self._dev(g_out, "g_out"), self._ntab)
+
+    def _field(self, t: torch.Tensor, name: str) -> int:
+        if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and t.dtype == self.dtype and tuple(t.shape) == self.shape[1:]):
+            raise ValueError(f"{name} must be a contiguous CUDA tensor of shape {self.shape[1:]} and dtype {self.dtype}")
+        return t.data_ptr()
+
+    def gravity_source(self, U, phi, dt: float) -> None:
+        _check(load().dh_gravity_source(self.ctx, self._dev(U, "U"), self._field(phi, "phi"), float(dt)))
+
+    def gravity_source_vjp(self, U, phi, dt: float, g_out):
+        g_in, g_phi = torch.empty_like(U), torch.empty_like(phi)
+        _check(load().dh_gravity_source_vjp(self.ctx, self._dev(U, "U"), self._field(phi, "phi"), float(dt), self._dev(g_out, "g_out"),
+                                            self._dev(g_in, "g_in"), self._field(g_phi, "g_phi")))
+        return g_in, g_phi
+
+    def step_gravity(self, mg, U, dt: float, four_pi_g: float, ncycles: int = 12) -> None:
+        _check(load().dh_step_gravity(self.ctx, mg.ctx, self._dev(U, "U"), float(dt), float(four_pi_g), int(ncycles)))
+
+    def step_gravity_vjp(self, mg, U, dt: float, four_pi_g: float, g_out, ncycles: int = 12):
+        g_in = torch.empty_like(U)
+        _check(load().dh_step_gravity_vjp(self.ctx, mg.ctx, self._dev(U, "U"), float(dt), float(four_pi_g), int(ncycles),
+                                          self._dev(g_out, "g_out"), self._dev(g_in, "g_in")))
+        return g_in
 
     def run_host(self, U_host, nsteps: int) -> float:
         return dh_run_host(self.ctx, self._host(U_host, "U_host"), nsteps)

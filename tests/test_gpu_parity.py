@@ -219,8 +219,9 @@ def _vjp_case(U, gamma, seed, dtype, okw, skw, max_excluded=0.25):
         assert err <= 1e-12, err
         return err
     cond = vjp_margins.vjp_condition(U.numpy(), dt, p)
+    sens = vjp_margins.vjp_sensitivity(U.numpy(), dt, p)           # van Leer only: conditioning of the limiter's derivative
     label = f"{tuple(U.shape[1:])} {okw}"
-    return vjp_margins.check_vjp(gin.cpu().numpy(), ref, cond, TOL[dtype], max_excluded=max_excluded, label=label)[0]
+    return vjp_margins.check_vjp(gin.cpu().numpy(), ref, cond, TOL[dtype], max_excluded=max_excluded, label=label, sens=sens)[0]
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
@@ -237,10 +238,16 @@ def test_vjp_parity_with_cooling(dtype):
     _vjp_case(U, 5 / 3, 6, dtype, kw, dict(cooling=1, lambda0=0.5))
 
 
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("limiter", ["vanleer", "mc"])
-def test_vjp_parity_other_limiters(limiter):
-    U = random_state((8, 10, 12), 19, 1.4, torch.float64)
-    _vjp_case(U, 1.4, 7, torch.float64, dict(limiter=limiter), dict(limiter=limiter))
+def test_vjp_parity_other_limiters(limiter, dtype, kernel):
+    """van Leer (the paper's fiducial limiter) and MC through the fused reverse pair (two branch factors per
+    slope, P and M terms stored separately) and through the gather kernels; several ragged tiles, cooling on in one case."""
+    U = random_state((13, 17, 132), 19, 1.4, dtype)
+    _vjp_case(U, 1.4, 7, dtype, dict(limiter=limiter), dict(limiter=limiter, kernel=kernel))
+    V = random_state((8, 10, 12), 20, 5 / 3, dtype)
+    _vjp_case(V, 5 / 3, 8, dtype, dict(limiter=limiter, cooling=True, lambda0=0.5), dict(limiter=limiter, kernel=kernel, cooling=1, lambda0=0.5))
 
 
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])

@@ -53,6 +53,45 @@ def stage_condition(X, p):
     return c
 
 
+def _line_max(m, a, r=2):
+    ax = m.ndim - 1 - a
+    out = m.copy()
+    for s in range(1, r + 1):
+        np.maximum(out, np.roll(m, s, axis=ax), out=out)
+        np.maximum(out, np.roll(m, -s, axis=ax), out=out)
+    return out
+
+
+def plus_max(c):
+    out = _line_max(c, 0)
+    for a in (1, 2):
+        np.maximum(out, _line_max(c, a), out=out)
+    return out
+
+
+def vjp_sensitivity(U, dt, p):
+    """[nz, ny, nx]: the largest limiter conditioning number (oracle.limiter_conditioning) over the slopes a cell's step-VJP entries
+    depend on (same stencil chain as vjp_condition).  Zero unless the limiter is van Leer, whose derivative 2 b^2 / (a + b)^2 is
+    smooth but moves by ~ 12 eps s / (|a| + |b|) when the differences are rounded to eps s; check_vjp widens the tolerance of an
+    entry by SENS_ULPS x 2^-24 x this number."""
+    if p.limiter != 1:
+        return None
+    states, _ = stage_states(U, dt, p)
+    sens = None
+    for X in reversed(states):
+        C = oracle.limiter_conditioning(X, p)
+        c = np.zeros(C.shape[1:])
+        for a in range(3):
+            np.maximum(c, _line_max(C[a], a), out=c)
+        if sens is not None:
+            np.maximum(c, plus_max(sens), out=c)
+        sens = c
+    return sens
+
+
+SENS_ULPS = 2.0
+
+
 def stage_states(U, dt, p):
     """The states at which D() is evaluated, in forward order, and the pre-cooling result (oracle step(), Eqs. A6-A7 /
     reading A18), assembled from oracle.flux_divergence."""
@@ -94,7 +133,7 @@ def gradient_scales(ref):
     return np.array([rms(ref[0]), sm, sm, sm, rms(ref[4])]).reshape(5, 1, 1, 1)
 
 
-def check_vjp(got, ref, cond, tol, bound=FP32_BOUND, max_excluded=1.0, scales=None, label=""):
+def check_vjp(got, ref, cond, tol, bound=FP32_BOUND, max_excluded=1.0, scales=None, label="", sens=None):
     """Every entry whose stencil margin is >= bound within `tol` (per-cell relative error, A15 normalisation); the
     others (either one-sided derivative is valid there) finite and of the gradient's magnitude.  Returns (worst
     well-conditioned error, excluded fraction)."""
@@ -102,6 +141,8 @@ def check_vjp(got, ref, cond, tol, bound=FP32_BOUND, max_excluded=1.0, scales=No
     ref = np.asarray(ref, dtype=np.float64)
     s = gradient_scales(ref) if scales is None else scales
     e = np.abs(got - ref) / np.maximum(np.abs(ref), s)
+    if sens is not None:                                 # van Leer: per-entry tolerance tol + SENS_ULPS 2^-24 sens; e is rescaled to `tol`
+        e = e * (tol / (tol + SENS_ULPS * 2.0 ** -24 * np.minimum(sens, 1e6)))
     well = np.broadcast_to(cond >= bound, e.shape)
     excluded = 1.0 - float(well[0].mean())
     worst = float(e[well].max()) if well.any() else 0.0
