@@ -619,7 +619,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 // One thread per pack (two x-adjacent cells) of a slab plane: adds the y neighbour terms (rows j -+ 1 of C) and, for the
 // packs at a tile edge, the x term that crossed it (Ce), then Ub = prim_vjp(U, Wb) + b1 + b2.
 template <class T, int LIM>
-__global__ void __launch_bounds__(128) rev_gather_kernel(const RevGatherParams<T> p) {
+__global__ void __launch_bounds__(128, 16) rev_gather_kernel(const RevGatherParams<T> p) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;       // pack index along x
   const int i = 2 * ip, j = blockIdx.y, kz = blockIdx.z;      // kz: plane relative to p.z0
   if (i >= p.nx) return;
