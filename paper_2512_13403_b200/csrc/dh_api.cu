@@ -507,7 +507,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
   for (int z0 = 0; z0 < c->nz; z0 += c->rev_slab) {
     const int nplanes = (c->nz - z0 < c->rev_slab) ? c->nz - z0 : c->rev_slab;
     a.zs = z0; a.nout = nplanes;
-    DH_CUDA(launch_rev_faces<T>(a, c->limiter, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
+    DH_CUDA(launch_rev_faces<T>(a, c->limiter, c->riemann, c->sm_count, c->stream), "dh_step_vjp: face-adjoint kernel launch");
     b.z0 = z0; b.nplanes = nplanes;
     DH_CUDA(launch_rev_gather<T>(b, c->limiter, c->stream), "dh_step_vjp: gather kernel launch");
     c->launches += 2;
@@ -517,8 +517,8 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
 
 template <class T>
 static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
-  // the fused pair handles HLLC (any limiter) on even nx; everything else takes the one-thread-per-cell gather kernel
-  if (c->kernel == 0 && c->riemann == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
+  // the fused pair handles every limiter and Riemann flux on even nx; odd nx and DH_OPT_KERNEL = 1 take the one-thread-per-cell gather kernel
+  if (c->kernel == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
   return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
 }
 

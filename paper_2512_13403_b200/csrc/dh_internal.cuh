@@ -185,7 +185,7 @@ template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int l
 template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s, bool* supported);
 template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);
-template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int sm_count, cudaStream_t s);
+template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s);
 int rev_scratch_words(int limiter);
 template <class T> cudaError_t launch_rev_gather(const RevGatherParams<T>& p, int limiter, cudaStream_t s);
 template <class T> cudaError_t launch_cool_fwd(T* U, size_t N, T dt, const T* dt_dev, const Consts<T>& c, cudaStream_t s);

@@ -121,6 +121,25 @@ DH_DI void hllc_vjp2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, con
   }
 }
 
+// the same for any Riemann flux (RS: 0 HLLC, 1 HLL, 2 Rusanov): riemann_flux_vjp() of dh_math.cuh on each half
+template <class T, int AX, int RS>
+DH_DI void riemann_vjp2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, const P2<T> Fb[5], P2<T> Lb[5], P2<T> Rb[5]) {
+#pragma unroll 1
+  for (int h = 0; h < 2; ++h) {
+    T l[5], r[5], fb[5], lb[5], rb[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      l[f] = h ? L[f].y : L[f].x; r[f] = h ? R[f].y : R[f].x; fb[f] = h ? Fb[f].y : Fb[f].x;
+      lb[f] = T(0); rb[f] = T(0);
+    }
+    riemann_flux_vjp<T, AX, RS>(l, r, c, fb, lb, rb);
+#pragma unroll
+    for (int f = 0; f < 5; ++f) {
+      if (h) { Lb[f].y = lb[f]; Rb[f].y = rb[f]; } else { Lb[f].x = lb[f]; Rb[f].x = rb[f]; }
+    }
+  }
+}
+
 template <class T> DH_DI P2<T> neg2(P2<T> a) { return {-a.x, -a.y}; }
 template <class T> DH_DI P2<T> zsel2(B2 m, P2<T> a) { return {m.x ? a.x : T(0), m.y ? a.y : T(0)}; }
 
@@ -291,7 +310,7 @@ DH_DI double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
 //          helper supplies the two cells beside the tile), its own y terms are added, its c^y goes to the scratch
 //   p-2    the z face above it is adjoined: its own z terms and the a-branch term of plane p-3 join the parked sum
 //   p-3    receives the b-branch term of plane p-2 and is stored: Wp' = everything except the y neighbour terms
-template <class T, int NW, int LIM>
+template <class T, int NW, int LIM, int RS>
 __global__ void __launch_bounds__(NW * 32, 1)
 rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
   using G = GeoR<NW>;
@@ -393,7 +412,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           lam[f] = mul2(cz, sub2(gq[f], gpp[f]));
           gpp[f] = gq[f];
         }
-        hllc_vjp2p<T, 2>(Lz, Rz, c, lam, Lb, Rb);
+        if (RS == 0) hllc_vjp2p<T, 2>(Lz, Rz, c, lam, Lb, Rb); else riemann_vjp2<T, 2, RS>(Lz, Rz, c, lam, Lb, Rb);
         const bool stz = (it >= 6) && store_ok;
 #pragma unroll
         for (int f = 0; f < 5; ++f) {
@@ -459,7 +478,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
             lam[PY[f]] = mul2(cy, sub2(rlds2(Gq_s + f * FP + so + RSW), gq[f]));
           }
         }
-        hllc_vjp2p<T, 0>(Lf, Rf, c, lam, Lb, Rb);
+        if (RS == 0) hllc_vjp2p<T, 0>(Lf, Rf, c, lam, Lb, Rb); else riemann_vjp2<T, 0, RS>(Lf, Rf, c, lam, Lb, Rb);
         if (ax == 0) {
 #pragma unroll
           for (int f = 0; f < 5; ++f) { Lbx[f] = Lb[f]; RbxA[f] = Rb[f].x; Bx_s[f * XF + xo + 1] = Rb[f].y; }
@@ -576,7 +595,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           const T* gc = Gq_s + f * FP + 2 * lane + 2;
           lam[f] = mul2(cy, sub2(rlds2(gc + 2 * RSW), rlds2(gc + RSW)));
         }
-        hllc_vjp2<T, 1>(Lf, Rf, c, lam, Lb, Rb);   // bottom y face of the tile
+        riemann_vjp2<T, 1, RS>(Lf, Rf, c, lam, Lb, Rb);   // bottom y face of the tile
 #pragma unroll
         for (int f = 0; f < 5; ++f) rsts2(By_s + f * YF + 2 * lane, Rb[f]);
 #pragma unroll
@@ -588,7 +607,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
           const T* gr = Gq_s + f * FP + (rl + 2) * RSW;
           lam[f] = bc2(p.coef[0] * (gr[2] - gr[1]));
         }
-        hllc_vjp2<T, 0>(Lf, Rf, c, lam, Lb, Rb);   // left x face of the tile, row rl
+        riemann_vjp2<T, 0, RS>(Lf, Rf, c, lam, Lb, Rb);   // left x face of the tile, row rl
         if (lane < TY) {
 #pragma unroll
           for (int f = 0; f < 5; ++f) Bx_s[f * XF + rl * RXP] = Rb[f].x;
@@ -676,7 +695,7 @@ __global__ void __launch_bounds__(128, 16) rev_gather_kernel(const RevGatherPara
 int rev_scratch_words(int limiter) { return limiter == 0 ? 10 : 15; }
 
 namespace {
-template <class T, int LIM>
+template <class T, int LIM, int RS>
 cudaError_t launch_rev_faces_l(const RevFaceParams<T>& p, int sm_count, cudaStream_t s) {
   constexpr int NW = sizeof(T) == 4 ? 8 : 4;      // fp64 (parity only): 3 row warps so that shared memory fits
   using G = GeoR<NW>;
@@ -685,7 +704,7 @@ cudaError_t launch_rev_faces_l(const RevFaceParams<T>& p, int sm_count, cudaStre
   int cur_dev = 0;
   cudaGetDevice(&cur_dev);
   if (cur_dev < 0 || cur_dev >= 64 || !configured[cur_dev]) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW, LIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute((const void*)rev_faces_kernel<T, NW, LIM, RS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
@@ -702,17 +721,23 @@ cudaError_t launch_rev_faces_l(const RevFaceParams<T>& p, int sm_count, cudaStre
   }
   const int ZL = (p.nout + bz - 1) / bz;
   dim3 grid(bx, by, bz), block(NW * 32);
-  rev_faces_kernel<T, NW, LIM><<<grid, block, smem, s>>>(p, ZL);
+  rev_faces_kernel<T, NW, LIM, RS><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
 }
 }  // namespace
 
 template <class T>
-cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int sm_count, cudaStream_t s) {
-  switch (limiter) {
-    case 1: return launch_rev_faces_l<T, 1>(p, sm_count, s);
-    case 2: return launch_rev_faces_l<T, 2>(p, sm_count, s);
-    default: return launch_rev_faces_l<T, 0>(p, sm_count, s);
+cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s) {
+  switch (limiter * 3 + riemann) {
+    case 1: return launch_rev_faces_l<T, 0, 1>(p, sm_count, s);
+    case 2: return launch_rev_faces_l<T, 0, 2>(p, sm_count, s);
+    case 3: return launch_rev_faces_l<T, 1, 0>(p, sm_count, s);
+    case 4: return launch_rev_faces_l<T, 1, 1>(p, sm_count, s);
+    case 5: return launch_rev_faces_l<T, 1, 2>(p, sm_count, s);
+    case 6: return launch_rev_faces_l<T, 2, 0>(p, sm_count, s);
+    case 7: return launch_rev_faces_l<T, 2, 1>(p, sm_count, s);
+    case 8: return launch_rev_faces_l<T, 2, 2>(p, sm_count, s);
+    default: return launch_rev_faces_l<T, 0, 0>(p, sm_count, s);
   }
 }
 
@@ -724,8 +749,8 @@ cudaError_t launch_rev_gather(const RevGatherParams<T>& p, int limiter, cudaStre
   return cudaGetLastError();
 }
 
-template cudaError_t launch_rev_faces<float>(const RevFaceParams<float>&, int, int, cudaStream_t);
-template cudaError_t launch_rev_faces<double>(const RevFaceParams<double>&, int, int, cudaStream_t);
+template cudaError_t launch_rev_faces<float>(const RevFaceParams<float>&, int, int, int, cudaStream_t);
+template cudaError_t launch_rev_faces<double>(const RevFaceParams<double>&, int, int, int, cudaStream_t);
 template cudaError_t launch_rev_gather<float>(const RevGatherParams<float>&, int, cudaStream_t);
 template cudaError_t launch_rev_gather<double>(const RevGatherParams<double>&, int, cudaStream_t);
 
