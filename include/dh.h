@@ -68,8 +68,9 @@ enum {
   DH_OPT_KERNEL = 10,    /* 0 (default): fused z-sweep stage kernel, 2x2 cells per thread; 1: one-thread-per-cell gather
                             kernels (same arithmetic, kept for cross-checking and as the fallback for odd nx) */
   DH_OPT_LIMITER = 11,   /* 0 minmod (default), 1 van Leer, 2 MC */
-  DH_OPT_REV_SLAB = 12,  /* planes per z slab of the fused reverse stages' scratch (20 words per cell of a slab);
-                            0 (default): as many as fit in min(32 GiB, half of the free device memory) */
+  DH_OPT_REV_SLAB = 12,  /* planes per z slab of the fused reverse stages' scratch (10 words per cell of a slab, 15 with the
+                            van Leer / MC limiters, plus a thin array of tile-edge terms);
+                            0 (default): as many as fit in min(48 GiB, 70 % of the free device memory) */
   DH_OPT_INTEGRATOR = 13,/* 0 (default): the predictor / corrector of Eqs. A6-A7;
                             1: Heun's RK2  U1 = U - dt D(U);  U' = 1/2 U + 1/2 (U1 - dt D(U1));
                             2: SSPRK3  U1 = U - dt D(U);  U2 = 3/4 U + 1/4 (U1 - dt D(U1));
