@@ -108,6 +108,7 @@ enum {
   DH_OPT_LAMBDA2 = 24,   /* >= 0, default 0 */
   DH_OPT_ALPHA2 = 25,    /* default 0.5 */
   DH_OPT_GAMMA0 = 26,    /* Gamma_0 of PAPER.md:286, 294, >= 0, default 0 */
+  DH_OPT_STREAM_SLAB = 28, /* planes per z slab of dh_stream_host's copies, integer >= 0; 0 (default): nz / 32, at least 8 */
   DH_OPT_COOL_FSUB = 27, /* DH_OPT_COOL_MODE = 2 (the masked per-cell choice of PAPER.md:342): a cell takes the sub-cycled update
                             of Eq. 23 (DH_OPT_COOL_NSUB substeps) when dt |Edot(T^n)| > f_sub |E_th^n|, else the trapezoid of
                             Eq. 22 (reading A26); > 0, default 0.1 */
@@ -199,6 +200,19 @@ int dh_adjoint(dh_ctx* ctx, void* U, void* gU, int nsteps, int every, double* dt
  * `nsteps` x (CFL dt + step) with the device-resident dt, copies the result back and synchronises.
  * dt_last_out (HOST, may be NULL) receives the last dt. */
 int dh_run_host(dh_ctx* ctx, void* U_host, int nsteps, double* dt_last_out);
+
+/* A state that LIVES in host memory: `nsteps` x (CFL dt + step), every step reading its input from U_host and writing its
+ * result back there (the host sees every intermediate state; 2 x state bytes cross the link per step).  Same steps as
+ * dh_advance (Eqs. A4-A8): U_host ends bit-identical to dh_run_host called nsteps times with one step each.
+ *   U_host: HOST, in/out, same layout; pinned memory (cudaHostAlloc / cudaHostRegister) is what makes the copies
+ *           asynchronous.  It must not be written by the caller during the call.
+ * The state moves in z slabs of DH_OPT_STREAM_SLAB planes on two copy streams the context owns, one per link direction:
+ * the write-back of step n, slab k is followed by the read of step n+1, slab k, the predictor of a step runs over the planes
+ * whose neighbours have arrived, the corrector slab by slab ahead of its write-back; dt of step n+1 comes from the device copy
+ * of step n's result.  In the steady state both directions are busy and a step costs max(H2D, D2H) instead of their sum plus the
+ * kernels.  The library holds two device states.  Heun / SSPRK3, the cooling integrators that run as a pass of their own and
+ * DH_OPT_KERNEL = 1 compute whole steps between the slab-wise copies.  Synchronises; dt_last_out as in dh_run_host. */
+int dh_stream_host(dh_ctx* ctx, void* U_host, int nsteps, double* dt_last_out);
 
 /* HOST-buffer VJP: copies U and gU_out in, runs dh_step_vjp, copies gU_in out, synchronises. */
 int dh_step_vjp_host(dh_ctx* ctx, const void* U_host, double dt, const void* gU_out_host, void* gU_in_host);

@@ -175,11 +175,15 @@ dh_ctx* dh_create(int nx, int ny, int nz, double gamma, int dtype) {
 
 void dh_destroy(dh_ctx* c) {
   if (!c) return;
-  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev, c->tab_dev, c->tab_dev_d, c->tab_part, c->grav_phi, c->grav_F, c->grav_gb, c->grav_U1, c->grav_g1};
+  void* dev[] = {c->Us, c->gs, c->Ub, c->Uc, c->ga, c->cand_list, c->cand_cnt, c->cand_thr, c->cand_stats, c->U1, c->g1, c->Uhost_dev, c->Uhost_dev2, c->gA, c->gB, c->rev_scratch, c->adj_states, c->adj_dts_dev, c->acc, c->dt_dev, c->result_dev, c->tab_dev, c->tab_dev_d, c->tab_part, c->grav_phi, c->grav_F, c->grav_gb, c->grav_U1, c->grav_g1};
   for (void* p : dev)
     if (p) cudaFree(p);
   if (c->result_host) cudaFreeHost(c->result_host);
   if (c->adj_dts_host) cudaFreeHost(c->adj_dts_host);
+  for (int i = 0; i < 3 * c->ev_n; ++i) cudaEventDestroy(c->ev_slab[i]);
+  free(c->ev_slab);
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+  if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
   prof_drop(c);
   free(c->prof);
   delete c;
@@ -225,6 +229,7 @@ int dh_set_option(dh_ctx* c, int key, double v) {
     case DH_OPT_ALPHA2: c->alpha2 = v; break;
     case DH_OPT_GAMMA0: if (v < 0) return fail(DH_ERR_ARG, "dh_set_option: gamma0 must be >= 0%s"); c->gamma0 = v; break;
     case DH_OPT_COOL_FSUB: if (!(v > 0)) return fail(DH_ERR_ARG, "dh_set_option: cool_fsub must be > 0%s"); c->f_sub = v; break;
+    case DH_OPT_STREAM_SLAB: if (v < 0 || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: stream_slab must be a non-negative integer%s"); c->stream_slab_opt = (int)v; break;
     case DH_OPT_COOL_NSUB:
       if (v < 1 || v > DH_COOL_NSUB_MAX || v != (double)(int)v) return fail(DH_ERR_ARG, "dh_set_option: cool_nsub must be an integer in 1 .. 64%s");
       c->cool_nsub = (int)v; break;
@@ -261,6 +266,7 @@ int dh_get_option(const dh_ctx* c, int key, double* out) {
     case DH_OPT_ALPHA2: *out = c->alpha2; break;
     case DH_OPT_GAMMA0: *out = c->gamma0; break;
     case DH_OPT_COOL_FSUB: *out = c->f_sub; break;
+    case DH_OPT_STREAM_SLAB: *out = c->stream_slab_opt; break;
     case DH_OPT_COOL_NSUB: *out = c->cool_nsub; break;
     default: return fail(DH_ERR_ARG, "dh_get_option: unknown key%s");
   }
@@ -295,6 +301,24 @@ int dh_profile_read(dh_ctx* c, double* ms_out, unsigned long long* launches_out)
 }
 
 }  // extern "C"
+
+// dh_advance / dh_stream_host: the CFL candidate list of DH_OPT_FUSE_CFL, allocated on first use, counters reset per call
+static int cand_alloc(dh_ctx* c) {
+  if (!c->cand_list) {
+    c->cand_cap = 1u << 20;
+    int rc = lazy_alloc(c, (void**)&c->cand_list, (size_t)c->cand_cap * sizeof(unsigned), "the CFL candidate list");
+    if (rc) return rc;
+    rc = lazy_alloc(c, (void**)&c->cand_cnt, 2 * sizeof(unsigned), "the CFL candidate counters");
+    if (rc) return rc;
+    rc = lazy_alloc(c, &c->cand_thr, 16, "the CFL candidate thresholds");
+    if (rc) return rc;
+    rc = lazy_alloc(c, (void**)&c->cand_stats, 3 * sizeof(unsigned long long), "the CFL candidate counters");
+    if (rc) return rc;
+    DH_CUDA(cudaMemsetAsync(c->cand_stats, 0, 3 * sizeof(unsigned long long), c->stream), "reset of the candidate statistics");
+  }
+  DH_CUDA(cudaMemsetAsync(c->cand_cnt, 0, 2 * sizeof(unsigned), c->stream), "reset of the candidate counters");
+  return DH_OK;
+}
 
 // ------------------------------------------------------------------------------------------------ CFL
 // cand: the state was written by a last stage that pushed its CFL candidates (dh_advance): exact recipe on those
@@ -339,10 +363,24 @@ static int cfl_launch(dh_ctx* c, const void* U, bool cand = false, bool force_tc
 }
 
 // ------------------------------------------------------------------------------------------ forward
+// What only the fused kernel can do: a z range of planes (dh_stream_host) and the base state formed in the kernel as
+// wB B + wX U (the Shu-Osher stages of Heun / SSPRK3)
+struct StageExtra {
+  int zbeg = 0, zcnt = 0;
+  bool combo = false;
+  double wB = 1.0, wX = 0.0;
+};
+static bool fused_ok(const dh_ctx* c) { return c->kernel == 0 && c->nx % 2 == 0 && (c->ny + 5) / 6 <= 65535; }
+// the in-kernel combination is compiled for fp64 and for the fp32 kernel with 16-byte staging copies (nx % 4 == 0)
+static bool combo_ok(const dh_ctx* c) { return fused_ok(c) && (c->dtype == DH_F64 || c->nx % 4 == 0); }
+
 template <class T>
 static int stage_launch(dh_ctx* c, int kind, const void* U, const void* B, void* out, double dt, bool devdt, double frac, bool cool,
-                        bool cand = false) {
+                        bool cand = false, const StageExtra& x = StageExtra()) {
+  if ((x.zcnt != 0 && !fused_ok(c)) || (x.combo && !combo_ok(c))) return fail(DH_ERR_ARG, "stage_launch: z ranges and in-kernel combinations need the fused kernel%s");
   StageParams<T> p;
+  p.zbeg = x.zbeg; p.zcnt = x.zcnt ? x.zcnt : c->nz;
+  p.combo = x.combo ? 1 : 0; p.wB = (T)x.wB; p.wX = (T)x.wX;
   p.U = (const T*)U; p.B = (const T*)B; p.out = (T*)out;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
   const int n[3] = {c->nx, c->ny, c->nz};
@@ -390,6 +428,18 @@ static int rk_prefix(dh_ctx* c, const void* U, double dt, bool devdt, const void
   if (rc) return rc;
   rc = stage_launch<T>(c, DH_K_STAGE1, U, U, c->Us, dt, devdt, 1.0, false);              // U1 = U - dt D(U)
   if (rc) return rc;
+  if (combo_ok(c)) {
+    // the combinations are formed inside the stage kernel (StageExtra::combo); *last_in / *last_frac as below, rk_last()
+    // passes the weights of the last stage itself
+    if (c->integrator == 1) { *last_in = c->Us; *last_frac = 0.5; return DH_OK; }
+    rc = lazy_alloc(c, &c->Uc, state_bytes(c), "the second stage state");
+    if (rc) return rc;
+    StageExtra x;
+    x.combo = true; x.wB = 0.75; x.wX = 0.25;
+    rc = stage_launch<T>(c, DH_K_STAGE1, c->Us, U, c->Uc, dt, devdt, 0.25, false, false, x);   // U2 = 3/4 U + 1/4 U1 - 1/4 dt D(U1)
+    *last_in = c->Uc; *last_frac = 2.0 / 3.0;
+    return rc;
+  }
   if (c->integrator == 1) {                                                                // Heun
     rc = lincomb<T>(c, c->Ub, 0.5, U, 0.5, c->Us);
     *last_in = c->Us; *last_frac = 0.5;
@@ -404,6 +454,15 @@ static int rk_prefix(dh_ctx* c, const void* U, double dt, bool devdt, const void
   rc = lincomb<T>(c, c->Ub, 1.0 / 3.0, U, 2.0 / 3.0, c->Uc);
   *last_in = c->Uc; *last_frac = 2.0 / 3.0;
   return rc;
+}
+
+// The last stage of Heun / SSPRK3 after rk_prefix:  out = (1 - w) U + w (X - dt D(X)),  X = last_in
+template <class T>
+static int rk_last(dh_ctx* c, const void* last_in, double w, const void* U, void* out, double dt, bool devdt, bool cool, bool cand) {
+  if (!combo_ok(c)) return stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, out, dt, devdt, w, cool, cand);
+  StageExtra x;
+  x.combo = true; x.wB = c->integrator == 1 ? 0.5 : 1.0 / 3.0; x.wX = w;
+  return stage_launch<T>(c, DH_K_STAGE2, last_in, U, out, dt, devdt, w, cool, cand, x);
 }
 
 // The cooling integrators the stage kernels do not fuse (sub-cycled Eq. 23 with N_sub > 1, trapezoid Eq. 22): one
@@ -429,7 +488,7 @@ static int step_impl(dh_ctx* c, void* U, double dt, bool devdt, bool cand = fals
     double w = 0.0;
     int rc = rk_prefix<T>(c, U, dt, devdt, &last_in, &w);
     if (rc) return rc;
-    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, U, dt, devdt, w, fused_cool, cand && !split_cool);
+    rc = rk_last<T>(c, last_in, w, U, U, dt, devdt, fused_cool, cand && !split_cool);
     if (rc || !split_cool) return rc;
     return cool_launch<T>(c, U, dt, devdt);
   }
@@ -443,9 +502,11 @@ static int step_impl(dh_ctx* c, void* U, double dt, bool devdt, bool cand = fals
 
 // ------------------------------------------------------------------------------------------ reverse
 template <class T>
-static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac,
+                      double w1, double w2) {
   RevParams<T> p;
   p.U = (const T*)U; p.g = (const T*)g; p.b1 = (const T*)b1; p.b2 = (const T*)b2; p.out = (T*)out;
+  p.w1 = (T)w1; p.w2 = (T)w2;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
   const int n[3] = {c->nx, c->ny, c->nz};
   for (int a = 0; a < 3; ++a) p.inv_dx[a] = (T)(n[a] / c->L[a]);
@@ -461,7 +522,8 @@ static int rev_launch(dh_ctx* c, int kind, const void* U, const void* g, const v
 // Fused reversed stage (dh_rev.cu): per z slab, the face-adjoint sweep over the slab (it reads 3 planes on each side), then
 // the gather over the slab.  The scratch (10 words per cell of a slab + the tile-edge array) is allocated on first use.
 template <class T>
-static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac,
+                     double w1, double w2) {
   const size_t NP = (size_t)c->nx * c->ny;
   const int ntx = (c->nx + 63) / 64;                       // tiles per row of rev_faces_kernel (RTX = 64)
   const size_t EP = (size_t)c->ny * ntx * 2;               // tile-edge words per plane and field
@@ -502,6 +564,7 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
   a.c = make_consts<T>(c);
   RevGatherParams<T> b;
   b.U = (const T*)U; b.Wp = a.Wp; b.C = a.C; b.Ce = a.Ce; b.b1 = (const T*)b1; b.b2 = (const T*)b2; b.out = (T*)out;
+  b.w1 = (T)w1; b.w2 = (T)w2;
   b.nx = c->nx; b.ny = c->ny; b.nz = c->nz; b.sp0 = 0; b.SP = SP; b.ntx = ntx; b.SPE = a.SPE; b.c = a.c;
   ProfScope ps(c, kind);
   for (int z0 = 0; z0 < c->nz; z0 += c->rev_slab) {
@@ -516,10 +579,11 @@ static int rev_fused(dh_ctx* c, int kind, const void* U, const void* g, const vo
 }
 
 template <class T>
-static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac) {
+static int rev_stage(dh_ctx* c, int kind, const void* U, const void* g, const void* b1, const void* b2, void* out, double dt, double frac,
+                     double w1 = 1.0, double w2 = 1.0) {
   // the fused pair handles every limiter and Riemann flux on even nx; odd nx and DH_OPT_KERNEL = 1 take the one-thread-per-cell gather kernel
-  if (c->kernel == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac);
-  return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac);
+  if (c->kernel == 0 && c->nx % 2 == 0) return rev_fused<T>(c, kind, U, g, b1, b2, out, dt, frac, w1, w2);
+  return rev_launch<T>(c, kind, U, g, b1, b2, out, dt, frac, w1, w2);
 }
 
 // VJP of a Heun / SSPRK3 step.  With a = w g (w the last stage's weight) the last stage gives
@@ -538,7 +602,7 @@ static int vjp_rk(dh_ctx* c, const void* U, double dt, const void* gout, void* g
     if (rc) return rc;
     rc = lazy_alloc(c, &c->g1, state_bytes(c), "the pre-cooling cotangent");
     if (rc) return rc;
-    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, c->U1, dt, false, w, false);
+    rc = rk_last<T>(c, last_in, w, U, c->U1, dt, false, false, false);
     if (rc) return rc;
     ProfScope ps(c, DH_K_COOL_VJP);
     DH_CUDA(launch_cool_vjp<T>((const T*)c->U1, (const T*)gout, (T*)c->g1, c->N, (T)dt, make_consts<T>(c), c->stream),
@@ -546,25 +610,19 @@ static int vjp_rk(dh_ctx* c, const void* U, double dt, const void* gout, void* g
     c->launches += 1;
     g1 = c->g1;
   }
-  void* const h = c->Ub;                                           // the base state is dead: scaled cotangents live there
+  void* const h = c->Ub;                                           // the base state is dead: a combined cotangent lives there
   if (c->integrator == 1) {
     // Heun: U' = 1/2 U + 1/2 (U1 - dt D(U1)), U1 = U - dt D(U)
-    rc = lincomb<T>(c, h, 0.5, g1, 0.0, nullptr);
+    rc = rev_stage<T>(c, DH_K_REV2, c->Us, g1, g1, nullptr, c->gs, dt, 0.5, 0.5);    // U1bar = 1/2 g1 - dt/2 J_D(U1)^T g1
     if (rc) return rc;
-    rc = rev_stage<T>(c, DH_K_REV2, c->Us, g1, h, nullptr, c->gs, dt, 0.5);          // U1bar = h - dt/2 J_D(U1)^T g1
-    if (rc) return rc;
-    return rev_stage<T>(c, DH_K_REV1, U, c->gs, h, c->gs, gin, dt, 1.0);             // Ubar = h + U1bar - dt J_D(U)^T U1bar
+    return rev_stage<T>(c, DH_K_REV1, U, c->gs, g1, c->gs, gin, dt, 1.0, 0.5, 1.0);  // Ubar = 1/2 g1 + U1bar - dt J_D(U)^T U1bar
   }
   // SSPRK3: U' = 1/3 U + 2/3 (U2 - dt D(U2)), U2 = 3/4 U + 1/4 (U1 - dt D(U1)), U1 = U - dt D(U)
   rc = lazy_alloc(c, &c->ga, state_bytes(c), "the first stage cotangent");
   if (rc) return rc;
-  rc = lincomb<T>(c, h, 2.0 / 3.0, g1, 0.0, nullptr);
+  rc = rev_stage<T>(c, DH_K_REV2, c->Uc, g1, g1, nullptr, c->gs, dt, 2.0 / 3.0, 2.0 / 3.0);   // U2bar = 2/3 g1 - 2/3 dt J_D(U2)^T g1
   if (rc) return rc;
-  rc = rev_stage<T>(c, DH_K_REV2, c->Uc, g1, h, nullptr, c->gs, dt, 2.0 / 3.0);      // U2bar = 2/3 g1 - 2/3 dt J_D(U2)^T g1
-  if (rc) return rc;
-  rc = lincomb<T>(c, h, 0.25, c->gs, 0.0, nullptr);
-  if (rc) return rc;
-  rc = rev_stage<T>(c, DH_K_REV1, c->Us, c->gs, h, nullptr, c->ga, dt, 0.25);        // U1bar = 1/4 U2bar - 1/4 dt J_D(U1)^T U2bar
+  rc = rev_stage<T>(c, DH_K_REV1, c->Us, c->gs, c->gs, nullptr, c->ga, dt, 0.25, 0.25);       // U1bar = 1/4 U2bar - 1/4 dt J_D(U1)^T U2bar
   if (rc) return rc;
   rc = lincomb<T>(c, h, 1.0 / 3.0, g1, 0.75, c->gs);
   if (rc) return rc;
@@ -656,19 +714,8 @@ int dh_advance(dh_ctx* c, void* U, int nsteps, double* dt_last_out) {
   // (not with the cooling-time limit of Eq. 21: t_cool needs every cell, so the full pass runs anyway)
   const bool fuse = c->fuse_cfl && nsteps > 1 && c->kernel == 0 && !(c->cooling != 0 && c->c_cool > 0.0);
   if (fuse) {
-    if (!c->cand_list) {
-      c->cand_cap = 1u << 20;
-      int rc = lazy_alloc(c, (void**)&c->cand_list, (size_t)c->cand_cap * sizeof(unsigned), "the CFL candidate list");
-      if (rc) return rc;
-      rc = lazy_alloc(c, (void**)&c->cand_cnt, 2 * sizeof(unsigned), "the CFL candidate counters");
-      if (rc) return rc;
-      rc = lazy_alloc(c, &c->cand_thr, 16, "the CFL candidate thresholds");
-      if (rc) return rc;
-      rc = lazy_alloc(c, (void**)&c->cand_stats, 3 * sizeof(unsigned long long), "the CFL candidate counters");
-      if (rc) return rc;
-      DH_CUDA(cudaMemsetAsync(c->cand_stats, 0, 3 * sizeof(unsigned long long), c->stream), "dh_advance: reset of the candidate statistics");
-    }
-    DH_CUDA(cudaMemsetAsync(c->cand_cnt, 0, 2 * sizeof(unsigned), c->stream), "dh_advance: reset of the candidate counters");
+    int rc = cand_alloc(c);
+    if (rc) return rc;
   }
   c->cand_ok = 0;
   for (int s = 0; s < nsteps; ++s) {
@@ -739,7 +786,7 @@ static int table_vjp_impl(dh_ctx* c, const void* U, double dt, const void* gout,
     double w = 0.0;
     rc = rk_prefix<T>(c, U, dt, false, &last_in, &w);
     if (rc) return rc;
-    rc = stage_launch<T>(c, DH_K_STAGE2, last_in, c->Ub, c->U1, dt, false, w, false);
+    rc = rk_last<T>(c, last_in, w, U, c->U1, dt, false, false, false);
   }
   if (rc) return rc;
   double* const res = c->tab_part + (size_t)cool_table_blocks() * 256;
@@ -952,6 +999,139 @@ int dh_step_gravity_vjp(dh_ctx* c, dh_mg* mg, const void* U, double dt, double f
   if (gU_in == U || gU_in == gU_out) return fail(DH_ERR_ARG, "dh_step_gravity_vjp: gU_in must not alias U or gU_out%s");
   return c->dtype == DH_F32 ? step_gravity_vjp_impl<float>(c, mg, U, dt, four_pi_g, ncycles, gU_out, gU_in)
                             : step_gravity_vjp_impl<double>(c, mg, U, dt, four_pi_g, ncycles, gU_out, gU_in);
+}
+
+}  // extern "C"
+
+// dh_stream_host: a state that lives in HOST memory, every step reading it from there and writing it back (dh.h).
+// Three streams: the link's two directions and the context's compute stream.  The state moves in z slabs; step n computes in
+// device state n % 2:
+//   H2D(n, k)   after D2H(n-1, k) has put slab k of the step's input into U_host          (h2d stream)
+//   dt_n        from the resident copy of the same values (output of step n-1; the candidate CFL pass of dh_advance)
+//   predictor   over the planes whose +-2 neighbours have arrived, as the slabs land (n >= 1; step 0 needs all of U for dt)
+//   corrector   slab by slab in place, each followed by D2H(n, k)                          (d2h stream)
+// so in the steady state both directions of the link are busy and the kernels hide behind them.  Results are those of
+// dh_advance on a resident state bit for bit: the kernels do the same arithmetic per cell whatever z range a launch covers.
+template <class T>
+static int stream_host_impl(dh_ctx* c, void* U_host, int nsteps) {
+  const size_t esz = sizeof(T), NP = (size_t)c->nx * c->ny, N = c->N;
+  int S = c->stream_slab_opt > 0 ? c->stream_slab_opt : (c->nz + 31) / 32;
+  if (S < 8) S = 8;
+  if (S > c->nz) S = c->nz;
+  const int ns = (c->nz + S - 1) / S;
+  int rc = lazy_alloc(c, &c->Uhost_dev, state_bytes(c), "the device state of the host entry point");
+  if (rc) return rc;
+  rc = lazy_alloc(c, &c->Uhost_dev2, state_bytes(c), "the second device state of dh_stream_host");
+  if (rc) return rc;
+  if (!c->h2d_stream) DH_CUDA(cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking), "dh_stream_host: stream");
+  if (!c->d2h_stream) DH_CUDA(cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking), "dh_stream_host: stream");
+  if (c->ev_n < ns + 1) {
+    for (int i = 0; i < 3 * c->ev_n; ++i) cudaEventDestroy(c->ev_slab[i]);
+    free(c->ev_slab);
+    c->ev_n = 0;
+    c->ev_slab = (cudaEvent_t*)calloc((size_t)3 * (ns + 1), sizeof(cudaEvent_t));
+    if (!c->ev_slab) return fail(DH_ERR_ALLOC, "dh_stream_host: out of host memory%s");
+    for (int i = 0; i < 3 * (ns + 1); ++i) DH_CUDA(cudaEventCreateWithFlags(&c->ev_slab[i], cudaEventDisableTiming), "dh_stream_host: event");
+    c->ev_n = ns + 1;
+  }
+  cudaEvent_t* const ev_in = c->ev_slab;
+  cudaEvent_t* const ev_cmp = c->ev_slab + c->ev_n;
+  cudaEvent_t* const ev_out = c->ev_slab + 2 * c->ev_n;
+  cudaEvent_t const ev_sync = ev_in[ns];                       // entry / exit ordering against the context's stream
+  void* const dev[2] = {c->Uhost_dev, c->Uhost_dev2};
+  auto copy_slab = [&](void* dst, const void* src, int k, cudaMemcpyKind kind, cudaStream_t st) -> cudaError_t {
+    const int z0 = k * S, cnt = (c->nz - z0 < S) ? c->nz - z0 : S;
+    for (int f = 0; f < 5; ++f) {
+      const size_t off = ((size_t)f * N + (size_t)z0 * NP) * esz;
+      cudaError_t e = cudaMemcpyAsync((char*)dst + off, (const char*)src + off, (size_t)cnt * NP * esz, kind, st);
+      if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+  };
+  // work queued earlier on the context's stream may still use the device states
+  DH_CUDA(cudaEventRecord(ev_sync, c->stream), "dh_stream_host: event record");
+  DH_CUDA(cudaStreamWaitEvent(c->h2d_stream, ev_sync, 0), "dh_stream_host: stream wait");
+  DH_CUDA(cudaStreamWaitEvent(c->d2h_stream, ev_sync, 0), "dh_stream_host: stream wait");
+
+  const bool split_cool = c->cooling != 0 && (c->cool_mode != 0 || c->cool_nsub > 1 || c->cool_law != 0);
+  const bool fused_cool = c->cooling != 0 && !split_cool;
+  const bool ranges = fused_ok(c) && c->integrator == 0 && !split_cool;        // else: whole-grid launches, only the copies overlap
+  const bool fuse = c->fuse_cfl && nsteps > 1 && c->kernel == 0 && !(c->cooling != 0 && c->c_cool > 0.0);
+  if (fuse) {
+    rc = cand_alloc(c);
+    if (rc) return rc;
+  }
+  c->cand_ok = 0;
+  for (int n = 0; n < nsteps; ++n) {
+    void* const Ud = dev[n & 1];
+    for (int k = 0; k < ns; ++k) {
+      if (n > 0) DH_CUDA(cudaStreamWaitEvent(c->h2d_stream, ev_out[k], 0), "dh_stream_host: stream wait");
+      DH_CUDA(copy_slab(Ud, U_host, k, cudaMemcpyHostToDevice, c->h2d_stream), "dh_stream_host: H2D");
+      DH_CUDA(cudaEventRecord(ev_in[k], c->h2d_stream), "dh_stream_host: event record");
+    }
+    const bool push = fuse && n + 1 < nsteps;
+    if (n == 0) {
+      DH_CUDA(cudaStreamWaitEvent(c->stream, ev_in[ns - 1], 0), "dh_stream_host: stream wait");
+      rc = cfl_launch<T>(c, Ud, false);
+    } else {
+      rc = cfl_launch<T>(c, dev[(n & 1) ^ 1], fuse && c->cand_ok);
+    }
+    if (rc) return rc;
+    if (ranges) {
+      StageExtra x;
+      if (n == 0) {
+        rc = stage_launch<T>(c, DH_K_STAGE1, Ud, Ud, c->Us, 0.0, true, 0.5, false);
+        if (rc) return rc;
+      } else {
+        int done = 2;                                           // planes [2, done) of U* are launched
+        for (int k = 0; k < ns; ++k) {
+          DH_CUDA(cudaStreamWaitEvent(c->stream, ev_in[k], 0), "dh_stream_host: stream wait");
+          const int landed = (k + 1) * S < c->nz ? (k + 1) * S : c->nz;
+          const int hi = (k == ns - 1) ? c->nz + 2 : landed - 2;   // the last launch wraps around: planes nz-2, nz-1, 0, 1
+          if (hi <= done) continue;
+          x.zbeg = done; x.zcnt = hi - done;
+          rc = stage_launch<T>(c, DH_K_STAGE1, Ud, Ud, c->Us, 0.0, true, 0.5, false, false, x);
+          if (rc) return rc;
+          done = hi;
+        }
+      }
+      bool pushed = true;
+      for (int k = 0; k < ns; ++k) {
+        x.zbeg = k * S; x.zcnt = (c->nz - k * S < S) ? c->nz - k * S : S;
+        rc = stage_launch<T>(c, DH_K_STAGE2, c->Us, Ud, Ud, 0.0, true, 1.0, fused_cool, push, x);
+        if (rc) return rc;
+        pushed = pushed && c->cand_ok;
+        DH_CUDA(cudaEventRecord(ev_cmp[k], c->stream), "dh_stream_host: event record");
+      }
+      c->cand_ok = pushed ? 1 : 0;
+    } else {
+      DH_CUDA(cudaStreamWaitEvent(c->stream, ev_in[ns - 1], 0), "dh_stream_host: stream wait");
+      rc = step_impl<T>(c, Ud, 0.0, true, push);
+      if (rc) return rc;
+      DH_CUDA(cudaEventRecord(ev_cmp[0], c->stream), "dh_stream_host: event record");
+    }
+    for (int k = 0; k < ns; ++k) {
+      DH_CUDA(cudaStreamWaitEvent(c->d2h_stream, ev_cmp[ranges ? k : 0], 0), "dh_stream_host: stream wait");
+      DH_CUDA(copy_slab(U_host, Ud, k, cudaMemcpyDeviceToHost, c->d2h_stream), "dh_stream_host: D2H");
+      DH_CUDA(cudaEventRecord(ev_out[k], c->d2h_stream), "dh_stream_host: event record");
+    }
+  }
+  c->cand_ok = 0;
+  DH_CUDA(cudaEventRecord(ev_sync, c->d2h_stream), "dh_stream_host: event record");
+  DH_CUDA(cudaStreamWaitEvent(c->stream, ev_sync, 0), "dh_stream_host: stream wait");
+  return DH_OK;
+}
+
+extern "C" {
+
+int dh_stream_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {
+  if (!c || !U_host || nsteps < 0) return fail(DH_ERR_ARG, "dh_stream_host: bad argument%s");
+  if (int drc = check_device(c, "dh_stream_host")) return drc;
+  if (nsteps > 0) {
+    int rc = c->dtype == DH_F32 ? stream_host_impl<float>(c, U_host, nsteps) : stream_host_impl<double>(c, U_host, nsteps);
+    if (rc) return rc;
+  }
+  return dh_poll_status(c, dt_last_out);
 }
 
 int dh_run_host(dh_ctx* c, void* U_host, int nsteps, double* dt_last_out) {

@@ -80,7 +80,7 @@ DH_DI void recon_x2(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
 
 }  // namespace
 
-template <class T, int LIM, int RS, int NRW, bool V16, bool CAND>
+template <class T, int LIM, int RS, int NRW, bool V16, bool CAND, bool COMBO>
 __global__ void __launch_bounds__((NRW + 1) * 32, 1)
 stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   using G = Geo2<NRW>;
@@ -93,12 +93,13 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   T* const Fxs = Rxs + 2 * G::XE;                  // [2][5][TY][XP2]     x flux through the LEFT face of lane l; slot 0: helper
   T* const Ust = Fxs + 2 * G::XE;                  // [5][TY][TX2]        raw U of the next plane (cp.async, private slots)
   T* const Bst = Ust + G::STAGE;                   // [2][5][TY][TX2]     base state, loaded one plane ahead (cp.async, private slots)
+  T* const Xst = Bst + 2 * G::STAGE;               // [2][5][TY][TX2]     raw U of planes p, p-1 (COMBO launches only: they get the room)
 
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
   const size_t NP = (size_t)nx * ny, N = NP * nz;
-  const int x0 = blockIdx.x * TX2, y0 = blockIdx.y * TY, z0 = blockIdx.z * ZL;
-  const int zl = min(ZL, nz - z0);
+  const int x0 = blockIdx.x * TX2, y0 = blockIdx.y * TY, z0 = p.zbeg + blockIdx.z * ZL;
+  const int zl = min(ZL, p.zbeg + p.zcnt - z0);
   const int nit = zl + 4;                          // planes z0-2 .. z0+zl+1
   const T dt = p.dt_dev ? *p.dt_dev : p.dt;
   const T tau = p.frac * dt;
@@ -108,6 +109,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
   const Consts<T>& c = p.c;
   const T cand_thr = CAND ? p.cand_thr[0] : T(0);   // CAND: push the CFL candidates of the result (dh_advance)
+  constexpr bool combo = COMBO;                     // out = wB B + wX U - tau D(U): the base state is formed here
   int pz = wrapm2(z0 - 2, nz);
   size_t op = (size_t)pz * NP, opm1 = op, opm2 = op;   // element offsets of planes p, p-1, p-2
 
@@ -152,6 +154,10 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       P2<T> NA[5], NB[5];                          // plane p: raw, then primitive
 #pragma unroll
       for (int f = 0; f < 5; ++f) { NA[f] = lds2_(Ust + f * FS + stA); NB[f] = lds2_(Ust + f * FS + stB); }
+      if (combo) {                                 // kept for the base state of this plane, formed one iteration later
+#pragma unroll
+        for (int f = 0; f < 5; ++f) { sts2_(Xst + bp * G::STAGE + f * FS + stA, NA[f]); sts2_(Xst + bp * G::STAGE + f * FS + stB, NB[f]); }
+      }
       // one plane ahead: the raw state of plane p+1 and the base state of plane p (used in the next iteration)
       int pzn = pz + 1;
       size_t opn = op + NP;
@@ -209,7 +215,11 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
             if (slot < p.cand_cap) p.cand_list[slot] = (unsigned)(opm2 + o_);                       \
           }                                                                                         \
         }                                                                                           \
-        _Pragma("unroll") for (int f = 0; f < 5; ++f) acc_[f] = fma2(cz, Fz[f], lds2_(Bst + bq * G::STAGE + f * FS + st_)); \
+        _Pragma("unroll") for (int f = 0; f < 5; ++f) {                                             \
+          P2<T> b = lds2_(Bst + bq * G::STAGE + f * FS + st_);                                      \
+          if (combo) b = fma2(bc2(p.wX), lds2_(Xst + bq * G::STAGE + f * FS + st_), mul2(bc2(p.wB), b)); \
+          acc_[f] = fma2(cz, Fz[f], b);                                                             \
+        }                                                                                           \
       }
       DH_ZPHASE(NA, WA, dA, LzA, accA, okA, oA, stA)
       // x neighbours of plane p-1, loaded here so that their latency hides behind the second z phase
@@ -404,15 +414,15 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
 
 namespace {
 
-template <class T, int LIM, int RS, int NRW, bool V16, bool CAND>
+template <class T, int LIM, int RS, int NRW, bool V16, bool CAND, bool COMBO>
 cudaError_t launch_one2c(const StageParams<T>& p, int sm_count, cudaStream_t s) {
   using G = Geo2<NRW>;
-  const size_t smem = (size_t)G::TOTAL * sizeof(T);
+  const size_t smem = (size_t)(G::TOTAL + (COMBO ? 2 * G::STAGE : 0)) * sizeof(T);
   static bool configured[64] = {};    // per instantiation and per device: the attribute belongs to the (function, device) pair
   int cur_dev = 0;
   cudaGetDevice(&cur_dev);
   if (cur_dev < 0 || cur_dev >= 64 || !configured[cur_dev]) {
-    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute((const void*)stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND, COMBO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     if (cur_dev >= 0 && cur_dev < 64) configured[cur_dev] = true;
   }
@@ -421,25 +431,33 @@ cudaError_t launch_one2c(const StageParams<T>& p, int sm_count, cudaStream_t s) 
   // pick the chunk count that minimises waves x (planes per chunk + 4)
   int dev = 0, per_sm = 1;
   cudaGetDevice(&dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND, COMBO>, (NRW + 1) * 32, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
   const long long slots = (long long)per_sm * sm_count, tiles = (long long)bx * by;
   int bz = 1;
   long long best = -1;
-  for (int cand = 1; cand <= p.nz / 4 && cand <= 65535; ++cand) {
-    const int zl_c = (p.nz + cand - 1) / cand;
-    if ((p.nz + zl_c - 1) / zl_c != cand) continue;
+  const int zc = p.zcnt;                           // planes of this launch (the whole grid or a z range)
+  for (int cand = 1; cand <= (zc < 4 ? 1 : zc / 4) && cand <= 65535; ++cand) {
+    const int zl_c = (zc + cand - 1) / cand;
+    if ((zc + zl_c - 1) / zl_c != cand) continue;
     const long long cost = ((tiles * cand + slots - 1) / slots) * (zl_c + 4);
     if (best < 0 || cost < best) { best = cost; bz = cand; }
   }
-  const int ZL = (p.nz + bz - 1) / bz;
+  const int ZL = (zc + bz - 1) / bz;
   dim3 grid(bx, by, bz), block((NRW + 1) * 32);
-  stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND><<<grid, block, smem, s>>>(p, ZL);
+  stage_fused2_kernel<T, LIM, RS, NRW, V16, CAND, COMBO><<<grid, block, smem, s>>>(p, ZL);
   return cudaGetLastError();
 }
 
 template <class T, int LIM, int RS, int NRW, bool V16>
 cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
-  return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false>(p, sm_count, s);
+  // COMBO is instantiated where combo_ok() (dh_api.cu) says so (fp64, and fp32 with 16-byte staging): the other shapes never ask for it
+  if constexpr (sizeof(T) == 8 || V16) {
+    if (p.combo)
+      return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true, true>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false, true>(p, sm_count, s);
+  } else {
+    if (p.combo) return cudaErrorInvalidValue;
+  }
+  return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true, false>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false, false>(p, sm_count, s);
 }
 
 }  // namespace

@@ -27,15 +27,23 @@ struct StageParams {
   unsigned* cand_cnt;     // [0] packs appended (may exceed cand_cap: overflow = fall back to the full reduction)
   const T* cand_thr;      // [0] derated threshold for the estimate
   unsigned cand_cap;
+  // z range of the launch (fused kernel only; zcnt == 0: the whole grid): planes zbeg .. zbeg + zcnt - 1, taken modulo nz
+  // (dh_stream_host computes the planes whose inputs have arrived)
+  int zbeg, zcnt;
+  // combo != 0 (fused kernel only): out = wB B + wX U - frac dt D(U): the Shu-Osher stages of Heun / SSPRK3
+  // without a pass that forms the combination first
+  int combo;
+  T wB, wX;
 };
 
-// Parameters of one reversed stage  out = b1 + b2 - frac*dt * J_D(U)^T g   (gather form).
+// Parameters of one reversed stage  out = w1 b1 + w2 b2 - frac*dt * J_D(U)^T g   (gather form).
 template <class T>
 struct RevParams {
   const T* U;        // primal state the stage was evaluated at
   const T* g;        // cotangent of the stage output
   const T* b1;       // optional additive terms (nullptr = none)
   const T* b2;
+  T w1, w2;          // their weights (the stage weights of Heun / SSPRK3 reversed; 1 for RK2)
   T* out;
   int nx, ny, nz;
   T inv_dx[3];
@@ -72,6 +80,7 @@ struct RevGatherParams {
   const T* Ce;
   const T* b1;       // optional additive terms (nullptr = none)
   const T* b2;
+  T w1, w2;          // their weights
   T* out;
   int nx, ny, nz;
   int z0, nplanes;   // planes z0 .. z0 + nplanes - 1 (all inside [0, nz))
@@ -144,6 +153,11 @@ struct Ctx {
   void* grav_U1;
   void* grav_g1;
   void* Uhost_dev;             // device state for the HOST entry points
+  void* Uhost_dev2;            // dh_stream_host: the second device state (steps alternate between the two)
+  cudaStream_t h2d_stream, d2h_stream;   // dh_stream_host: one stream per link direction (non-blocking, created on first use)
+  cudaEvent_t* ev_slab;        // dh_stream_host: [3][ev_n] slab arrived / slab computed / slab written back
+  int ev_n;
+  int stream_slab_opt;         // DH_OPT_STREAM_SLAB (0 = automatic)
   void* gA;                    // device cotangent buffers for dh_step_vjp_host
   void* gB;
   void* rev_scratch;           // 20 words per cell of a z slab (+2 planes), fused reverse stages

@@ -165,8 +165,8 @@ __global__ void __launch_bounds__(64) rev_naive_kernel(const RevParams<T> p) {
 #pragma unroll
   for (int f = 0; f < 5; ++f) {
     T v = Ub[f];
-    if (p.b1) v += p.b1[f * N + c0];
-    if (p.b2) v += p.b2[f * N + c0];
+    if (p.b1) v += p.w1 * p.b1[f * N + c0];
+    if (p.b2) v += p.w2 * p.b2[f * N + c0];
     p.out[f * N + c0] = v;
   }
 }

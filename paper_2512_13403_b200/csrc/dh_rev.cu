@@ -1,6 +1,6 @@
 // dh_rev.cu — fused reverse-mode stage (step a7 of SURVEY.md §8(a), dt constant per PAPER.md:876).
 //
-// One reversed stage  out = b1 + b2 - tau J_D(U)^T g  (D(U) = sum_a (F_{a,+1/2} - F_{a,-1/2}) / dx_a, Eq. A4) is the
+// One reversed stage  out = w1 b1 + w2 b2 - tau J_D(U)^T g  (D(U) = sum_a (F_{a,+1/2} - F_{a,-1/2}) / dx_a, Eq. A4) is the
 // transpose of: primitives -> minmod slopes -> face states -> HLLC flux -> flux difference.  Written per axis for
 // cell i (coef = tau / dx_a):
 //     lambda_{i+1/2} = coef (g_{i+1} - g_i)                                   face cotangent
@@ -21,7 +21,7 @@
 //                         per cell it writes  Wp = everything but the y neighbour terms  and  c^y; the x terms that cross a
 //                         tile edge go through a thin array of the tile rows' first and last c^x;
 //   B  rev_gather_kernel  streaming: Wb_i = Wp_i + [a-branch c^y_{j-1}] - [b-branch c^y_{j+1}] (+ the tile-edge x term),
-//                         then Ub = prim_vjp(U, Wb) + b1 + b2.
+//                         then Ub = prim_vjp(U, Wb) + w1 b1 + w2 b2.
 // Scratch is 10 words per cell of a z slab (+ 10 / 64 for the tile edges); the API layer walks the slabs.  minmod only
 // (the branch flag is one bit); other limiters take the gather kernels.  No atomics; deterministic.
 #include "dh_internal.cuh"
@@ -636,7 +636,7 @@ rev_faces_kernel(const RevFaceParams<T> p, const int ZL) {
 
 // ------------------------------------------------------------------------------------------------ kernel B
 // One thread per pack (two x-adjacent cells) of a slab plane: adds the y neighbour terms (rows j -+ 1 of C) and, for the
-// packs at a tile edge, the x term that crossed it (Ce), then Ub = prim_vjp(U, Wb) + b1 + b2.
+// packs at a tile edge, the x term that crossed it (Ce), then Ub = prim_vjp(U, Wb) + w1 b1 + w2 b2.
 template <class T, int LIM>
 __global__ void __launch_bounds__(128, 16) rev_gather_kernel(const RevGatherParams<T> p) {
   const int ip = blockIdx.x * blockDim.x + threadIdx.x;       // pack index along x
@@ -684,8 +684,8 @@ __global__ void __launch_bounds__(128, 16) rev_gather_kernel(const RevGatherPara
 #pragma unroll
   for (int f = 0; f < 5; ++f) {
     P2<T> v = {ubx[f], uby[f]};
-    if (p.b1) v = add2(v, rldg2(p.b1 + f * N + cell));
-    if (p.b2) v = add2(v, rldg2(p.b2 + f * N + cell));
+    if (p.b1) v = fma2(bc2(p.w1), rldg2(p.b1 + f * N + cell), v);
+    if (p.b2) v = fma2(bc2(p.w2), rldg2(p.b2 + f * N + cell), v);
     rstg2(p.out + f * N + cell, v);
   }
 }

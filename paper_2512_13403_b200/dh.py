@@ -21,7 +21,7 @@ OPTIONS = {
     "cfl": 0, "lx": 1, "ly": 2, "lz": 3, "cooling": 4, "lambda0": 5, "alpha": 6, "t_floor": 7,
     "rho_floor": 8, "p_floor": 9, "kernel": 10, "limiter": 11, "rev_slab": 12, "integrator": 13, "fuse_cfl": 14,
     "riemann": 15, "cool_mode": 16, "cool_nsub": 17, "c_cool": 18, "dt_max": 19, "cool_law": 20, "t_switch": 21,
-    "lambda1": 22, "alpha1": 23, "lambda2": 24, "alpha2": 25, "gamma0": 26, "f_sub": 27,
+    "lambda1": 22, "alpha1": 23, "lambda2": 24, "alpha2": 25, "gamma0": 26, "f_sub": 27, "stream_slab": 28,
 }
 LIMITERS = {"minmod": 0, "vanleer": 1, "mc": 2}
 RIEMANN = {"hllc": 0, "hll": 1, "rusanov": 2}       # DH_OPT_RIEMANN
@@ -33,7 +33,7 @@ KERNELS = {"fused": 0, "gather": 1}
 # every symbol include/dh.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
     "dh_create", "dh_destroy", "dh_set_stream", "dh_set_option", "dh_get_option", "dh_cfl_dt", "dh_step",
-    "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_step_vjp_host",
+    "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_stream_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
     "dh_cfl_stats", "dh_cool_tmin", "dh_set_cooling_table", "dh_cool_table_vjp",
     "dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp",
@@ -76,6 +76,8 @@ def load(rebuild: bool = False):
     lib.dh_step_devdt.argtypes = [vp, vp]
     lib.dh_step_vjp.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_run_host.argtypes = [vp, vp, ci, pd]
+    lib.dh_stream_host.argtypes = [vp, vp, ci, pd]
+    lib.dh_stream_host.restype = ci
     lib.dh_advance.argtypes = [vp, vp, ci, pd]
     lib.dh_adjoint.argtypes = [vp, vp, vp, ci, ci, pd]
     lib.dh_step_vjp_host.argtypes = [vp, vp, cd, vp, vp]
@@ -212,6 +214,12 @@ def dh_adjoint(ctx, U_ptr: int, gU_ptr: int, nsteps: int, every: int) -> list:
 def dh_run_host(ctx, U_host_ptr: int, nsteps: int) -> float:
     out = ctypes.c_double()
     _check(load().dh_run_host(ctx, ctypes.c_void_p(U_host_ptr), int(nsteps), ctypes.byref(out)))
+    return out.value
+
+
+def dh_stream_host(ctx, U_host_ptr: int, nsteps: int) -> float:
+    out = ctypes.c_double()
+    _check(load().dh_stream_host(ctx, ctypes.c_void_p(U_host_ptr), int(nsteps), ctypes.byref(out)))
     return out.value
 
 
@@ -374,6 +382,9 @@ class Solver:
 
     def run_host(self, U_host, nsteps: int) -> float:
         return dh_run_host(self.ctx, self._host(U_host, "U_host"), nsteps)
+
+    def stream_host(self, U_host, nsteps: int) -> float:
+        return dh_stream_host(self.ctx, self._host(U_host, "U_host"), nsteps)
 
     def step_vjp_host(self, U_host, dt: float, g_out_host, g_in_host) -> None:
         dh_step_vjp_host(self.ctx, self._host(U_host, "U_host"), dt, self._host(g_out_host, "g_out_host"),
