@@ -2,6 +2,6 @@
 #include "dh_fused2_impl.cuh"
 
 namespace dh {
-template cudaError_t launch_stage_fused2_rs<float, 1>(const StageParams<float>&, int, int, cudaStream_t, bool*);
-template cudaError_t launch_stage_fused2_rs<double, 1>(const StageParams<double>&, int, int, cudaStream_t, bool*);
+template cudaError_t launch_stage_fused2_rs<float, 1, false>(const StageParams<float>&, int, int, cudaStream_t, bool*);
+template cudaError_t launch_stage_fused2_rs<double, 1, false>(const StageParams<double>&, int, int, cudaStream_t, bool*);
 }  // namespace dh

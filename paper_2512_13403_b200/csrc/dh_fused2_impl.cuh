@@ -23,7 +23,7 @@
 // cells and predicate the stores.  The loop body is branch-free: lead-in / lead-out planes run the same
 // instructions on data nobody stores.
 // One translation unit per Riemann flux (dh_fused2.cu HLLC, dh_fused2_hll.cu, dh_fused2_rusanov.cu) includes this file
-// and instantiates launch_stage_fused2_rs<T, RS>; they compile side by side.
+// and instantiates launch_stage_fused2_rs<T, RS, COMBO>; they compile side by side.
 #pragma once
 #include "dh_internal.cuh"
 #include "dh_pack.cuh"
@@ -448,21 +448,16 @@ cudaError_t launch_one2c(const StageParams<T>& p, int sm_count, cudaStream_t s) 
   return cudaGetLastError();
 }
 
-template <class T, int LIM, int RS, int NRW, bool V16>
+template <class T, int LIM, int RS, int NRW, bool V16, bool COMBO>
 cudaError_t launch_one2(const StageParams<T>& p, int sm_count, cudaStream_t s) {
-  // COMBO is instantiated where combo_ok() (dh_api.cu) says so (fp64, and fp32 with 16-byte staging): the other shapes never ask for it
-  if constexpr (sizeof(T) == 8 || V16) {
-    if (p.combo)
-      return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true, true>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false, true>(p, sm_count, s);
-  } else {
-    if (p.combo) return cudaErrorInvalidValue;
-  }
-  return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true, false>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false, false>(p, sm_count, s);
+  return p.cand_list ? launch_one2c<T, LIM, RS, NRW, V16, true, COMBO>(p, sm_count, s) : launch_one2c<T, LIM, RS, NRW, V16, false, COMBO>(p, sm_count, s);
 }
 
 }  // namespace
 
-template <class T, int RS>
+// COMBO (StageParams::combo, the Shu-Osher stages of Heun / SSPRK3) is a set of instantiations of its own, built in translation
+// units of its own (dh_fused2_combo*.cu): a run-time flag costs the default kernel 8 registers and 3-4 %.
+template <class T, int RS, bool COMBO>
 cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported) {
   // packs are two cells adjacent in x: nx must be even; grid.y/z <= 65535
   *supported = (p.nx % 2 == 0) && ((p.ny + 5) / 6 <= 65535);
@@ -472,15 +467,19 @@ cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_
   constexpr int NRW = sizeof(T) == 4 ? 7 : 3;
   if (sizeof(T) == 4 && p.nx % 4 == 0) {             // 16-byte staging copies
     switch (limiter) {
-      case 1: return launch_one2<T, 1, RS, NRW, true>(p, sm_count, s);
-      case 2: return launch_one2<T, 2, RS, NRW, true>(p, sm_count, s);
-      default: return launch_one2<T, 0, RS, NRW, true>(p, sm_count, s);
+      case 1: return launch_one2<T, 1, RS, NRW, true, COMBO>(p, sm_count, s);
+      case 2: return launch_one2<T, 2, RS, NRW, true, COMBO>(p, sm_count, s);
+      default: return launch_one2<T, 0, RS, NRW, true, COMBO>(p, sm_count, s);
     }
   }
-  switch (limiter) {
-    case 1: return launch_one2<T, 1, RS, NRW, false>(p, sm_count, s);
-    case 2: return launch_one2<T, 2, RS, NRW, false>(p, sm_count, s);
-    default: return launch_one2<T, 0, RS, NRW, false>(p, sm_count, s);
+  if constexpr (COMBO && sizeof(T) == 4) {
+    return cudaErrorInvalidValue;                    // combo_ok() in dh_api.cu never asks: fp32 COMBO is built for nx % 4 == 0 only
+  } else {
+    switch (limiter) {
+      case 1: return launch_one2<T, 1, RS, NRW, false, COMBO>(p, sm_count, s);
+      case 2: return launch_one2<T, 2, RS, NRW, false, COMBO>(p, sm_count, s);
+      default: return launch_one2<T, 0, RS, NRW, false, COMBO>(p, sm_count, s);
+    }
   }
 }
 

@@ -197,7 +197,7 @@ size_t elem_size(const Ctx* c);
 // launchers (each returns the cudaError_t of the launch)
 template <class T> cudaError_t launch_stage_naive(const StageParams<T>& p, int limiter, int riemann, cudaStream_t s);
 template <class T> cudaError_t launch_stage_fused2(const StageParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s, bool* supported);
-template <class T, int RS> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
+template <class T, int RS, bool COMBO> cudaError_t launch_stage_fused2_rs(const StageParams<T>& p, int limiter, int sm_count, cudaStream_t s, bool* supported);
 template <class T> cudaError_t launch_rev_naive(const RevParams<T>& p, int limiter, int riemann, cudaStream_t s);
 template <class T> cudaError_t launch_rev_faces(const RevFaceParams<T>& p, int limiter, int riemann, int sm_count, cudaStream_t s);
 int rev_scratch_words(int limiter);
