@@ -36,6 +36,8 @@
 #ifndef DH_H_
 #define DH_H_
 
+#include <stddef.h>
+
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -145,6 +147,23 @@ int dh_cool_table_vjp(dh_ctx* ctx, const void* U, double dt, const void* gU_out,
  * dt_out: HOST; receives the T value widened exactly.  Synchronises the stream (the only host sync of
  * the path).  Returns DH_ERR_NONFINITE (and leaves *dt_out untouched) if any input or speed is NaN/Inf. */
 int dh_cfl_dt(dh_ctx* ctx, const void* U, double* dt_out);
+
+/* Eq. A8 for callers that must not allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): NO context (dh_create allocates) and no cudaMalloc / cudaFree / allocating library call inside.  The scratch of the
+ * reduction (one 32-byte record of block maxima per 16384 cells) lives in a file-scope device array of 256 KiB that every GPU
+ * loading the library holds until exit, so the grid is limited to dh_static_max_cells() = 2^27 cells (512^3); larger grids return
+ * DH_ERR_ARG with a message saying so.  Same per-cell recipe and epilogue as dh_cfl_dt: dt is bit-identical to it.
+ *   U:         DEVICE, read only, [5][nz][ny][nx] of `dtype` (DH_F32 / DH_F64).
+ *   box:       HOST, the three box lengths, or NULL for 1, 1, 1.   gamma > 1, cfl > 0, floors >= 0 (dh_create's defaults: 1e-10).
+ *   out5_dev:  DEVICE, caller-owned, 5 doubles: dt (the T value widened), max S_x, max S_y, max S_z, 1.0 if a NaN / Inf input
+ *              or wave speed was seen (dt is then meaningless), else 0.0.
+ *   cuda_stream: the stream both kernels are launched on (NULL = the default stream).  Asynchronous; nothing is synchronised.
+ * The device array is shared by every call on that GPU and keeps the last call's records (each call overwrites the records it
+ * reads, nothing has to be cleared): calls that overlap on the GPU, e.g. on two streams without a dependency, race.  The array's
+ * device address is looked up once per device (cudaGetSymbolAddress, with that device current, at the first call there). */
+int dh_cfl_dt_static(const void* U, int nx, int ny, int nz, int dtype, double gamma, double cfl, const double* box, double rho_floor,
+                     double p_floor, double* out5_dev, void* cuda_stream);
+size_t dh_static_max_cells(void);
 
 /* min_x t_cool(x), Eq. 20, for the cooling parameters of the context (DH_OPT_LAMBDA0 / DH_OPT_ALPHA; DH_OPT_COOLING
  * need not be on): one pass of the CFL reduction kernel with the cooling-time branch.  U: DEVICE, read only.

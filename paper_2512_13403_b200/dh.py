@@ -36,7 +36,7 @@ SYMBOLS = [
     "dh_step_devdt", "dh_cfl_dt_async", "dh_poll_status", "dh_step_vjp", "dh_run_host", "dh_stream_host", "dh_step_vjp_host",
     "dh_advance", "dh_adjoint", "dh_launch_count", "dh_last_error", "dh_version", "dh_profile_enable", "dh_profile_read",
     "dh_cfl_stats", "dh_cool_tmin", "dh_set_cooling_table", "dh_cool_table_vjp",
-    "dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp",
+    "dh_cfl_dt_static", "dh_static_max_cells", "dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp",
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
     "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
@@ -77,6 +77,10 @@ def load(rebuild: bool = False):
     lib.dh_step_vjp.argtypes = [vp, vp, cd, vp, vp]
     lib.dh_run_host.argtypes = [vp, vp, ci, pd]
     lib.dh_stream_host.argtypes = [vp, vp, ci, pd]
+    lib.dh_cfl_dt_static.argtypes = [vp, ci, ci, ci, ci, cd, cd, pd, cd, cd, vp, vp]
+    lib.dh_cfl_dt_static.restype = ci
+    lib.dh_static_max_cells.argtypes = []
+    lib.dh_static_max_cells.restype = ctypes.c_size_t
     lib.dh_stream_host.restype = ci
     lib.dh_advance.argtypes = [vp, vp, ci, pd]
     lib.dh_adjoint.argtypes = [vp, vp, vp, ci, ci, pd]
@@ -170,6 +174,18 @@ def dh_cfl_dt(ctx, U_ptr: int) -> float:
     out = ctypes.c_double()
     _check(load().dh_cfl_dt(ctx, ctypes.c_void_p(U_ptr), ctypes.byref(out)))
     return out.value
+
+
+def dh_cfl_dt_static(U_ptr: int, nx: int, ny: int, nz: int, dtype: int, gamma: float, cfl: float, box, rho_floor: float,
+                     p_floor: float, out5_ptr: int, stream_ptr: int = 0) -> None:
+    """No context, no allocation (include/dh.h): out5_ptr is a DEVICE array of 5 doubles the caller owns."""
+    b = (ctypes.c_double * 3)(*[float(v) for v in box]) if box is not None else None
+    _check(load().dh_cfl_dt_static(ctypes.c_void_p(U_ptr), int(nx), int(ny), int(nz), int(dtype), float(gamma), float(cfl), b,
+                                   float(rho_floor), float(p_floor), ctypes.c_void_p(out5_ptr), ctypes.c_void_p(stream_ptr)))
+
+
+def dh_static_max_cells() -> int:
+    return int(load().dh_static_max_cells())
 
 
 def dh_cfl_dt_async(ctx, U_ptr: int) -> None:
