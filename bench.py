@@ -64,6 +64,7 @@ def parse_args():
     ap.add_argument("--poisson", type=int, default=0, metavar="N",
                     help="instead of the hydro step: time multigrid cycles of the periodic Poisson solver on an N^3 grid (SURVEY 8(f) item 3)")
     ap.add_argument("--mg-cycle", choices=["V", "W"], default="V")
+    ap.add_argument("--mg-subtree", type=int, default=1, help="DH_MG_SUBTREE: 1 (default) the levels of <= 4096 cells in one block, 0 one launch per operator")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -517,7 +518,7 @@ def run_poisson(a):
     F = torch.randn((n, n, n), generator=gen, device="cuda", dtype=torch.float32)
     F -= F.mean()
     phi = torch.zeros_like(F)
-    s = dh.Multigrid(n, n, n, 1.0 / n, dtype=torch.float32, cycle=a.mg_cycle)
+    s = dh.Multigrid(n, n, n, 1.0 / n, dtype=torch.float32, cycle=a.mg_cycle, subtree=a.mg_subtree)
     for _ in range(W):
         s.cycle(phi, F)
     phi.zero_()

@@ -293,7 +293,9 @@ enum {
   DH_MG_GAMMA = 2,      /* 1 V-cycle (default), 2 W-cycle (the paper's default for gravity) */
   DH_MG_NU_COARSE = 3,  /* Jacobi sweeps on the coarsest level, default 64 */
   DH_MG_OMEGA = 4,      /* Jacobi weight, default 2/3 */
-  DH_MG_GRAPH = 5       /* 1 (default) / 0: replay each cycle as a CUDA graph captured once per (phi, F, options) */
+  DH_MG_GRAPH = 5,      /* 1 (default) / 0: replay each cycle as a CUDA graph captured once per (phi, F, options) */
+  DH_MG_SUBTREE = 6     /* 1 (default) / 0: a level of <= 4096 cells and every level below it run as ONE kernel (one block, all
+                           levels in shared memory) instead of one launch per operator: same operators, same order of operations */
 };
 
 dh_mg* dh_mg_create(int nx, int ny, int nz, double h, int dtype);   /* NULL on failure (dh_last_error) */

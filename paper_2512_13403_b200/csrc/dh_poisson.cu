@@ -13,11 +13,12 @@
 //                               residual never reaches HBM (algorithmic 2 words per fine cell + 1/8 written)
 //   mg_prolong_add_kernel       phi += P e2h: one thread per coarse cell writes its 2x2x2 children (27 coarse reads from
 //                               L1 / L2; algorithmic 2 words per fine cell + 1/8 read)
+//   mg_subtree_kernel           a level of <= 4096 cells and all levels below it in ONE block (DH_MG_SUBTREE, default)
 //   mg_coarse_kernel            the coarsest level in ONE block: nu_coarse sweeps in shared memory (<= 1024 cells)
 //   mg_sum_kernel / mg_sum_finish_kernel / mg_shift_kernel   deterministic mean (fixed-order two-stage sum in fp64)
 //   mg_resnorm_kernel           |F - A phi|^2 and |F|^2 for the reported relative residual (two-stage, deterministic)
 // A cycle is captured once into a CUDA graph per (phi, F) pointer pair: the coarse levels are launch bound (a W-cycle
-// at 512^3 is ~1000 launches, most of them on grids of a few thousand cells).
+// at 512^3 is 1786 launches one per operator, 218 with the coarse levels in one block: mg_subtree_kernel).
 #include <cstdio>
 #include <vector>
 
@@ -180,6 +181,191 @@ __global__ void __launch_bounds__(1024) mg_coarse_kernel(T* out, const T* init, 
   if (on) out[t] = v;
 }
 
+// ----------------------------------------------- the coarse levels of a cycle in ONE block (DH_MG_SUBTREE)
+// A level of <= MG_SUB_MAX_CELLS cells and everything below it (16^3, 8^3, 4^3, 2^3 for power-of-two grids) is pure launch
+// latency as separate kernels: a W-cycle at 512^3 visits the 16^3 level 32 times and the levels below it 2, 4, 8 times per
+// visit (1600 launches of 1786).  This kernel runs that whole sub-cycle - the same operators, per cell in the same order of
+// operations as the kernels above - with every level's iterate, right-hand side and Jacobi scratch in shared memory
+// (3 x 4681 words for 16^3: 56 KB fp32, 112 KB fp64) and one block barrier per operator.  Level index L is a template
+// parameter, so the level pointers live in registers.
+constexpr int MG_SUB_MAX_CELLS = 4096;
+constexpr int MG_SUB_MAX_LEV = 6;
+
+struct MgSub {
+  int nlev;
+  int nx[MG_SUB_MAX_LEV], ny[MG_SUB_MAX_LEV], nz[MG_SUB_MAX_LEV];
+  double h2[MG_SUB_MAX_LEV];          // h_l^2
+  int nu1, nu2, gamma, nu_coarse;
+  double omega;
+};
+
+template <class T>
+struct MgSubMem {
+  T* x[MG_SUB_MAX_LEV];               // iterate (may swap roles with s)
+  T* s[MG_SUB_MAX_LEV];               // Jacobi scratch
+  T* r[MG_SUB_MAX_LEV];               // right-hand side
+};
+
+template <class T>
+__device__ __forceinline__ void sub_sweep(T* out, const T* in, const T* F, int nx, int ny, int nz, T c0, T c1, T h2, bool zero_in) {
+  const int n = nx * ny * nz;
+  for (int t = threadIdx.x; t < n; t += blockDim.x) {
+    const T f = F[t];
+    T o;
+    if (zero_in) {
+      o = -c1 * h2 * f;
+    } else {
+      const int i = t % nx, j = (t / nx) % ny, k = t / (nx * ny);
+      const int row = (k * ny + j) * nx;
+      const T sum = ((in[row + wrp(i - 1, nx)] + in[row + wrp(i + 1, nx)]) +
+                     (in[(k * ny + wrp(j - 1, ny)) * nx + i] + in[(k * ny + wrp(j + 1, ny)) * nx + i])) +
+                    (in[(wrp(k - 1, nz) * ny + j) * nx + i] + in[(wrp(k + 1, nz) * ny + j) * nx + i]);
+      o = c0 * in[t] + c1 * (sum - h2 * f);
+    }
+    out[t] = o;
+  }
+  __syncthreads();
+}
+
+template <class T>
+__device__ __forceinline__ void sub_smooth(T*& x, T*& sc, const T* F, int nx, int ny, int nz, T c0, T c1, T h2, int nu, bool from_zero) {
+  for (int q = 0; q < nu; ++q) {
+    sub_sweep<T>(sc, x, F, nx, ny, nz, c0, c1, h2, from_zero && q == 0);
+    T* tmp = x; x = sc; sc = tmp;
+  }
+}
+
+template <class T>
+__device__ __forceinline__ void sub_residual_restrict(T* rc, const T* phi, const T* F, int nx, int ny, int nz, T inv_h2) {
+  const int cx = nx >> 1, cy = ny >> 1, cz = nz >> 1, nc = cx * cy * cz;
+  for (int t = threadIdx.x; t < nc; t += blockDim.x) {
+    const int I = t % cx, J = (t / cx) % cy, K = t / (cx * cy);
+    const int i = 2 * I, im = wrp(i - 1, nx), ip = wrp(i + 2, nx);
+    T acc = T(0);
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk) {
+#pragma unroll
+      for (int dj = 0; dj < 2; ++dj) {
+        const int j = 2 * J + dj, k = 2 * K + dk;
+        const int row = (k * ny + j) * nx;
+        const int rym = (k * ny + wrp(j - 1, ny)) * nx, ryp = (k * ny + wrp(j + 1, ny)) * nx;
+        const int rzm = (wrp(k - 1, nz) * ny + j) * nx, rzp = (wrp(k + 1, nz) * ny + j) * nx;
+        const T c0 = phi[row + i], c1 = phi[row + i + 1];
+        const T s0 = ((phi[row + im] + c1) + (phi[rym + i] + phi[ryp + i])) + (phi[rzm + i] + phi[rzp + i]);
+        const T s1 = ((c0 + phi[row + ip]) + (phi[rym + i + 1] + phi[ryp + i + 1])) + (phi[rzm + i + 1] + phi[rzp + i + 1]);
+        acc += (F[row + i] - (s0 - T(6) * c0) * inv_h2) + (F[row + i + 1] - (s1 - T(6) * c1) * inv_h2);
+      }
+    }
+    rc[t] = T(0.125) * acc;
+  }
+  __syncthreads();
+}
+
+template <class T>
+__device__ __forceinline__ void sub_prolong_add(T* phi, const T* e, int nx, int ny, int nz) {
+  const int cx = nx >> 1, cy = ny >> 1, cz = nz >> 1, nc = cx * cy * cz;
+  for (int t = threadIdx.x; t < nc; t += blockDim.x) {
+    const int I = t % cx, J = (t / cx) % cy, K = t / (cx * cy);
+    const int Is[3] = {wrp(I - 1, cx), I, wrp(I + 1, cx)};
+    const int Js[3] = {wrp(J - 1, cy), J, wrp(J + 1, cy)};
+    const int Ks[3] = {wrp(K - 1, cz), K, wrp(K + 1, cz)};
+    T x0[3][3], x1[3][3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+#pragma unroll
+      for (int b = 0; b < 3; ++b) {
+        const T* r = e + (Ks[a] * cy + Js[b]) * cx;
+        const T m = r[Is[0]], c = r[Is[1]], p = r[Is[2]];
+        x0[a][b] = T(0.75) * c + T(0.25) * m;
+        x1[a][b] = T(0.75) * c + T(0.25) * p;
+      }
+#pragma unroll
+    for (int dk = 0; dk < 2; ++dk)
+#pragma unroll
+      for (int dj = 0; dj < 2; ++dj) {
+        const int kn = dk ? 2 : 0, jn = dj ? 2 : 0;
+        const T y0c = T(0.75) * x0[1][1] + T(0.25) * x0[1][jn], y0n = T(0.75) * x0[kn][1] + T(0.25) * x0[kn][jn];
+        const T y1c = T(0.75) * x1[1][1] + T(0.25) * x1[1][jn], y1n = T(0.75) * x1[kn][1] + T(0.25) * x1[kn][jn];
+        const int o = ((2 * K + dk) * ny + (2 * J + dj)) * nx + 2 * I;
+        phi[o] += T(0.75) * y0c + T(0.25) * y0n;
+        phi[o + 1] += T(0.75) * y1c + T(0.25) * y1n;
+      }
+  }
+  __syncthreads();
+}
+
+// one cycle on sub-level L for A x = r[L], starting from x[L] (zero if from_zero); every thread of the block takes the same path
+template <class T, int L>
+__device__ void sub_cycle(MgSubMem<T>& m, const MgSub& sp, bool from_zero) {
+  const int nx = sp.nx[L], ny = sp.ny[L], nz = sp.nz[L], n = nx * ny * nz;
+  const T c0 = (T)(1.0 - sp.omega), c1 = (T)(sp.omega / 6.0), h2 = (T)sp.h2[L];
+  if (L == sp.nlev - 1) {                               // coarsest level (reading A22)
+    if (sp.nu_coarse == 0) {
+      if (from_zero) {
+        for (int t = threadIdx.x; t < n; t += blockDim.x) m.x[L][t] = T(0);
+        __syncthreads();
+      }
+      return;
+    }
+    if (n <= 32) {
+      // a grid of at most one warp (2^3 for power-of-two grids): warp 0 sweeps alone with warp barriers, the block waits once
+      if (threadIdx.x < 32) {
+        T* a = m.x[L];
+        T* b = m.s[L];
+        const int t = threadIdx.x;
+        const bool on = t < n;
+        const int i = on ? t % nx : 0, j = on ? (t / nx) % ny : 0, k = on ? t / (nx * ny) : 0;
+        const int row = (k * ny + j) * nx;
+        const int n0 = row + wrp(i - 1, nx), n1 = row + wrp(i + 1, nx), n2 = (k * ny + wrp(j - 1, ny)) * nx + i,
+                  n3 = (k * ny + wrp(j + 1, ny)) * nx + i, n4 = (wrp(k - 1, nz) * ny + j) * nx + i, n5 = (wrp(k + 1, nz) * ny + j) * nx + i;
+        const T f = on ? m.r[L][t] : T(0);
+        for (int q = 0; q < sp.nu_coarse; ++q) {
+          if (on) b[t] = (from_zero && q == 0) ? -c1 * h2 * f : c0 * a[t] + c1 * ((((a[n0] + a[n1]) + (a[n2] + a[n3])) + (a[n4] + a[n5])) - h2 * f);
+          __syncwarp();
+          T* tmp = a; a = b; b = tmp;
+        }
+      }
+      if (sp.nu_coarse & 1) { T* tmp = m.x[L]; m.x[L] = m.s[L]; m.s[L] = tmp; }
+      __syncthreads();
+      return;
+    }
+    sub_smooth<T>(m.x[L], m.s[L], m.r[L], nx, ny, nz, c0, c1, h2, sp.nu_coarse, from_zero);
+    return;
+  }
+  if constexpr (L + 1 < MG_SUB_MAX_LEV) {
+    sub_smooth<T>(m.x[L], m.s[L], m.r[L], nx, ny, nz, c0, c1, h2, sp.nu1, from_zero);
+    if (from_zero && sp.nu1 == 0) {
+      for (int t = threadIdx.x; t < n; t += blockDim.x) m.x[L][t] = T(0);
+      __syncthreads();
+    }
+    sub_residual_restrict<T>(m.r[L + 1], m.x[L], m.r[L], nx, ny, nz, (T)(1.0 / sp.h2[L]));
+    for (int v = 0; v < sp.gamma; ++v) sub_cycle<T, L + 1>(m, sp, v == 0);
+    sub_prolong_add<T>(m.x[L], m.x[L + 1], nx, ny, nz);
+    sub_smooth<T>(m.x[L], m.s[L], m.r[L], nx, ny, nz, c0, c1, h2, sp.nu2, false);
+  }
+}
+
+template <class T>
+__global__ void __launch_bounds__(1024) mg_subtree_kernel(T* x_g, const T* __restrict__ F_g, const MgSub sp, const int from_zero) {
+  extern __shared__ __align__(16) unsigned char mg_sub_smem[];
+  MgSubMem<T> m;
+  T* q = reinterpret_cast<T*>(mg_sub_smem);
+#pragma unroll
+  for (int l = 0; l < MG_SUB_MAX_LEV; ++l) {
+    const int n = l < sp.nlev ? sp.nx[l] * sp.ny[l] * sp.nz[l] : 0;
+    m.x[l] = q; m.s[l] = q + n; m.r[l] = q + 2 * n;
+    q += 3 * n;
+  }
+  const int n0 = sp.nx[0] * sp.ny[0] * sp.nz[0];
+  for (int t = threadIdx.x; t < n0; t += blockDim.x) {
+    m.r[0][t] = F_g[t];
+    if (!from_zero) m.x[0][t] = x_g[t];
+  }
+  __syncthreads();
+  sub_cycle<T, 0>(m, sp, from_zero != 0);
+  for (int t = threadIdx.x; t < n0; t += blockDim.x) x_g[t] = m.x[0][t];
+}
+
 // ------------------------------------------------------------------ deterministic sums (fp64, fixed order)
 constexpr int SUM_BLOCKS = 592, SUM_THREADS = 256;   // 4 blocks per SM
 
@@ -253,6 +439,7 @@ struct dh_mg {
   int nu1, nu2, gamma, nu_coarse;
   double omega;
   int use_graph;
+  int subtree;                         // DH_MG_SUBTREE: levels of <= 4096 cells and everything below them in one block
   int nlev;
   std::vector<int> lx, ly, lz;         // extents per level
   std::vector<void*> e, r, t;          // per level >= 1: error, right-hand side, Jacobi scratch; level 0: t only
@@ -320,6 +507,34 @@ cudaError_t cycle_rec(dh_mg* c, int l, void** px, void** pscratch, const void* F
   cudaError_t e;
   const int nx = c->lx[l], ny = c->ly[l], nz = c->lz[l];
   const double hl = c->h * (double)(1 << l);
+  if (c->subtree && l < c->nlev - 1 && cells(c, l) <= (size_t)MG_SUB_MAX_CELLS && c->nlev - l <= MG_SUB_MAX_LEV) {
+    // this level and everything below it in one block (mg_subtree_kernel)
+    MgSub sp;
+    sp.nlev = c->nlev - l;
+    size_t words = 0;
+    for (int q = 0; q < MG_SUB_MAX_LEV; ++q) {
+      const bool in = q < sp.nlev;
+      sp.nx[q] = in ? c->lx[l + q] : 0; sp.ny[q] = in ? c->ly[l + q] : 0; sp.nz[q] = in ? c->lz[l + q] : 0;
+      const double hq = c->h * (double)(1 << (l + q));
+      sp.h2[q] = hq * hq;
+      if (in) words += 3 * cells(c, l + q);
+    }
+    sp.nu1 = c->nu1; sp.nu2 = c->nu2; sp.gamma = c->gamma; sp.nu_coarse = c->nu_coarse; sp.omega = c->omega;
+    const size_t smem = words * sizeof(T);
+    static bool configured[64] = {};                 // per (T, device): the opt-in to > 48 KB of dynamic shared memory
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
+      e = cudaFuncSetAttribute((const void*)mg_subtree_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               (int)(3 * 4681 * sizeof(T)));
+      if (e != cudaSuccess) return e;
+      if (dev >= 0 && dev < 64) configured[dev] = true;
+    }
+    // 512 threads: 1024 / 512 / 256 / 128 measured 5.03 / 4.95 / 5.06 / 5.41 ms per W-cycle at 512^3 (the block is latency bound)
+    mg_subtree_kernel<T><<<1, 512, smem, c->ls>>>((T*)*px, (const T*)F, sp, from_zero ? 1 : 0);
+    c->launches += 1;
+    return cudaGetLastError();
+  }
   if (l == c->nlev - 1) {                          // coarsest level (reading A22)
     if (cells(c, l) <= 1024 && c->nu_coarse >= 1) {
       mg_coarse_kernel<T><<<1, 1024, 0, c->ls>>>((T*)*px, from_zero ? nullptr : (const T*)*px, (const T*)F, nx, ny, nz,
@@ -374,7 +589,7 @@ int cycle_top(dh_mg* c, void* phi, const void* F) {
 template <class T>
 int cycle_graph(dh_mg* c, void* phi, const void* F) {
   if (!c->use_graph) return cycle_top<T>(c, phi, F);
-  const int key[5] = {c->nu1, c->nu2, c->gamma, c->nu_coarse, (int)(c->omega * 1e9)};
+  const int key[5] = {c->nu1, c->nu2, c->gamma + 16 * c->subtree, c->nu_coarse, (int)(c->omega * 1e9)};
   bool same = c->graph && c->g_phi == phi && c->g_F == F;
   for (int q = 0; q < 5; ++q) same = same && c->g_key[q] == key[q];
   if (!same) {
@@ -458,7 +673,7 @@ dh_mg* dh_mg_create(int nx, int ny, int nz, double h, int dtype) {
   }
   dh_mg* c = new dh_mg();
   c->n[0] = nx; c->n[1] = ny; c->n[2] = nz; c->h = h; c->dtype = dtype; c->stream = 0; c->ls = 0; c->cap = nullptr;
-  c->nu1 = 2; c->nu2 = 2; c->gamma = 1; c->nu_coarse = 64; c->omega = 2.0 / 3.0; c->use_graph = 1;
+  c->nu1 = 2; c->nu2 = 2; c->gamma = 1; c->nu_coarse = 64; c->omega = 2.0 / 3.0; c->use_graph = 1; c->subtree = 1;
   c->F0 = nullptr; c->partial = nullptr; c->result = nullptr; c->result_host = nullptr; c->launches = 0;
   c->graph = nullptr; c->g_phi = nullptr; c->g_F = nullptr; c->g_launches = 0;
   int x = nx, y = ny, z = nz;
@@ -512,6 +727,7 @@ int dh_mg_set_option(dh_mg* c, int key, double v) {
     case DH_MG_NU_COARSE: if (!whole || v < 0 || v > 4096) return mg_fail(DH_ERR_ARG, "dh_mg_set_option: nu_coarse must be an integer in 0 .. 4096"); c->nu_coarse = (int)v; break;
     case DH_MG_OMEGA: if (!(v > 0.0 && v <= 1.0)) return mg_fail(DH_ERR_ARG, "dh_mg_set_option: omega must be in (0, 1]"); c->omega = v; break;
     case DH_MG_GRAPH: c->use_graph = (v != 0.0); break;
+    case DH_MG_SUBTREE: c->subtree = (v != 0.0); break;
     default: return mg_fail(DH_ERR_ARG, "dh_mg_set_option: unknown key");
   }
   return DH_OK;

@@ -40,7 +40,7 @@ SYMBOLS = [
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
     "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
 ]
-MG_OPTIONS = {"nu1": 0, "nu2": 1, "gamma": 2, "nu_coarse": 3, "omega": 4, "graph": 5}
+MG_OPTIONS = {"nu1": 0, "nu2": 1, "gamma": 2, "nu_coarse": 3, "omega": 4, "graph": 5, "subtree": 6}
 MG_CYCLES = {"V": 1, "W": 2}
 KERNEL_KINDS = ["cfl_reduce", "cfl_finish", "stage1", "stage2", "rev2", "rev1", "cool_vjp", "lincomb", "cool", "cfl_cand"]
 

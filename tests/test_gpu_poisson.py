@@ -94,6 +94,33 @@ def test_cycle_options_and_graph_replay(dtype):
     assert sa.launches == sb.launches > 0
 
 
+@pytest.mark.parametrize("cycle", ["V", "W"])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("shape", [(64, 64, 64), (16, 16, 16), (32, 16, 64), (24, 48, 96), (16, 8, 24), (64, 8, 8)],
+                         ids=lambda s: "x".join(map(str, s)))
+def test_coarse_levels_in_one_block_equal_the_launch_sequence(shape, dtype, cycle):
+    """DH_MG_SUBTREE: a level of <= 4096 cells and everything below it as ONE kernel (levels in shared memory, the one-warp
+    coarsest grid swept by warp 0 alone) against one launch per operator: the same operators in the same order of
+    operations, so the results agree to rounding of differently contracted expressions (1e-14 / 2e-6 of the maximum), with
+    far fewer launches; and both agree with the oracle (64^3: two levels of launches above the 16^3 subtree)."""
+    h = 1.0 / shape[2]
+    kw = dict(nu1=2, nu2=3, nu_coarse=9)                   # odd sweep counts: the iterate changes buffers inside the block
+    F, phi = _rand(shape, 41, dtype), _rand(shape, 42, dtype, zero_mean=False)
+    sa, sb = _solver(shape, h, dtype, cycle=cycle, subtree=1, **kw), _solver(shape, h, dtype, cycle=cycle, subtree=0, **kw)
+    a, b, Fd = phi.cuda(), phi.cuda(), F.cuda()
+    ref = phi.numpy().astype(np.float64)
+    for _ in range(2):
+        sa.cycle(a, Fd)
+        sb.cycle(b, Fd)
+        ref = mg.cycle(ref, F.numpy().astype(np.float64), h, gamma={"V": 1, "W": 2}[cycle], **kw)
+    assert _err(a.cpu().numpy(), b.cpu().numpy()) <= (1e-14 if dtype == torch.float64 else 2e-6)
+    assert _err(a.cpu().numpy(), ref) <= TOL[dtype] * (1 if dtype == torch.float64 else 4)
+    assert sa.launches < sb.launches
+    if shape == (64, 64, 64) and cycle == "W":
+        # levels 64^3, 32^3 by launches: (1 + 2) x (5 sweeps + restrict + prolong) + 4 visits of the 16^3 subtree
+        assert sa.launches == 2 * (3 * 7 + 4)
+
+
 @pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
 @pytest.mark.parametrize("shape", [(32, 32, 32), (12, 24, 48)], ids=lambda s: "x".join(map(str, s)))
 def test_solve_matches_oracle_and_the_fft_definition(shape, dtype):
