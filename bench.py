@@ -65,6 +65,9 @@ def parse_args():
                     help="instead of the hydro step: time multigrid cycles of the periodic Poisson solver on an N^3 grid (SURVEY 8(f) item 3)")
     ap.add_argument("--mg-cycle", choices=["V", "W"], default="V")
     ap.add_argument("--mg-subtree", type=int, default=1, help="DH_MG_SUBTREE: 1 (default) the levels of <= 4096 cells in one block, 0 one launch per operator")
+    ap.add_argument("--issue-probe", action="store_true",
+                    help="instead of the hydro step: dh_issue_probe, the issue cost of the instruction mixes the stage kernels are made of "
+                         "(SM cycles per group per scheduler at 2 and 4 warps per scheduler; DESIGN.md section 7b)")
     ap.add_argument("--no-vjp", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
@@ -103,6 +106,32 @@ def committed_capture(n: int):
                          "commit": e.get("commit"), "predictor": e["predictor"], "corrector": e["corrector"]}
     except Exception:
         return None, None
+
+
+def issue_bound(counters: dict, ms_per_launch: float, clocks: dict, N: int, peak: float):
+    """The issue-port reading of the stage kernel (profiles/r02d_issue_bound.md): executed warp instructions of the
+    committed ncu capture x the issue-port cycles per instruction that `sass_cost` derives from the kernel's SASS under the rule that
+    `dh_issue_probe` measures (max(1, register operands read / 2) cycles per instruction), against the port cycles this run's launch had
+    (schedulers x measured time x the SM clock sampled during the run).  A cost model over hardware counters: `kind` says so."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            m = json.load(f)["issue_model"]
+        mhz = float(clocks.get("sm_mhz") or 0.0) if isinstance(clocks, dict) else 0.0
+        ghz = mhz / 1e3 if mhz > 0 else float(m["sm_clock_ghz"])
+        ports = m["schedulers_per_sm"] * m["sm_count"]
+        need = 0.0
+        for stage in ("predictor", "corrector"):
+            cpi = m[stage]["static_issue_cycles"] / m[stage]["static_instructions"]
+            need += 0.5 * counters[stage]["warp_instructions"] * cpi          # average over the two launches, like `achieved`
+        have = ports * ms_per_launch * 1e-3 * ghz * 1e9
+        hbm_ms = 0.5 * (STAGE_WORDS["stage1"] + STAGE_WORDS["stage2"]) * 4.0 * N / (peak * 1e9) * 1e3
+        return {"kind": "cost model (measured per-instruction issue cost x executed-instruction counter of the committed capture)",
+                "rule": m["rule"], "issue_port_cycles_needed_per_launch": need, "issue_port_cycles_available_per_launch": have,
+                "utilisation": need / have, "lane_issue_cycles_per_cell_stage": need * 32.0 / N,
+                "ms_per_launch_at_full_utilisation": ms_per_launch * need / have,
+                "hbm_frac_at_full_utilisation": hbm_ms / (ms_per_launch * need / have)}
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -269,7 +298,8 @@ def run_dh(a):
                   lambda0=wl.lambda0, alpha=wl.alpha, t_floor=wl.t_floor, integrator=a.integrator, riemann=a.riemann, limiter=a.limiter,
                   cool_mode=a.cool_mode, cool_nsub=a.cool_nsub, c_cool=a.c_cool)
     # algorithmic words per cell of one step: CFL 5 + per stage (5 in [+ 5 base] + 5 out) + per combination 15
-    fwd_words = {"vl2": FWD_WORDS, "heun": 5 + 10 + 15, "ssprk3": 5 + 10 + 15 + 15}[a.integrator]   # the combinations are formed inside the stage kernel
+    # words per cell and step with a full CFL pass (5) in front; the combinations of Heun / SSPRK3 are formed inside the stage kernel
+    fwd_words = {"vl2": 5 + FWD_WORDS, "heun": 5 + 10 + 15, "ssprk3": 5 + 10 + 15 + 15}[a.integrator]
 
     def barrier():
         if world > 1:
@@ -370,6 +400,9 @@ def run_dh(a):
                 "step_bytes_note": f"{fwd_words - 5} words/cell/step + 5 words/cell for each of the {full_passes} full CFL passes in the {K} timed steps"}
     if counters is not None:
         roofline["counters"] = counters
+        issue = issue_bound(counters, st_ms / max(st_cnt, 1), clocks, N, peak)
+        if issue is not None:
+            roofline["issue"] = issue
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_fwd / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
@@ -586,9 +619,27 @@ def run_poisson(a):
     print(json.dumps(line))
 
 
+def run_issue_probe(a):
+    """A measurement, not a benchmark of the path: prints one JSON line with the dh_issue_probe table."""
+    import torch
+    from paper_2512_13403_b200 import dh
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --issue-probe needs a GPU")
+    torch.cuda.set_device(0)
+    rows = {}
+    for wps in (2, 4):
+        for r in dh.issue_probe(warps_per_scheduler=wps, iters=4000):
+            e = rows.setdefault(r["mix"], {"instructions": r["instructions"]})
+            e[f"cycles_per_group_{wps}_warps"] = round(r["cycles_per_group"], 3)
+    print(json.dumps({"metric": "issue cost of instruction mixes (dh_issue_probe)", "unit": "SM cycles per group per scheduler",
+                      "device": torch.cuda.get_device_name(0), "chains_per_thread": 8, "mixes": rows}))
+
+
 def main():
     a = parse_args()
-    if a.poisson:
+    if a.issue_probe:
+        run_issue_probe(a)
+    elif a.poisson:
         run_poisson(a)
     elif a.impl == "reference":
         run_reference(a)

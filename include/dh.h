@@ -337,6 +337,19 @@ int dh_step_gravity(dh_ctx* ctx, dh_mg* mg, void* U, double dt, double four_pi_g
  * solve, Eqs. 46-48) and the hydro step (dh_step_vjp).  U = U^n (pre-step); gU_in overwritten, must not alias U or gU_out. */
 int dh_step_gravity_vjp(dh_ctx* ctx, dh_mg* mg, const void* U, double dt, double four_pi_g, int ncycles, const void* gU_out, void* gU_in);
 
+/* ---- Diagnostics (measurements; not part of the path) ----
+ * dh_issue_probe times one short instruction mix of the kind the stage kernels consist of (half-rate ALU-pipe FMNMX / LOP3 / FSEL,
+ * scalar FADD / FFMA, the packed FADD2 / FMUL2 / FFMA2 of sm_100 in the operand forms the kernels use, alone and combined) on every
+ * SM of the current device, with `warps_per_scheduler` (1..4) warps per SM sub-partition and 8 independent chains per thread, and
+ * returns the SM cycles (clock64, worst block) per instruction group per scheduler in *cycles_per_group (HOST) and the number of
+ * instructions of a group in *instructions_per_group (HOST or NULL).  DESIGN.md section 7b derives the issue bound of
+ * stage_fused2_kernel from this table (`python bench.py --issue-probe`; profiles/r02d_issue_bound.md).  Allocates and frees a few
+ * KB of device memory and synchronises the device.  mix in [0, DH_ISSUE_PROBE_MIXES); dh_issue_probe_name(mix) is a static string
+ * naming the group (NULL for an unknown mix). */
+#define DH_ISSUE_PROBE_MIXES 24
+int dh_issue_probe(int mix, int warps_per_scheduler, int iters, double* cycles_per_group, int* instructions_per_group);
+const char* dh_issue_probe_name(int mix);
+
 #ifdef __cplusplus
 }
 #endif

@@ -58,6 +58,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     extra = ["-Xptxas", "-v"] if verbose else []
+    extra += os.environ.get("DH_BUILD_DEFINES", "").split()      # e.g. -DDH_TIMING_PROBE (csrc/dh_fused2_impl.cuh)
 
     def compile_one(src: str):
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + f".{os.getpid()}.o")

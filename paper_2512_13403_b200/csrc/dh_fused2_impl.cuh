@@ -25,10 +25,22 @@
 // One translation unit per Riemann flux (dh_fused2.cu HLLC, dh_fused2_hll.cu, dh_fused2_rusanov.cu) includes this file
 // and instantiates launch_stage_fused2_rs<T, RS, COMBO>; they compile side by side.
 #pragma once
+#include <cstdio>
 #include "dh_internal.cuh"
 #include "dh_pack.cuh"
 
 namespace dh {
+
+// -DDH_TIMING_PROBE (DH_BUILD_DEFINES=-DDH_TIMING_PROBE python -m paper_2512_13403_b200.build --force): lane 0 of every warp
+// of block (1, 1, 0) prints the SM cycles it spends in plane 40 of its sweep, from the top of the loop body to its arrival
+// at the block barrier (profiles/r02d_issue_bound.md).  Compiled out otherwise.
+#ifdef DH_TIMING_PROBE
+#define DH_PROBE_BEGIN const bool prb_ = blockIdx.x == 1 && blockIdx.y == 1 && blockIdx.z == 0 && it == 40 && lane == 0; long long prb_t0 = 0; if (prb_) prb_t0 = clock64();
+#define DH_PROBE_END(tag) if (prb_) printf("probe warp %2d %s start %lld cycles %lld\n", w, tag, prb_t0, clock64() - prb_t0);
+#else
+#define DH_PROBE_BEGIN
+#define DH_PROBE_END(tag)
+#endif
 
 namespace {
 
@@ -146,6 +158,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
 
 #pragma unroll 1
     for (int it = 0; it < nit; ++it) {
+      DH_PROBE_BEGIN
       const int bp = it & 1, bq = bp ^ 1;
       T* const Wp_s = Wsm + bp * G::PLANE;
       const T* const Wq_s = Wsm + bq * G::PLANE;
@@ -301,6 +314,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       opm1 = op;
       op = opn;
       pz = pzn;
+      DH_PROBE_END("row")
       __syncthreads();
     }
   } else {
@@ -331,6 +345,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
 
 #pragma unroll 1
     for (int it = 0; it < nit; ++it) {
+      DH_PROBE_BEGIN
       const int bp = it & 1, bq = bp ^ 1;
       T* const Wp_s = Wsm + bp * G::PLANE;
       const T* const Wq_s = Wsm + bq * G::PLANE;
@@ -407,6 +422,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
       if (pzn == nz) { pzn = 0; opn = 0; }
       op = opn;
       pz = pzn;
+      DH_PROBE_END("helper")
       __syncthreads();
     }
   }

@@ -38,7 +38,7 @@ SYMBOLS = [
     "dh_cfl_stats", "dh_cool_tmin", "dh_set_cooling_table", "dh_cool_table_vjp",
     "dh_cfl_dt_static", "dh_static_max_cells", "dh_gravity_source", "dh_gravity_source_vjp", "dh_step_gravity", "dh_step_gravity_vjp",
     "dh_mg_create", "dh_mg_destroy", "dh_mg_set_stream", "dh_mg_set_option", "dh_mg_levels", "dh_mg_launches",
-    "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp",
+    "dh_mg_cycle", "dh_mg_solve", "dh_mg_solve_vjp", "dh_issue_probe", "dh_issue_probe_name",
 ]
 MG_OPTIONS = {"nu1": 0, "nu2": 1, "gamma": 2, "nu_coarse": 3, "omega": 4, "graph": 5, "subtree": 6}
 MG_CYCLES = {"V": 1, "W": 2}
@@ -81,6 +81,10 @@ def load(rebuild: bool = False):
     lib.dh_cfl_dt_static.restype = ci
     lib.dh_static_max_cells.argtypes = []
     lib.dh_static_max_cells.restype = ctypes.c_size_t
+    lib.dh_issue_probe.argtypes = [ci, ci, ci, pd, ctypes.POINTER(ci)]
+    lib.dh_issue_probe.restype = ci
+    lib.dh_issue_probe_name.argtypes = [ci]
+    lib.dh_issue_probe_name.restype = ctypes.c_char_p
     lib.dh_stream_host.restype = ci
     lib.dh_advance.argtypes = [vp, vp, ci, pd]
     lib.dh_adjoint.argtypes = [vp, vp, vp, ci, ci, pd]
@@ -186,6 +190,20 @@ def dh_cfl_dt_static(U_ptr: int, nx: int, ny: int, nz: int, dtype: int, gamma: f
 
 def dh_static_max_cells() -> int:
     return int(load().dh_static_max_cells())
+
+
+ISSUE_PROBE_MIXES = 24
+
+
+def issue_probe(warps_per_scheduler: int = 4, iters: int = 4000) -> list[dict]:
+    """dh_issue_probe for every mix: SM cycles per instruction group per scheduler (a measurement)."""
+    lib = load()
+    out = []
+    for mix in range(ISSUE_PROBE_MIXES):
+        cyc, n = ctypes.c_double(0.0), ctypes.c_int(0)
+        _check(lib.dh_issue_probe(mix, int(warps_per_scheduler), int(iters), ctypes.byref(cyc), ctypes.byref(n)))
+        out.append({"mix": lib.dh_issue_probe_name(mix).decode(), "instructions": n.value, "cycles_per_group": cyc.value})
+    return out
 
 
 def dh_cfl_dt_async(ctx, U_ptr: int) -> None:
