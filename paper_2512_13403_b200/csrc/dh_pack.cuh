@@ -112,8 +112,8 @@ DH_DI T limit1(T a, T b) {
 template <class T, int LIM>
 DH_DI P2<T> limit2(P2<T> a, P2<T> b) { return {limit1<T, LIM>(a.x, b.x), limit1<T, LIM>(a.y, b.y)}; }
 
-// HLLC flux of two faces with normal axis AX (Eq. A3 for the wave speeds); the same
-// arrangement as hllc() in dh_math.cuh: star state on the upwind side only, supersonic branches folded
+// HLLC flux of two faces with normal axis AX (Eq. A3 for the wave speeds); the
+// arrangement of hllc() in dh_math.cuh (up to H_K = E_K + P_K being formed in one piece here): star state on the upwind side only, supersonic branches folded
 // into S_eff = min(S_L, 0) / max(S_R, 0), transverse momentum flux = v_t * F_mass, one rsqrt per sound
 // speed (c = gP * rsqrt(gP * rho)), E_K formed without a density reciprocal.
 template <class T, int AX>
@@ -135,7 +135,9 @@ DH_DI void hllc2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F
   const P2<T> PK = sel2(left, L[4], R[4]), aK = sel2(left, aL, aR), dK = sel2(left, dL, dR);
   const P2<T> Seff = sel2(left, min2(SL, T(0)), max2(SR, T(0)));   // 0 in the supersonic branches -> F = F_K
   const P2<T> q = fma2(v2, v2, fma2(v1, v1, mul2(uK, uK)));
-  const P2<T> EK = fma2(mul2(bc2(T(0.5)), rhoK), q, mul2(bc2(c.inv_gm1), PK));
+  // H_K = E_K + P_K in one piece (gamma / (gamma - 1) = 1 + 1 / (gamma - 1)): E_K alone is never needed, and both places that
+  // used it added P_K (two packed additions per face pair fewer)
+  const P2<T> HK = fma2(mul2(bc2(T(0.5)), rhoK), q, mul2(bc2(c.inv_gm1 + T(1)), PK));
   const P2<T> mK = mul2(rhoK, uK);
   const P2<T> Y = sub2(Ss, uK);
   // star-state jumps in terms of w = (S* - u_K) / (S_K - S*):  rho* - rho = rho w,  (rho u)* - rho u = rho (Y + w S*),
@@ -144,12 +146,12 @@ DH_DI void hllc2(const P2<T> L[5], const P2<T> R[5], const Consts<T>& c, P2<T> F
   const P2<T> w = mul2(Y, rcp2(sub2(dK, Y)));
   const P2<T> t = mul2(Seff, rhoK);
   const P2<T> Fm = fma2(t, w, mK);
-  const P2<T> ZE = add2(fma2(aK, Ss, PK), EK);
+  const P2<T> ZE = fma2(aK, Ss, HK);
   F[0] = Fm;
   F[n] = fma2(t, fma2(w, Ss, Y), fma2(mK, uK, PK));
   F[t1] = mul2(v1, Fm);
   F[t2] = mul2(v2, Fm);
-  F[4] = fma2(mul2(Seff, w), ZE, mul2(uK, add2(EK, PK)));
+  F[4] = fma2(mul2(Seff, w), ZE, mul2(uK, HK));
 }
 
 // HLL (RS = 1) and Rusanov (RS = 2) fluxes of two faces (wave speeds of Eq. A3), the arrangement of
