@@ -85,9 +85,9 @@ template <int N> DH_DI void cp_async_wait2() { asm volatile("cp.async.wait_group
 template <class T, int LIM>
 DH_DI void recon_x2(P2<T> W, T wl, T wr, P2<T>& L, P2<T>& R) {
   const T d0 = W.x - wl, d1 = W.y - W.x, d2 = wr - W.y;
-  const P2<T> s = {limit1<T, LIM>(d1, d0), limit1<T, LIM>(d2, d1)};
-  L = fma2(bc2(T(0.5)), s, W);
-  R = fma2(bc2(T(-0.5)), s, W);
+  const P2<T> s = {limit1s<T, LIM>(d1, d0), limit1s<T, LIM>(d2, d1)};
+  L = fma2(bc2(T(0.5) / SlopeScale<T, LIM>::k), s, W);
+  R = fma2(bc2(T(-0.5) / SlopeScale<T, LIM>::k), s, W);
 }
 
 }  // namespace
@@ -118,7 +118,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
   const P2<T> ncx = bc2(-tau * p.inv_dx[0]);
   const P2<T> cy = bc2(tau * p.inv_dx[1]), ncy = bc2(-tau * p.inv_dx[1]);
   const P2<T> cz = bc2(tau * p.inv_dx[2]), ncz = bc2(-tau * p.inv_dx[2]);
-  const P2<T> half = bc2(T(0.5)), nhalf = bc2(T(-0.5));
+  const P2<T> half = bc2(T(0.5) / SlopeScale<T, LIM>::k), nhalf = bc2(T(-0.5) / SlopeScale<T, LIM>::k);   // of the scaled slopes (limit2s)
   const Consts<T>& c = p.c;
   const T cand_thr = CAND ? p.cand_thr[0] : T(0);   // CAND: push the CFL candidates of the result (dh_advance)
   constexpr bool combo = COMBO;                     // out = wB B + wX U - tau D(U): the base state is formed here
@@ -212,7 +212,7 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
         P2<T> Rz[5], Fz[5], s[5];                                                                   \
         _Pragma("unroll") for (int f = 0; f < 5; ++f) {                                             \
           const P2<T> a = sub2(N_[f], W_[f]);                                                       \
-          s[f] = limit2<T, LIM>(a, d_[f]);                                                          \
+          s[f] = limit2s<T, LIM>(a, d_[f]);                                                          \
           Rz[f] = fma2(nhalf, s[f], W_[f]);                                                         \
           d_[f] = a;                                                                                \
         }                                                                                           \
@@ -290,9 +290,9 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
           const T* col = Wq_s + f * FP + soA;
           const P2<T> Wm = lds2_(col - SW2), W2 = lds2_(col + 2 * SW2), W3 = lds2_(col + 3 * SW2);
           const P2<T> dBA = sub2(WB[f], WA[f]), d2B = sub2(W2, WB[f]);
-          const P2<T> sA = limit2<T, LIM>(dBA, sub2(WA[f], Wm));
-          const P2<T> sB = limit2<T, LIM>(d2B, dBA);
-          const P2<T> s2 = limit2<T, LIM>(sub2(W3, W2), d2B);
+          const P2<T> sA = limit2s<T, LIM>(dBA, sub2(WA[f], Wm));
+          const P2<T> sB = limit2s<T, LIM>(d2B, dBA);
+          const P2<T> s2 = limit2s<T, LIM>(sub2(W3, W2), d2B);
           L1[f] = fma2(half, sA, WA[f]);
           R1[f] = fma2(nhalf, sB, WB[f]);
           L2[f] = fma2(half, sB, WB[f]);
@@ -367,8 +367,8 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
           const T* col = Wq_s + f * FP + 2 * lane + 2;
           const P2<T> Wm2 = lds2_(col), Wm1 = lds2_(col + SW2), W0 = lds2_(col + 2 * SW2), W1 = lds2_(col + 3 * SW2);
           const P2<T> d0 = sub2(W0, Wm1);
-          const P2<T> sm = limit2<T, LIM>(d0, sub2(Wm1, Wm2));
-          const P2<T> s0 = limit2<T, LIM>(sub2(W1, W0), d0);
+          const P2<T> sm = limit2s<T, LIM>(d0, sub2(Wm1, Wm2));
+          const P2<T> s0 = limit2s<T, LIM>(sub2(W1, W0), d0);
           L[f] = fma2(half, sm, Wm1);
           R[f] = fma2(nhalf, s0, W0);
         }
@@ -401,11 +401,11 @@ stage_fused2_kernel(const StageParams<T> p, const int ZL) {
           const T nx_ = __shfl_down_sync(0xffffffffu, Wh[f].x, 1), ny_ = __shfl_down_sync(0xffffffffu, Wh[f].y, 1);
           const T pv_ = __shfl_up_sync(0xffffffffu, Wh[f].y, 1);
           const T dl = Wh[f].y - Wh[f].x, dc = nx_ - Wh[f].y, dr = ny_ - nx_;
-          const T sl = limit1<T, LIM>(dc, dl), sc = limit1<T, LIM>(dr, dc);
-          L[f] = bc2(fma_(T(0.5), sl, Wh[f].y));
-          R[f] = bc2(fma_(T(-0.5), sc, nx_));
-          const T se = limit1<T, LIM>(dl, Wh[f].x - pv_);
-          Re[f] = fma_(T(-0.5), se, Wh[f].x);
+          const T sl = limit1s<T, LIM>(dc, dl), sc = limit1s<T, LIM>(dr, dc);
+          L[f] = bc2(fma_(T(0.5) / SlopeScale<T, LIM>::k, sl, Wh[f].y));
+          R[f] = bc2(fma_(T(-0.5) / SlopeScale<T, LIM>::k, sc, nx_));
+          const T se = limit1s<T, LIM>(dl, Wh[f].x - pv_);
+          Re[f] = fma_(T(-0.5) / SlopeScale<T, LIM>::k, se, Wh[f].x);
         }
         riemann2<T, 0, RS>(L, R, c, F);
         if (live && kind == 0) {

@@ -60,6 +60,15 @@ DH_DI float minmod_(float a, float b) {
   d = fmaxf(d, 0.0f);
   return __uint_as_float(__float_as_uint(d) | (__float_as_uint(a) & 0x80000000u));
 }
+// twice minmod(a, b): the clamp at zero as d + |d| (= 2 d or +0, exact) on the FMA pipe instead of max(d, 0) on the half-rate ALU
+// pipe; the face states take the factor back (W +- 0.25 s2 is bit for bit W +- 0.5 s: scaling by a power of two is exact).
+// The fused forward kernel is bound by its math-pipe cycles: one ALU instruction (two cycles) becomes one FADD (one).
+DH_DI float minmod2x_(float a, float b) {
+  float d;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));
+  d = __fadd_rn(d, fabsf(d));
+  return __uint_as_float(__float_as_uint(d) | (__float_as_uint(a) & 0x80000000u));
+}
 DH_DI double minmod_(double a, double b) {
   const double mn = fmin(a, b), mx = fmax(a, b);
   return fmin(fmax(mn, 0.0), mx);
@@ -111,6 +120,16 @@ DH_DI T limit1(T a, T b) {
 }
 template <class T, int LIM>
 DH_DI P2<T> limit2(P2<T> a, P2<T> b) { return {limit1<T, LIM>(a.x, b.x), limit1<T, LIM>(a.y, b.y)}; }
+// the limited slope scaled by SlopeScale<T, LIM>::k (fp32 minmod: 2, see minmod2x_; everything else: 1); a face state is
+// W +- (0.5 / k) s
+template <class T, int LIM> struct SlopeScale { static constexpr int k = (LIM == 0 && sizeof(T) == 4) ? 2 : 1; };
+template <class T, int LIM>
+DH_DI T limit1s(T a, T b) {
+  if constexpr (LIM == 0 && sizeof(T) == 4) return minmod2x_(a, b);
+  else return limit1<T, LIM>(a, b);
+}
+template <class T, int LIM>
+DH_DI P2<T> limit2s(P2<T> a, P2<T> b) { return {limit1s<T, LIM>(a.x, b.x), limit1s<T, LIM>(a.y, b.y)}; }
 
 // HLLC flux of two faces with normal axis AX (Eq. A3 for the wave speeds); the
 // arrangement of hllc() in dh_math.cuh (up to H_K = E_K + P_K being formed in one piece here): star state on the upwind side only, supersonic branches folded
