@@ -31,22 +31,18 @@ NO_DEST = {"STS", "STG", "ST", "STL", "BAR", "BRA", "LDGSTS", "BSYNC", "BSSY", "
 
 def disassemble(lib: str, kernel: str) -> list[tuple[int, str]]:
     """(address, text) of every instruction of the first function whose mangled name contains `kernel`."""
-    out = subprocess.run(["cuobjdump", "-sass", lib], capture_output=True, text=True, check=True).stdout
-    ins: list[tuple[int, str]] = []
-    inside = False
-    for line in out.splitlines():
-        m = re.match(r"\s*Function : (\S+)", line)
-        if m:
-            if inside:
-                break
-            inside = kernel in m.group(1)
-            continue
-        if inside:
-            m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(.*?);", line)
-            if m:
-                ins.append((int(m.group(1), 16), m.group(2).strip()))
-    if not ins:
+    names = subprocess.run(["cuobjdump", "-res-usage", lib], capture_output=True, text=True, check=True).stdout
+    full = next((m.group(1) for m in re.finditer(r"Function (\S+?):", names) if kernel in m.group(1)), None)
+    if full is None:
         raise SystemExit(f"no function containing '{kernel}' in {lib}")
+    out = subprocess.run(["cuobjdump", "-sass", "-fun", full, lib], capture_output=True, text=True).stdout
+    ins: list[tuple[int, str]] = []
+    for line in out.splitlines():
+        m = re.match(r"\s+/\*([0-9a-f]{4,})\*/\s+(.*?);", line)
+        if m:
+            ins.append((int(m.group(1), 16), m.group(2).strip()))
+    if not ins:
+        raise SystemExit(f"cuobjdump printed no SASS for {full}")
     return ins
 
 
